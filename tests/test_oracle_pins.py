@@ -1,0 +1,405 @@
+"""Pins for the CPU oracle (oracle/cans_oracle.py): everything here checks the oracle against
+something OTHER than itself -- matrices assembled in this file from the 7-point stencil of eq. 5
+ and the ghost-cell rules, scipy/LAPACK routines, closed forms and invariants of
+eqs. 2b-2c.  No GPU needed."""
+import itertools
+
+import numpy as np
+import pytest
+import scipy.fft
+import scipy.linalg
+
+from oracle import cans_oracle as orc
+
+PAIRS_XY = ["PP", "NN", "DD", "ND", "DN"]
+PAIRS_Z = ["NN", "DD", "ND", "DN", "PP"]
+
+
+# ----------------------------------------------------------------------------------------------
+# independent assembly of the operator from the stencil + ghost rules (written out here, not
+# imported): neighbour outside the range -> wrap (P), +self (N), -self (D)
+# ----------------------------------------------------------------------------------------------
+def second_difference_1d(n, pair, lo_coef=None, up_coef=None):
+    """n x n matrix of  lo_k*(phi_{k-1}-phi_k) + up_k*(phi_{k+1}-phi_k)  with ghost rules."""
+    lo_coef = np.ones(n) if lo_coef is None else lo_coef
+    up_coef = np.ones(n) if up_coef is None else up_coef
+    M = np.zeros((n, n))
+    for k in range(n):
+        for off, coef, side in ((-1, lo_coef[k], 0), (+1, up_coef[k], 1)):
+            M[k, k] -= coef
+            kk = k + off
+            if 0 <= kk < n:
+                M[k, kk] += coef
+            elif pair == "PP":
+                M[k, kk % n] += coef
+            elif pair[side] == "N":
+                M[k, k] += coef
+            elif pair[side] == "D":
+                M[k, k] -= coef
+            else:
+                raise AssertionError
+    return M
+
+
+def stretched(nz, lz, a):
+    """Independent tanh grid for the tests (faces mapped, centres = midpoints)."""
+    Z = np.arange(nz + 1) / nz
+    zf = 0.5 * (1 + np.tanh(a * (Z - 0.5)) / np.tanh(a / 2)) * lz
+    dzf = np.diff(zf)
+    zc = 0.5 * (zf[1:] + zf[:-1])
+    dzc = np.empty(nz + 1)
+    dzc[1:nz] = np.diff(zc)
+    dzc[0] = dzf[0]
+    dzc[nz] = dzf[-1]
+    return dzc, dzf
+
+
+def laplacian_matrix(nx, ny, nz, lx, ly, lz, bc, dzc, dzf):
+    """Dense (N x N) matrix of eq. 5 on the x-fastest ordering, from Kronecker sums of the 1-D
+    stencil matrices above (z: lo = 1/(dzf dzc_k), up = 1/(dzf dzc_{k+1}))."""
+    px, py, pz = (b[0] + b[1] for b in bc)
+    Lx = second_difference_1d(nx, px) / (lx / nx) ** 2
+    Ly = second_difference_1d(ny, py) / (ly / ny) ** 2
+    Lz = second_difference_1d(nz, pz, 1.0 / (dzf * dzc[:nz]), 1.0 / (dzf * dzc[1:]))
+    Ix, Iy, Iz = np.eye(nx), np.eye(ny), np.eye(nz)
+    return (np.kron(Iz, np.kron(Iy, Lx)) + np.kron(Iz, np.kron(Ly, Ix)) + np.kron(Lz, np.kron(Iy, Ix)))
+
+
+def bc_of(px, py, pz):
+    return ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+
+
+# ----------------------------------------------------------------------------------------------
+# 1-D tables (O2)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("pair", PAIRS_XY)
+@pytest.mark.parametrize("n", [2, 5, 8, 12, 33])
+def test_basis_diagonalises_stencil(pair, n):
+    B, lam, w = orc.basis(pair, n)
+    L = second_difference_1d(n, pair)
+    assert np.max(np.abs(L @ B.T - B.T * lam[None, :])) < 5e-14
+    assert np.max(np.abs((B.T * w[None, :]) @ B - np.eye(n))) < 5e-15 * n
+    assert np.all(lam <= 0)
+
+
+@pytest.mark.parametrize("n", [8, 12, 768, 1024])
+def test_basis_matches_scipy_transforms(n):
+    rng = np.random.default_rng(n)
+    x = rng.standard_normal(n)
+    scale = np.sqrt(n)
+    B, _, _ = orc.basis("NN", n)
+    assert np.max(np.abs(2 * B @ x - scipy.fft.dct(x, type=2))) < 2e-14 * scale * 2
+    B, _, _ = orc.basis("DD", n)
+    assert np.max(np.abs(2 * B @ x - scipy.fft.dst(x, type=2))) < 2e-14 * scale * 2
+    B, _, _ = orc.basis("ND", n)
+    assert np.max(np.abs(2 * B @ x - scipy.fft.dct(x, type=4))) < 2e-14 * scale * 2
+    B, _, _ = orc.basis("DN", n)
+    assert np.max(np.abs(2 * B @ x - scipy.fft.dst(x, type=4))) < 2e-14 * scale * 2
+    B, _, _ = orc.basis("PP", n)
+    X = np.fft.rfft(x)
+    got = B @ x
+    nc = n // 2 + 1
+    assert np.max(np.abs(got[:nc] - X.real)) < 2e-14 * scale
+    assert np.max(np.abs(got[nc:] + X.imag[1:(n + 1) // 2])) < 2e-14 * scale
+
+
+def test_inverse_weights_roundtrip_odd_even():
+    for pair, n in itertools.product(PAIRS_XY, [7, 16]):
+        B, _, w = orc.basis(pair, n)
+        x = np.random.default_rng(1).standard_normal(n)
+        assert np.max(np.abs((B.T * w) @ (B @ x) - x)) < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------
+# Thomas (O3) against LAPACK
+# ----------------------------------------------------------------------------------------------
+def test_thomas_vs_banded_random_dominant():
+    rng = np.random.default_rng(3)
+    nz = 200
+    a = rng.uniform(0.5, 2.0, nz)
+    c = rng.uniform(0.5, 2.0, nz)
+    b = -(a + c) - rng.uniform(0.01, 3.0, nz)
+    d = rng.standard_normal((nz, 4, 3))
+    x = orc.thomas(a, b[:, None, None] * np.ones((1, 4, 3)), c, d)
+    ab = np.zeros((3, nz))
+    ab[0, 1:] = c[:-1]
+    ab[1] = b
+    ab[2, :-1] = a[1:]
+    ref = scipy.linalg.solve_banded((1, 1), ab, d.reshape(nz, -1)).reshape(d.shape)
+    assert np.max(np.abs(x - ref)) / np.max(np.abs(ref)) < 1e-13
+
+
+def test_thomas_near_singular_low_mode():
+    # stretched 512-point grid, small shift: cond ~ 3e6.  Thomas (no pivoting) and LAPACK's pivoted
+    # banded LU are two correct algorithms; both sit ~1e-12 from a long-double solve, so the bound is
+    # a small multiple of cond*eps: 3e-18*cond (1e-11 at cond 3e6, 1e-15 floor).
+    nz = 512
+    dzc, dzf = stretched(nz, 2.0, 2.0)
+    a, b, c = orc.z_matrix_rows("NN", dzc, dzf)
+    rng = np.random.default_rng(5)
+    d = rng.standard_normal((nz, 1))
+    for lam in (-0.25, -1.0, -2.7e4):
+        x = orc.thomas(a, (b + lam)[:, None], c, d)
+        ab = np.zeros((3, nz))
+        ab[0, 1:] = c[:-1]
+        ab[1] = b + lam
+        ab[2, :-1] = a[1:]
+        ref = scipy.linalg.solve_banded((1, 1), ab, d)
+        M = np.diag(b + lam) + np.diag(a[1:], -1) + np.diag(c[:-1], 1)
+        tol = max(1e-15, 3e-18 * np.linalg.cond(M))
+        assert np.linalg.norm(x - ref) / np.linalg.norm(ref) < tol
+
+
+def test_z_rows_match_stencil_matrix():
+    nz = 9
+    dzc, dzf = stretched(nz, 1.3, 1.7)
+    for pz in ("NN", "DD", "ND", "DN"):
+        a, b, c = orc.z_matrix_rows(pz, dzc, dzf)
+        M = np.diag(b) + np.diag(a[1:], -1) + np.diag(c[:-1], 1)
+        ref = second_difference_1d(nz, pz, 1.0 / (dzf * dzc[:nz]), 1.0 / (dzf * dzc[1:]))
+        assert np.max(np.abs(M - ref)) < 1e-12 * np.max(np.abs(ref))
+
+
+# ----------------------------------------------------------------------------------------------
+# the operator (O1) and the whole solve (O2-O5) against dense LU, every boundary combination
+# ----------------------------------------------------------------------------------------------
+def _dense_reference(M, f, singular, dzf, shape):
+    nz, ny, nx = shape
+    if not singular:
+        return np.linalg.solve(M, f.ravel()).reshape(shape)
+    # bordered system [L 1; wT 0][phi; mu] = [f; 0] with w = cell volumes (dzf weights)
+    wvec = np.repeat(dzf, ny * nx)
+    N = M.shape[0]
+    A = np.zeros((N + 1, N + 1))
+    A[:N, :N] = M
+    A[:N, N] = 1.0
+    A[N, :N] = wvec
+    rhs = np.concatenate([f.ravel(), [0.0]])
+    sol = np.linalg.solve(A, rhs)
+    return sol[:N].reshape(shape)
+
+
+@pytest.mark.parametrize("grid", ["uniform", "stretched"])
+def test_solve_vs_dense_lu_all_boundary_combinations(grid):
+    nx, ny, nz = 8, 8, 8
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    if grid == "uniform":
+        dzc, dzf = orc.uniform_spacing(nz, lz)
+    else:
+        dzc, dzf = stretched(nz, lz, 1.6)
+    rng = np.random.default_rng(11)
+    worst = 0.0
+    for px, py, pz in itertools.product(PAIRS_XY, PAIRS_XY, PAIRS_Z):
+        bc = bc_of(px, py, pz)
+        M = laplacian_matrix(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        f = rng.uniform(-1, 1, (nz, ny, nx))
+        singular = orc.is_singular(bc)
+        assert singular == all(p in ("PP", "NN") for p in (px, py, pz))
+        if singular:
+            f -= np.sum(f * dzf[:, None, None]) / (np.sum(dzf) * nx * ny)   # compatibility (S3)
+        # pin O1: the oracle's operator equals the independently assembled matrix
+        phi_r = rng.standard_normal((nz, ny, nx))
+        lap = orc.apply_laplacian(phi_r, lx, ly, lz, bc, dzc, dzf)
+        assert np.max(np.abs(lap.ravel() - M @ phi_r.ravel())) < 1e-11
+        # pin O2-O5
+        phi = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        ref = _dense_reference(M, f, singular, dzf, (nz, ny, nx))
+        err = np.max(np.abs(phi - ref)) / max(np.max(np.abs(ref)), 1e-300)
+        worst = max(worst, err)
+        assert err < 2e-12, (px, py, pz, err)
+        if singular:
+            assert abs(np.sum(phi * dzf[:, None, None])) < 1e-12
+    assert worst < 2e-12
+
+
+def test_solve_vs_dense_lu_ragged_sizes():
+    # non-power-of-two, all different extents: catches transposed operands / swapped axes
+    nx, ny, nz = 6, 5, 7
+    lx, ly, lz = 1.0, 2.5, 0.7
+    dzc, dzf = stretched(nz, lz, 2.0)
+    rng = np.random.default_rng(12)
+    for px, py, pz in [("PP", "NN", "DN"), ("DD", "PP", "NN"), ("ND", "DN", "DD"), ("NN", "NN", "NN"),
+                       ("PP", "PP", "PP")]:
+        bc = bc_of(px, py, pz)
+        M = laplacian_matrix(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        f = rng.uniform(-1, 1, (nz, ny, nx))
+        singular = orc.is_singular(bc)
+        if singular:
+            f -= np.sum(f * dzf[:, None, None]) / (np.sum(dzf) * nx * ny)
+        phi = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        ref = _dense_reference(M, f, singular, dzf, (nz, ny, nx))
+        assert np.max(np.abs(phi - ref)) / np.max(np.abs(ref)) < 2e-12
+
+
+# ----------------------------------------------------------------------------------------------
+# eigenmodes: f = X_q (x) Y_r (x) Z_s  =>  Phi = f / (lam_q/dx^2 + lam_r/dy^2 + mu_s)   (eq. 6)
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("px,py,pz,a", [("PP", "PP", "NN", 1.6), ("NN", "NN", "DN", None),
+                                        ("PP", "DD", "NN", 2.0), ("DD", "NN", "DD", None)])
+def test_eigenmode_solution_is_f_over_lambda(px, py, pz, a):
+    nx, ny, nz = 24, 18, 20
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc, dzf = orc.uniform_spacing(nz, lz) if a is None else stretched(nz, lz, a)
+    # z eigenpairs from LAPACK on the symmetrised stencil matrix (independent of the oracle's tables)
+    Tz = second_difference_1d(nz, pz, 1.0 / (dzf * dzc[:nz]), 1.0 / (dzf * dzc[1:]))
+    D = np.diag(dzf)
+    mu, Zs = scipy.linalg.eigh(D @ Tz, D)
+    Lx = second_difference_1d(nx, px)
+    Ly = second_difference_1d(ny, py)
+    lamx, Xs = np.linalg.eigh(Lx)
+    lamy, Ys = np.linalg.eigh(Ly)
+    rng = np.random.default_rng(17)
+    bc = bc_of(px, py, pz)
+    for _ in range(6):
+        q, r, s = rng.integers(nx), rng.integers(ny), rng.integers(nz)
+        lam = lamx[q] / (lx / nx) ** 2 + lamy[r] / (ly / ny) ** 2 + mu[s]
+        if abs(lam) < 1e-9:
+            continue
+        f = Zs[:, s][:, None, None] * Ys[:, r][None, :, None] * Xs[:, q][None, None, :]
+        f /= np.max(np.abs(f))
+        phi = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        assert np.max(np.abs(phi - f / lam)) < 1e-11 * np.max(np.abs(f / lam))
+
+
+# ----------------------------------------------------------------------------------------------
+# residual / backward error at a size with several hundred modes per direction
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("px,py,pz,a", [("PP", "PP", "NN", 1.5), ("NN", "NN", "DN", None),
+                                        ("PP", "DD", "NN", 2.0), ("DN", "ND", "ND", 1.2)])
+def test_residual_below_1e12(px, py, pz, a):
+    nx, ny, nz = 96, 80, 64
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc, dzf = orc.uniform_spacing(nz, lz) if a is None else stretched(nz, lz, a)
+    bc = bc_of(px, py, pz)
+    rng = np.random.default_rng(23)
+    f = rng.uniform(-1, 1, (nz, ny, nx))
+    if orc.is_singular(bc):
+        f -= np.sum(f * dzf[:, None, None]) / (np.sum(dzf) * nx * ny)
+    phi = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+    res = orc.apply_laplacian(phi, lx, ly, lz, bc, dzc, dzf) - f
+    assert np.linalg.norm(res) / np.linalg.norm(f) < 1e-12          # white-noise RHS (S13)
+    # normwise backward error with |L||phi| from the independently assembled 1-D matrices
+    Lx = np.abs(second_difference_1d(nx, px)) / (lx / nx) ** 2
+    Ly = np.abs(second_difference_1d(ny, py)) / (ly / ny) ** 2
+    Lz = np.abs(second_difference_1d(nz, pz, 1.0 / (dzf * dzc[:nz]), 1.0 / (dzf * dzc[1:])))
+    ap = np.abs(phi)
+    absl = ap @ Lx.T + np.einsum("rj,kjq->krq", Ly, ap) + np.einsum("sk,kjq->sjq", Lz, ap)
+    assert np.linalg.norm(res) / (np.linalg.norm(absl) + np.linalg.norm(f)) < 1e-12
+
+
+def test_uniform_z_matches_full_3d_spectral_closed_form():
+    # on a uniform grid the z direction diagonalises too: Phi^ = f^ / (lx+ly+lz), a closed form that
+    # never touches the Thomas recurrence
+    nx, ny, nz = 20, 12, 16
+    lx, ly, lz = 1.0, 2.0, 3.0
+    rng = np.random.default_rng(29)
+    for px, py, pz in [("PP", "NN", "DD"), ("DD", "PP", "ND"), ("NN", "DN", "DN")]:
+        bc = bc_of(px, py, pz)
+        f = rng.standard_normal((nz, ny, nx))
+        Lx = second_difference_1d(nx, px) / (lx / nx) ** 2
+        Ly = second_difference_1d(ny, py) / (ly / ny) ** 2
+        Lz = second_difference_1d(nz, pz) / (lz / nz) ** 2
+        ex, Vx = np.linalg.eigh(Lx)
+        ey, Vy = np.linalg.eigh(Ly)
+        ez, Vz = np.linalg.eigh(Lz)
+        fh = np.einsum("kjq,qa->kja", f, Vx)
+        fh = np.einsum("kja,jb->kba", fh, Vy)
+        fh = np.einsum("kba,kc->cba", fh, Vz)
+        fh /= ez[:, None, None] + ey[None, :, None] + ex[None, None, :]
+        ref = np.einsum("cba,kc->kba", fh, Vz)
+        ref = np.einsum("kba,jb->kja", ref, Vy)
+        ref = np.einsum("kja,qa->kjq", ref, Vx)
+        phi = orc.poisson_solve(f, lx, ly, lz, bc)
+        assert np.max(np.abs(phi - ref)) < 1e-12 * np.max(np.abs(ref))
+
+
+# ----------------------------------------------------------------------------------------------
+# divergence / gradient (O6): D G = L, and the projection invariants of eqs. 2b-2c
+# ----------------------------------------------------------------------------------------------
+def _gradient_via_correction(phi, lx, ly, lz, bc, dzc, dzf, faces):
+    nz, ny, nx = phi.shape
+    z = np.zeros_like(phi)
+    un, vn, wn, fn = orc.correct_velocity(z, z, z, phi, -1.0, lx, ly, lz, bc, dzc, dzf, faces)
+    return un, vn, wn, fn
+
+
+@pytest.mark.parametrize("px,py,pz", list(itertools.product(["PP", "NN", "DD", "ND", "DN"],
+                                                             ["PP", "DN"], ["NN", "DD", "ND", "DN", "PP"])))
+def test_div_of_grad_is_the_laplacian(px, py, pz):
+    nx, ny, nz = 6, 4, 5
+    lx, ly, lz = 1.1, 0.9, 1.7
+    dzc, dzf = stretched(nz, lz, 1.4)
+    bc = bc_of(px, py, pz)
+    rng = np.random.default_rng(31)
+    phi = rng.standard_normal((nz, ny, nx))
+    faces = {}
+    shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+    for d, p in enumerate((px, py, pz)):
+        if p[0] == "D":
+            faces[d] = np.zeros(shapes[d])
+    gu, gv, gw, gf = _gradient_via_correction(phi, lx, ly, lz, bc, dzc, dzf, faces)
+    div = orc.divergence(gu, gv, gw, lx, ly, lz, bc, dzc, dzf, gf)
+    M = laplacian_matrix(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    assert np.max(np.abs(div.ravel() - M @ phi.ravel())) < 1e-11
+
+
+@pytest.mark.parametrize("px,py,pz", [("PP", "PP", "NN"), ("PP", "NN", "NN"), ("NN", "NN", "NN"),
+                                      ("PP", "PP", "ND"), ("PP", "DD", "NN"), ("NN", "NN", "DN")])
+def test_projection_invariants(px, py, pz):
+    nx, ny, nz = 24, 16, 20
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc, dzf = stretched(nz, lz, 1.6)
+    bc = bc_of(px, py, pz)
+    rng = np.random.default_rng(37)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    faces = {}
+    shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+    pairs = (px, py, pz)
+    for d, p in enumerate(pairs):
+        if p[0] == "D":
+            faces[d] = rng.standard_normal(shapes[d])
+    # closed (upper 'N') boundary faces carry no flow so that the singular problems are compatible
+    if px[1] == "N":
+        u[:, :, -1] = 0
+    if py[1] == "N":
+        v[:, -1, :] = 0
+    if pz[1] == "N":
+        w[-1] = 0
+    dt = 1e-2
+    un, vn, wn, phi, fn = orc.projection(u, v, w, dt, lx, ly, lz, bc, dzc, dzf, faces)
+    # (i) discretely divergence free
+    div = orc.divergence(un, vn, wn, lx, ly, lz, bc, dzc, dzf, fn)
+    assert np.max(np.abs(div)) < 1e-11 * np.max(np.abs(u)) / min(lx / nx, ly / ny, dzf.min())
+    # (ii) idempotent
+    u2, v2, w2, phi2, _ = orc.projection(un, vn, wn, dt, lx, ly, lz, bc, dzc, dzf, fn)
+    assert np.max(np.abs(dt * phi2)) < 1e-11
+    assert np.max(np.abs(u2 - un)) < 1e-11
+    # (v) upper 'N' boundary faces unchanged exactly
+    if px[1] == "N":
+        assert np.array_equal(un[:, :, -1], u[:, :, -1])
+    if py[1] == "N":
+        assert np.array_equal(vn[:, -1, :], v[:, -1, :])
+    if pz[1] == "N":
+        assert np.array_equal(wn[-1], w[-1])
+
+
+def test_projection_annihilates_pure_gradient_and_keeps_poiseuille():
+    nx, ny, nz = 16, 12, 24
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc, dzf = stretched(nz, lz, 1.6)
+    bc = bc_of("PP", "PP", "NN")
+    rng = np.random.default_rng(41)
+    psi = rng.standard_normal((nz, ny, nx))
+    dt = 1e-3
+    z = np.zeros_like(psi)
+    gu, gv, gw, _ = orc.correct_velocity(z, z, z, psi, -dt, lx, ly, lz, bc, dzc, dzf)   # u* = dt G psi
+    un, vn, wn, phi, _ = orc.projection(gu, gv, gw, dt, lx, ly, lz, bc, dzc, dzf)
+    scale = np.max(np.abs(gu))
+    assert max(np.max(np.abs(un)), np.max(np.abs(vn)), np.max(np.abs(wn))) < 1e-11 * scale
+    wmean = np.sum(psi * dzf[:, None, None]) / (np.sum(dzf) * nx * ny)
+    assert np.max(np.abs(phi - (psi - wmean))) < 1e-10 * np.max(np.abs(psi))
+    # (iv) a Poiseuille profile u(z) is already solenoidal: returned unchanged with Phi ~ 0
+    zc = np.cumsum(dzf) - 0.5 * dzf
+    up = np.broadcast_to((6 * (zc / lz) * (1 - zc / lz))[:, None, None], (nz, ny, nx)).copy()
+    un, vn, wn, phi, _ = orc.projection(up, z, z, dt, lx, ly, lz, bc, dzc, dzf)
+    assert np.max(np.abs(un - up)) < 1e-14 and np.max(np.abs(dt * phi)) < 1e-13
