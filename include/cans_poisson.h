@@ -1,0 +1,129 @@
+/*
+ * cans_poisson.h -- C ABI of the B200-native FP64 pressure-projection library.
+ *
+ * What the library computes (citations: /root/reference/PAPER.md, "P:L<n>" = line n):
+ *
+ *   eq. 2b  P:L59    L Phi = D u* / (gamma_k dt)           divergence of the staggered velocity
+ *   eq. 5   P:L95    7-point second-order Laplacian        the linear system
+ *   eq. 6   P:L102   F^x, F^y, tridiagonal in z            eigenfunction-expansion direct solve
+ *   P:L98-100        "Gauss elimination" along z           Thomas solve per (kx, ky) mode
+ *   P:L104           z may be non-uniform                  dzc / dzf arrays
+ *   eq. 2c  P:L62    u^{k+1} = u* - gamma_k dt G Phi       pressure-gradient correction
+ *
+ * Every step runs in hand-written sm_100a CUDA kernels on the device the caller made current;
+ * there is no CPU fallback and no other backend.  All floating point is FP64.
+ *
+ * Layout: every field is a DEVICE pointer to nx*ny*nz contiguous doubles, x fastest
+ * (linear index i + nx*(j + ny*k); a torch tensor of shape (nz, ny, nx)), no halo,
+ * 16-byte aligned, owned by the caller; the library never frees or retains it.
+ * Staggering (marker-and-cell): u[i,j,k] lives on the +x face of cell (i,j,k), v on the
+ * +y face, w on the +z face.  Out-of-range neighbours are synthesised from `bc`.
+ *
+ * Threading: calls only enqueue work on `stream` (a cudaStream_t passed as void*) and never
+ * synchronise.  A plan is immutable after creation apart from the registered lower-face planes;
+ * it may be used by one stream at a time.  No function throws or prints.
+ */
+#ifndef CANS_POISSON_H
+#define CANS_POISSON_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the library */
+
+/* Return codes of the int-valued entry points. */
+#define CANS_OK                    0
+#define CANS_ERR_INVALID_ARG       1   /* null pointer, n < 2, non-positive length/spacing/dt, bad bc letter, one-sided 'P' */
+#define CANS_ERR_UNSUPPORTED_BC    2   /* boundary pair the kernels do not implement yet (see cans_poisson_plan_create) */
+#define CANS_ERR_UNSUPPORTED_SIZE  3   /* nx or ny not in the instantiated transform sizes, or nz too large */
+#define CANS_ERR_ALLOC             4   /* device or host allocation failed */
+#define CANS_ERR_CUDA              5   /* a CUDA runtime call or kernel launch failed */
+#define CANS_ERR_NEEDS_FACE        6   /* projection with a lower 'D' side needs cans_projection_set_lower_face */
+
+/*
+ * cans_poisson_plan_create -- build the plan for L Phi = f (eqs. 5-6).
+ *
+ *   nx, ny, nz   cells per direction (x, y uniform: "uniformly-spaced in two directions").
+ *                nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048;
+ *                2 <= nz <= 1024.
+ *   lx, ly, lz   domain lengths (> 0); dx = lx/nx, dy = ly/ny.
+ *   bc           bc[d][0] / bc[d][1] = PRESSURE boundary condition on the lower / upper face of
+ *                direction d (0 = x, 1 = y, 2 = z), homogeneous, imposed at the boundary face:
+ *                'P' periodic (both sides), 'N' dPhi/dn = 0, 'D' Phi = 0.
+ *                Implemented: x, y in {PP, NN, DD}; z in {NN, DD, ND, DN}.
+ *                Mixed N/D pairs in x, y and periodic z return NULL with CANS_ERR_UNSUPPORTED_BC.
+ *   dzc          HOST, nz+1 doubles: dzc[k] = distance between the centres of cells k-1 and k
+ *                (k = 0 and k = nz reach the mirror ghost centres), or NULL.
+ *   dzf          HOST, nz doubles: dzf[k] = width of cell k, or NULL.  Both NULL => uniform lz/nz.
+ *                The arrays are copied; the caller keeps ownership.
+ *
+ * Returns NULL on failure; cans_last_error()/cans_last_status() tell why.
+ * The plan owns O(nx + ny + nz + nx*ny*nz/16) doubles of device tables; the solve is in place.
+ */
+cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz,
+                                            double lx, double ly, double lz,
+                                            const char bc[3][2],
+                                            const double* dzc, const double* dzf);
+
+/* Free the plan and its device tables.  NULL is ignored.  Outstanding work must have completed. */
+void cans_poisson_plan_destroy(cans_poisson_plan* plan);
+
+/*
+ * cans_poisson_solve -- in-place direct solve of eq. 5 by eq. 6.
+ *   p       DEVICE, nx*ny*nz doubles.  On entry f, on exit Phi with L Phi = f.
+ *           If every direction is PP or NN the operator is singular: f must satisfy
+ *           sum f*dzf = 0 to rounding and the returned Phi has zero dzf-weighted mean
+ *           (the kx = ky = 0 column is solved with its last row dropped, then shifted).
+ *   stream  cudaStream_t as void* (NULL = default stream).
+ */
+int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream);
+
+/*
+ * cans_projection -- one pressure-projection step, eqs. 2b-2c:
+ *     f = D(u,v,w)/dt ;  L Phi = f ;  (u,v,w) -= dt * G Phi.
+ *   u, v, w  DEVICE, corrected in place.
+ *   p        DEVICE, overwritten with Phi (entry contents ignored; eq. 2d is the caller's).
+ *   dt       the whole factor gamma_k*Delta_t of eqs. 2b-2c (> 0).
+ * The boundary-normal velocity on a lower 'P' face is the wrapped value, on a lower 'N' face 0
+ * (or the plane registered with cans_projection_set_lower_face); the value on an upper 'N' face
+ * (array index n-1) is read and left bit-identical.
+ */
+int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, double* p,
+                    double dt, void* stream);
+
+/*
+ * cans_projection_set_lower_face -- register the boundary-normal velocity on the LOWER face of
+ * direction dir (0,1,2): DEVICE plane of (product of the other two extents) doubles, x fastest,
+ * or NULL to unregister.  On a 'D' side the plane is read by the divergence and corrected
+ * (-= dt*2*Phi_0/h); on an 'N' side it is a prescribed inflow and is not modified.
+ * (Not implemented yet: returns CANS_ERR_UNSUPPORTED_BC for a non-NULL plane.)
+ */
+int cans_projection_set_lower_face(cans_poisson_plan* plan, int dir, double* face_plane);
+
+/*
+ * Host-buffer convenience entry points (used for end-to-end timing): copy the HOST arrays to
+ * device buffers owned by the plan (allocated on first use), run the device path on `stream`,
+ * copy the results back and synchronise the stream.  Pinned host memory gives full PCIe rate.
+ */
+int cans_poisson_solve_host(cans_poisson_plan* plan, double* p_host, void* stream);
+int cans_projection_host(cans_poisson_plan* plan, double* u_host, double* v_host, double* w_host,
+                         double* p_host, double dt, void* stream);
+
+/* Thread-local message / status code of the last failure on this thread ("" / CANS_OK if none). */
+const char* cans_last_error(void);
+int cans_last_status(void);
+
+/* Number of kernel launches one cans_poisson_solve / cans_projection call enqueues (for bench.py). */
+int cans_plan_launches_per_solve(const cans_poisson_plan* plan);
+int cans_plan_launches_per_projection(const cans_poisson_plan* plan);
+
+/* "x.y" version string of the library. */
+const char* cans_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CANS_POISSON_H */

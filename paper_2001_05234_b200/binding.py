@@ -1,0 +1,184 @@
+"""Thin ctypes binding of libcans_poisson.so (include/cans_poisson.h) -- argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; torch is used for device memory and
+streams.  If the shared library is missing this module raises at import time: there is no fallback.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcans_poisson.so")
+
+CANS_OK = 0
+CANS_ERR_INVALID_ARG = 1
+CANS_ERR_UNSUPPORTED_BC = 2
+CANS_ERR_UNSUPPORTED_SIZE = 3
+CANS_ERR_ALLOC = 4
+CANS_ERR_CUDA = 5
+CANS_ERR_NEEDS_FACE = 6
+
+EXPORTED_SYMBOLS = (
+    "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
+    "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
+    "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
+    "cans_plan_launches_per_projection", "cans_version",
+)
+
+
+class CansError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"cans_poisson error {status}: {message}")
+        self.status = status
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} not found: build it with `python -m paper_2001_05234_b200.build` "
+            "(nvcc, sm_100a). There is no CPU or library fallback.")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, dbl, i32 = ctypes.c_void_p, ctypes.c_double, ctypes.c_int
+    lib.cans_poisson_plan_create.restype = vp
+    lib.cans_poisson_plan_create.argtypes = [i32, i32, i32, dbl, dbl, dbl, ctypes.c_char_p, vp, vp]
+    lib.cans_poisson_plan_destroy.restype = None
+    lib.cans_poisson_plan_destroy.argtypes = [vp]
+    lib.cans_poisson_solve.restype = i32
+    lib.cans_poisson_solve.argtypes = [vp, vp, vp]
+    lib.cans_projection.restype = i32
+    lib.cans_projection.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
+    lib.cans_projection_set_lower_face.restype = i32
+    lib.cans_projection_set_lower_face.argtypes = [vp, i32, vp]
+    lib.cans_poisson_solve_host.restype = i32
+    lib.cans_poisson_solve_host.argtypes = [vp, vp, vp]
+    lib.cans_projection_host.restype = i32
+    lib.cans_projection_host.argtypes = [vp, vp, vp, vp, vp, dbl, vp]
+    lib.cans_last_error.restype = ctypes.c_char_p
+    lib.cans_last_error.argtypes = []
+    lib.cans_last_status.restype = i32
+    lib.cans_last_status.argtypes = []
+    lib.cans_plan_launches_per_solve.restype = i32
+    lib.cans_plan_launches_per_solve.argtypes = [vp]
+    lib.cans_plan_launches_per_projection.restype = i32
+    lib.cans_plan_launches_per_projection.argtypes = [vp]
+    lib.cans_version.restype = ctypes.c_char_p
+    lib.cans_version.argtypes = []
+    return lib
+
+
+_lib = _load()
+
+
+def version() -> str:
+    return _lib.cans_version().decode()
+
+
+def last_error() -> str:
+    return _lib.cans_last_error().decode()
+
+
+def _check(rc: int):
+    if rc != CANS_OK:
+        raise CansError(rc, last_error())
+
+
+def _bc_bytes(bc) -> bytes:
+    flat = "".join(str(bc[d][s]) for d in range(3) for s in range(2))
+    return flat.encode("ascii")
+
+
+def _dev_ptr(t: torch.Tensor, shape) -> int:
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise ValueError(f"expected a contiguous CUDA float64 tensor of shape {tuple(shape)}")
+    return t.data_ptr()
+
+
+def _host_ptr(t: torch.Tensor, shape) -> int:
+    if t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous() or tuple(t.shape) != tuple(shape):
+        raise ValueError(f"expected a contiguous CPU float64 tensor of shape {tuple(shape)}")
+    return t.data_ptr()
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+class PoissonPlan:
+    """cans_poisson_plan_create / _destroy.  Fields are torch CUDA float64 tensors of shape (nz, ny, nx)."""
+
+    def __init__(self, nx: int, ny: int, nz: int, lx: float, ly: float, lz: float, bc,
+                 dzc: Optional[Sequence[float]] = None, dzf: Optional[Sequence[float]] = None):
+        self.shape = (nz, ny, nx)
+        self._h = None
+        dzc_t = dzf_t = None
+        pc = pf = None
+        if dzc is not None:
+            dzc_t = torch.as_tensor(dzc, dtype=torch.float64, device="cpu").contiguous()
+            if dzc_t.numel() != nz + 1:
+                raise ValueError("dzc must have nz+1 entries")
+            pc = dzc_t.data_ptr()
+        if dzf is not None:
+            dzf_t = torch.as_tensor(dzf, dtype=torch.float64, device="cpu").contiguous()
+            if dzf_t.numel() != nz:
+                raise ValueError("dzf must have nz entries")
+            pf = dzf_t.data_ptr()
+        h = _lib.cans_poisson_plan_create(nx, ny, nz, float(lx), float(ly), float(lz), _bc_bytes(bc), pc, pf)
+        if not h:
+            raise CansError(_lib.cans_last_status(), last_error())
+        self._h = h
+
+    def close(self):
+        if self._h:
+            _lib.cans_poisson_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # --- device entry points -------------------------------------------------------------------
+    def poisson_solve(self, p: torch.Tensor, stream=None):
+        """cans_poisson_solve: p (f on entry) is overwritten with Phi."""
+        _check(_lib.cans_poisson_solve(self._h, _dev_ptr(p, self.shape), _stream_ptr(stream)))
+
+    def projection(self, u, v, w, p, dt: float, stream=None):
+        """cans_projection: u, v, w corrected in place, p overwritten with Phi."""
+        _check(_lib.cans_projection(self._h, _dev_ptr(u, self.shape), _dev_ptr(v, self.shape),
+                                    _dev_ptr(w, self.shape), _dev_ptr(p, self.shape), float(dt),
+                                    _stream_ptr(stream)))
+
+    def set_lower_face(self, direction: int, plane: Optional[torch.Tensor]):
+        ptr = None if plane is None else plane.data_ptr()
+        _check(_lib.cans_projection_set_lower_face(self._h, int(direction), ptr))
+
+    # --- host-buffer entry points (end-to-end timing) ---------------------------------------------
+    def poisson_solve_host(self, p_host: torch.Tensor, stream=None):
+        _check(_lib.cans_poisson_solve_host(self._h, _host_ptr(p_host, self.shape), _stream_ptr(stream)))
+
+    def projection_host(self, u, v, w, p, dt: float, stream=None):
+        _check(_lib.cans_projection_host(self._h, _host_ptr(u, self.shape), _host_ptr(v, self.shape),
+                                         _host_ptr(w, self.shape), _host_ptr(p, self.shape), float(dt),
+                                         _stream_ptr(stream)))
+
+    @property
+    def launches_per_solve(self) -> int:
+        return _lib.cans_plan_launches_per_solve(self._h)
+
+    @property
+    def launches_per_projection(self) -> int:
+        return _lib.cans_plan_launches_per_projection(self._h)
+
+
+def plan_for(workload) -> PoissonPlan:
+    """Plan for a workloads.Workload."""
+    nx, ny, nz = workload.n
+    lx, ly, lz = workload.lengths
+    return PoissonPlan(nx, ny, nz, lx, ly, lz, workload.bc, workload.dzc, workload.dzf)

@@ -1,0 +1,423 @@
+// cans_poisson.cu -- the C ABI of include/cans_poisson.h: plan creation (tables), the z-solve and
+// gradient-correction kernels, and the launch sequences of cans_poisson_solve / cans_projection.
+//
+// Hot path (eqs. 2b, 5, 6, 2c):
+//   a1+a2  x_pass_kernel<fwd, DIV>   divergence fused into the forward x transform
+//   a3     y_pass_kernel<fwd>        forward y transform (strided, staged in shared memory)
+//   a4     z_solve_kernel            Thomas solve per (kx, ky) mode, singular mode pinned
+//   a5     y_pass_kernel<inv>
+//   a6     x_pass_kernel<inv>
+//   a7     grad_correct_kernel       u -= dt G Phi
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/cans_poisson.h"
+#include "plan_tables.hpp"
+#include "xy_kernels.cuh"
+#include "z_pass.cuh"
+#include "grad_pass.cuh"
+
+namespace cans {
+
+static thread_local std::string g_err;
+static thread_local int g_status = CANS_OK;
+
+static int fail(int code, const std::string& msg) {
+    g_status = code;
+    g_err = msg;
+    return code;
+}
+static int fail_cuda(cudaError_t e, const char* where) {
+    return fail(CANS_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+
+constexpr int Z_MROWS = 16;   // rows per thread in the z solve
+// columns per CTA: 16 consecutive x-indices (128 B per row) while the CTA stays <= 512 threads
+// (nz <= 512), else 8 (nz <= 1024)
+static int z_tc_for(int nseg) { return nseg <= 32 ? 16 : 8; }
+
+// ------------------------------------------------------------------------------------------------
+// z kernels
+// ------------------------------------------------------------------------------------------------
+template <int MROWS, int TC>
+__global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a) {
+    extern __shared__ __align__(16) double zsm[];
+    typedef ZPass<MROWS, TC> Z;
+    const int tid = threadIdx.x;
+    const int nthreads = blockDim.x;
+    if (a.singular && blockIdx.x == gridDim.x - 1) {
+        // extra CTA: the singular (0,0) column, staged in shared memory, solved by one thread
+        for (int k = tid; k < a.nz; k += nthreads) zsm[k] = a.p[(size_t)k * a.ncols];
+        __syncthreads();
+        if (tid == 0) z_singular_column(a, zsm);
+        return;
+    }
+    Z::load_tables(a, zsm, tid, nthreads);
+    __syncthreads();
+    ZState<MROWS> st;
+    Z::phase1(a, zsm, st, (long)blockIdx.x, tid);
+    __syncthreads();
+    Z::phase2a(a, zsm, st, tid);
+    __syncthreads();
+    Z::phase2b(a, zsm, st, tid);
+    __syncthreads();
+    Z::phase3(a, zsm, st, tid);
+}
+
+template <int MROWS>
+__global__ void z_setup_kernel(const ZArgs a, double* rstart, double* r00) {
+    const long col = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (col < a.ncols) z_setup_column<MROWS>(a, rstart, r00, col);
+}
+
+// ------------------------------------------------------------------------------------------------
+// a7: velocity correction u -= dt G Phi (eq. 2c): grid-stride loop over pairs of x-adjacent cells
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
+    const size_t npair = (size_t)a.nx / 2 * a.ny * a.nz;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < npair; t += (size_t)gridDim.x * blockDim.x)
+        grad_correct_pair(a, t);
+}
+
+}  // namespace cans
+
+using namespace cans;
+
+// ------------------------------------------------------------------------------------------------
+// the plan
+// ------------------------------------------------------------------------------------------------
+struct cans_poisson_plan {
+    int nx, ny, nz;
+    double lx, ly, lz;
+    char bc[3][2];
+    int kind_x, kind_y;
+    int singular;
+    int nseg, nzp;
+    int num_sms;
+    std::vector<void*> dev_allocs;
+    // device tables
+    double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc, *rstart, *r00;
+    cplx *tw_x, *tw_y, *wpost_x, *wpost_y;
+    double inv_lz;
+    // device buffers for the *_host entry points (lazily allocated)
+    double* hostbuf[4];
+};
+
+static int kind_of(char lo, char up, int* kind) {
+    if (lo == 'P' && up == 'P') { *kind = KIND_PP; return CANS_OK; }
+    if (lo == 'N' && up == 'N') { *kind = KIND_NN; return CANS_OK; }
+    if (lo == 'D' && up == 'D') { *kind = KIND_DD; return CANS_OK; }
+    return CANS_ERR_UNSUPPORTED_BC;
+}
+
+template <class T>
+static cudaError_t upload(cans_poisson_plan* pl, const std::vector<double>& h, T** dptr) {
+    void* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, h.size() * sizeof(double));
+    if (e != cudaSuccess) return e;
+    pl->dev_allocs.push_back(d);
+    e = cudaMemcpy(d, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice);
+    *dptr = reinterpret_cast<T*>(d);
+    return e;
+}
+
+static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
+    ZArgs z;
+    z.nx = pl->nx; z.ny = pl->ny; z.nz = pl->nz;
+    z.nseg = pl->nseg;
+    z.ncols = (long)pl->nx * pl->ny;
+    z.p = p;
+    z.lamx = pl->lamx; z.lamy = pl->lamy;
+    z.az = pl->az; z.bz = pl->bz; z.cz = pl->cz; z.gz = pl->gz;
+    z.rstart = pl->rstart;
+    z.scale = 1.0 / ((double)pl->nx * (double)pl->ny);
+    z.singular = pl->singular;
+    z.r00 = pl->r00;
+    z.dzf = pl->dzf;
+    z.inv_lz = pl->inv_lz;
+    return z;
+}
+
+extern "C" {
+
+const char* cans_last_error(void) { return g_err.c_str(); }
+int cans_last_status(void) { return g_status; }
+const char* cans_version(void) { return "0.1"; }
+
+void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
+    if (!plan) return;
+    for (void* d : plan->dev_allocs) cudaFree(d);
+    for (int i = 0; i < 4; ++i) if (plan->hostbuf[i]) cudaFree(plan->hostbuf[i]);
+    delete plan;
+}
+
+cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
+                                            const char bc[3][2], const double* dzc, const double* dzf) {
+    g_status = CANS_OK;
+    g_err.clear();
+    if (!bc) { fail(CANS_ERR_INVALID_ARG, "bc is NULL"); return nullptr; }
+    if (nx < 2 || ny < 2 || nz < 2) { fail(CANS_ERR_INVALID_ARG, "nx, ny, nz must be >= 2"); return nullptr; }
+    if (!(lx > 0.0) || !(ly > 0.0) || !(lz > 0.0)) { fail(CANS_ERR_INVALID_ARG, "lx, ly, lz must be > 0"); return nullptr; }
+    if ((dzc == nullptr) != (dzf == nullptr)) { fail(CANS_ERR_INVALID_ARG, "dzc and dzf must both be given or both be NULL"); return nullptr; }
+    for (int d = 0; d < 3; ++d)
+        for (int s = 0; s < 2; ++s) {
+            const char ch = bc[d][s];
+            if (ch != 'P' && ch != 'N' && ch != 'D') { fail(CANS_ERR_INVALID_ARG, "bc letters must be 'P', 'N' or 'D'"); return nullptr; }
+        }
+    for (int d = 0; d < 3; ++d)
+        if ((bc[d][0] == 'P') != (bc[d][1] == 'P')) { fail(CANS_ERR_INVALID_ARG, "periodic boundaries must be two-sided"); return nullptr; }
+    int kx, ky;
+    if (kind_of(bc[0][0], bc[0][1], &kx) != CANS_OK || kind_of(bc[1][0], bc[1][1], &ky) != CANS_OK) {
+        fail(CANS_ERR_UNSUPPORTED_BC, "mixed Neumann/Dirichlet pairs in x or y are not implemented (DCT-IV/DST-IV)");
+        return nullptr;
+    }
+    if (bc[2][0] == 'P') { fail(CANS_ERR_UNSUPPORTED_BC, "periodic z is not implemented (cyclic tridiagonal)"); return nullptr; }
+    FftRadices fx, fy;
+    if (!fft_lookup(nx, &fx) || !fft_lookup(ny, &fy)) {
+        fail(CANS_ERR_UNSUPPORTED_SIZE, "nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048");
+        return nullptr;
+    }
+    const int nseg = (nz + Z_MROWS - 1) / Z_MROWS;
+    if (nseg > 64) { fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the z-solve tiling (max 1024)"); return nullptr; }
+    std::vector<double> hdzc(nz + 1), hdzf(nz);
+    for (int k = 0; k < nz; ++k) hdzf[k] = dzf ? dzf[k] : lz / nz;
+    for (int k = 0; k <= nz; ++k) hdzc[k] = dzc ? dzc[k] : lz / nz;
+    for (int k = 0; k < nz; ++k) if (!(hdzf[k] > 0.0)) { fail(CANS_ERR_INVALID_ARG, "dzf must be positive"); return nullptr; }
+    for (int k = 0; k <= nz; ++k) if (!(hdzc[k] > 0.0)) { fail(CANS_ERR_INVALID_ARG, "dzc must be positive"); return nullptr; }
+
+    cans_poisson_plan* pl = new (std::nothrow) cans_poisson_plan();
+    if (!pl) { fail(CANS_ERR_ALLOC, "host allocation failed"); return nullptr; }
+    pl->nx = nx; pl->ny = ny; pl->nz = nz; pl->lx = lx; pl->ly = ly; pl->lz = lz;
+    std::memcpy(pl->bc, bc, 6);
+    pl->kind_x = kx; pl->kind_y = ky;
+    pl->nseg = nseg; pl->nzp = nseg * Z_MROWS;
+    for (int i = 0; i < 4; ++i) pl->hostbuf[i] = nullptr;
+    pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
+    int dev = 0;
+    cudaGetDevice(&dev);
+    pl->num_sms = 148;
+    cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, dev);
+
+    const double dx = lx / nx, dy = ly / ny;
+    ZRows zr = make_z_rows(nz, pl->nzp, hdzc.data(), hdzf.data(), bc[2][0], bc[2][1]);
+    pl->inv_lz = 1.0 / zr.lz_sum;
+    std::vector<double> rdzc(nz);
+    for (int k = 0; k < nz; ++k) rdzc[k] = 1.0 / hdzc[k + 1];
+
+    cudaError_t e = cudaSuccess;
+    auto up = [&](const std::vector<double>& h, auto** d) { if (e == cudaSuccess) e = upload(pl, h, d); };
+    up(make_lambda_positions(nx, kx, dx), &pl->lamx);
+    up(make_lambda_positions(ny, ky, dy), &pl->lamy);
+    up(zr.a, &pl->az); up(zr.b, &pl->bz); up(zr.c, &pl->cz); up(zr.g, &pl->gz);
+    up(zr.rdzf, &pl->rdzf); up(zr.dzf, &pl->dzf); up(rdzc, &pl->rdzc);
+    up(make_pass_twiddles(fx), &pl->tw_x);
+    up(make_pass_twiddles(fy), &pl->tw_y);
+    up(make_post_twiddles(nx), &pl->wpost_x);
+    up(make_post_twiddles(ny), &pl->wpost_y);
+    if (e == cudaSuccess) {
+        void* d = nullptr;
+        e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
+        if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->rstart = (double*)d; }
+    }
+    if (e == cudaSuccess) {
+        void* d = nullptr;
+        e = cudaMalloc(&d, sizeof(double) * (size_t)nz);
+        if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->r00 = (double*)d; }
+    }
+    if (e == cudaSuccess) {
+        ZArgs z = make_zargs(pl, nullptr);
+        const long ncols = z.ncols;
+        z_setup_kernel<Z_MROWS><<<(unsigned)((ncols + 127) / 128), 128>>>(z, pl->rstart, pl->r00);
+        e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    }
+    if (e == cudaSuccess) {
+        size_t zsmem = sizeof(double) * ZPass<Z_MROWS, 16>::smem_doubles(nseg);
+        if (sizeof(double) * (size_t)nz > zsmem) zsmem = sizeof(double) * (size_t)nz;
+        if (z_tc_for(nseg) == 16)
+            e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zsmem);
+        else
+            e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zsmem);
+    }
+    if (e != cudaSuccess) {
+        const bool oom = (e == cudaErrorMemoryAllocation);
+        std::string msg = std::string("plan creation: ") + cudaGetErrorString(e);
+        cans_poisson_plan_destroy(pl);
+        cudaGetLastError();
+        fail(oom ? CANS_ERR_ALLOC : CANS_ERR_CUDA, msg);
+        return nullptr;
+    }
+    return pl;
+}
+
+static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
+    XYArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.nx = pl->nx; a.ny = pl->ny; a.nz = pl->nz;
+    a.kind = xdir ? pl->kind_x : pl->kind_y;
+    a.tw = xdir ? pl->tw_x : pl->tw_y;
+    a.wpost = xdir ? pl->wpost_x : pl->wpost_y;
+    a.p = p;
+    return a;
+}
+
+static int launch_xy_any(int n, int op, const XYArgs& a, cudaStream_t st) {
+    cudaError_t err = cudaSuccess;
+    if (launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||
+        launch_xy_group_c(n, op, a, st, &err) || launch_xy_group_d(n, op, a, st, &err)) {
+        if (err != cudaSuccess) return fail_cuda(err, "x/y transform launch");
+        return CANS_OK;
+    }
+    return fail(CANS_ERR_UNSUPPORTED_SIZE, "transform length not instantiated");
+}
+
+static int launch_z(const cans_poisson_plan* pl, double* p, cudaStream_t st) {
+    ZArgs z = make_zargs(pl, p);
+    const int tc = z_tc_for(pl->nseg);
+    const long ntiles = (z.ncols + tc - 1) / tc;
+    const unsigned grid = (unsigned)(ntiles + (pl->singular ? 1 : 0));
+    size_t smem = sizeof(double) * (tc == 16 ? ZPass<Z_MROWS, 16>::smem_doubles(pl->nseg)
+                                             : ZPass<Z_MROWS, 8>::smem_doubles(pl->nseg));
+    if (pl->singular && sizeof(double) * (size_t)pl->nz > smem) smem = sizeof(double) * (size_t)pl->nz;
+    if (tc == 16) z_solve_kernel<Z_MROWS, 16><<<grid, 16 * pl->nseg, smem, st>>>(z);
+    else z_solve_kernel<Z_MROWS, 8><<<grid, 8 * pl->nseg, smem, st>>>(z);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "z solve launch");
+    return CANS_OK;
+}
+
+// the transform/solve/transform core shared by both entry points; `div` selects the fused-divergence load
+static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, cudaStream_t st) {
+    int rc;
+    if (divargs) rc = launch_xy_any(pl->nx, OP_X_FWD_DIV, *divargs, st);
+    else rc = launch_xy_any(pl->nx, OP_X_FWD, make_xyargs(pl, p, true), st);
+    if (rc) return rc;
+    if ((rc = launch_xy_any(pl->ny, OP_Y_FWD, make_xyargs(pl, p, false), st))) return rc;
+    if ((rc = launch_z(pl, p, st))) return rc;
+    if ((rc = launch_xy_any(pl->ny, OP_Y_INV, make_xyargs(pl, p, false), st))) return rc;
+    if ((rc = launch_xy_any(pl->nx, OP_X_INV, make_xyargs(pl, p, true), st))) return rc;
+    return CANS_OK;
+}
+
+int cans_plan_launches_per_solve(const cans_poisson_plan*) { return 5; }
+int cans_plan_launches_per_projection(const cans_poisson_plan*) { return 6; }
+
+int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream) {
+    g_status = CANS_OK;
+    if (!plan || !p) return fail(CANS_ERR_INVALID_ARG, "plan and p must be non-NULL");
+    if ((reinterpret_cast<size_t>(p) & 15) != 0) return fail(CANS_ERR_INVALID_ARG, "p must be 16-byte aligned");
+    return run_core(plan, p, nullptr, (cudaStream_t)stream);
+}
+
+int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double dt, void* stream) {
+    g_status = CANS_OK;
+    if (!plan || !u || !v || !w || !p) return fail(CANS_ERR_INVALID_ARG, "plan, u, v, w, p must be non-NULL");
+    if (!(dt > 0.0)) return fail(CANS_ERR_INVALID_ARG, "dt must be > 0");
+    if (((reinterpret_cast<size_t>(p) | reinterpret_cast<size_t>(u) | reinterpret_cast<size_t>(v) |
+          reinterpret_cast<size_t>(w)) & 15) != 0)
+        return fail(CANS_ERR_INVALID_ARG, "fields must be 16-byte aligned");
+    for (int d = 0; d < 3; ++d)
+        if (plan->bc[d][0] == 'D')
+            return fail(CANS_ERR_NEEDS_FACE, "a lower 'D' side needs a registered lower-face plane (not implemented)");
+    cudaStream_t st = (cudaStream_t)stream;
+    XYArgs a = make_xyargs(plan, p, true);
+    a.u = u; a.v = v; a.w = w;
+    a.rdzf = plan->rdzf;
+    a.rdx = (double)plan->nx / plan->lx;
+    a.rdy = (double)plan->ny / plan->ly;
+    a.rdt = 1.0 / dt;
+    a.wrap_x = plan->bc[0][0] == 'P';
+    a.wrap_y = plan->bc[1][0] == 'P';
+    a.wrap_z = plan->bc[2][0] == 'P';
+    int rc = run_core(plan, p, &a, st);
+    if (rc) return rc;
+    GradArgs g;
+    g.nx = plan->nx; g.ny = plan->ny; g.nz = plan->nz;
+    g.u = u; g.v = v; g.w = w; g.phi = p;
+    g.rdzc = plan->rdzc;
+    g.dt = dt;
+    g.dt_rdx = dt * a.rdx;
+    g.dt_rdy = dt * a.rdy;
+    auto ghost = [](char up, int n, int* idx, double* sgn) {
+        if (up == 'P') { *idx = 0; *sgn = 1.0; }
+        else if (up == 'N') { *idx = n - 1; *sgn = 1.0; }
+        else { *idx = n - 1; *sgn = -1.0; }
+    };
+    ghost(plan->bc[0][1], plan->nx, &g.gx_idx, &g.gx_sgn);
+    ghost(plan->bc[1][1], plan->ny, &g.gy_idx, &g.gy_sgn);
+    ghost(plan->bc[2][1], plan->nz, &g.gz_idx, &g.gz_sgn);
+    const size_t npair = (size_t)plan->nx / 2 * plan->ny * plan->nz;
+    size_t blocks = (npair + 255) / 256;
+    const size_t cap = (size_t)plan->num_sms * 32;
+    if (blocks > cap) blocks = cap;
+    grad_correct_kernel<<<(unsigned)blocks, 256, 0, st>>>(g);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
+    return CANS_OK;
+}
+
+int cans_projection_set_lower_face(cans_poisson_plan* plan, int dir, double* face_plane) {
+    g_status = CANS_OK;
+    if (!plan || dir < 0 || dir > 2) return fail(CANS_ERR_INVALID_ARG, "bad plan or direction");
+    if (face_plane) return fail(CANS_ERR_UNSUPPORTED_BC, "lower-face planes are not implemented yet");
+    return CANS_OK;
+}
+
+static int ensure_hostbufs(cans_poisson_plan* pl, int count) {
+    const size_t bytes = sizeof(double) * (size_t)pl->nx * pl->ny * pl->nz;
+    for (int i = 0; i < count; ++i)
+        if (!pl->hostbuf[i]) {
+            cudaError_t e = cudaMalloc((void**)&pl->hostbuf[i], bytes);
+            if (e != cudaSuccess) { cudaGetLastError(); return fail(CANS_ERR_ALLOC, "device buffer for host entry point"); }
+        }
+    return CANS_OK;
+}
+
+int cans_poisson_solve_host(cans_poisson_plan* plan, double* p_host, void* stream) {
+    g_status = CANS_OK;
+    if (!plan || !p_host) return fail(CANS_ERR_INVALID_ARG, "plan and p_host must be non-NULL");
+    int rc = ensure_hostbufs(plan, 1);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = sizeof(double) * (size_t)plan->nx * plan->ny * plan->nz;
+    cudaError_t e = cudaMemcpyAsync(plan->hostbuf[0], p_host, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return fail_cuda(e, "H2D copy");
+    if ((rc = cans_poisson_solve(plan, plan->hostbuf[0], stream))) return rc;
+    e = cudaMemcpyAsync(p_host, plan->hostbuf[0], bytes, cudaMemcpyDeviceToHost, st);
+    if (e != cudaSuccess) return fail_cuda(e, "D2H copy");
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(e, "stream synchronize");
+    return CANS_OK;
+}
+
+int cans_projection_host(cans_poisson_plan* plan, double* u_host, double* v_host, double* w_host,
+                         double* p_host, double dt, void* stream) {
+    g_status = CANS_OK;
+    if (!plan || !u_host || !v_host || !w_host || !p_host) return fail(CANS_ERR_INVALID_ARG, "NULL argument");
+    int rc = ensure_hostbufs(plan, 4);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t bytes = sizeof(double) * (size_t)plan->nx * plan->ny * plan->nz;
+    double* hsrc[3] = {u_host, v_host, w_host};
+    cudaError_t e;
+    for (int i = 0; i < 3; ++i) {
+        e = cudaMemcpyAsync(plan->hostbuf[i], hsrc[i], bytes, cudaMemcpyHostToDevice, st);
+        if (e != cudaSuccess) return fail_cuda(e, "H2D copy");
+    }
+    if ((rc = cans_projection(plan, plan->hostbuf[0], plan->hostbuf[1], plan->hostbuf[2], plan->hostbuf[3], dt, stream))) return rc;
+    double* hdst[4] = {u_host, v_host, w_host, p_host};
+    for (int i = 0; i < 4; ++i) {
+        e = cudaMemcpyAsync(hdst[i], plan->hostbuf[i], bytes, cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) return fail_cuda(e, "D2H copy");
+    }
+    e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return fail_cuda(e, "stream synchronize");
+    return CANS_OK;
+}
+
+}  // extern "C"

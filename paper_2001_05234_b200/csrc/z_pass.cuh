@@ -1,0 +1,227 @@
+// z_pass.cuh -- the tridiagonal solve along z for every (kx, ky) mode: eq. 6, "solved very
+// efficiently with Gauss elimination", on a possibly non-uniform z grid.
+//
+//   (b_k + lam) x_k + a_k x_{k-1} + c_k x_{k+1} = d_k ,   lam = lam_x(i)/dx^2 + lam_y(j)/dy^2 <= 0
+//
+// Thomas recurrence (same algebra as the sequential algorithm):
+//   r_k = 1 / (b_k + lam - a_k c_{k-1} r_{k-1}),  d'_k = (d_k - a_k d'_{k-1}) r_k,  x_k = d'_k - c_k r_k x_{k+1}
+//
+// B200 mapping ("register-resident partitioned Thomas"): a column is cut into P segments of MROWS rows;
+// thread (c, s) owns segment s of column c with its MROWS right-hand sides in registers, so a warp
+// reads/writes 16-32 consecutive x-indices per row (coalesced) and the whole column never leaves the
+// SM between the forward and backward sweeps (16 B/cell of HBM traffic, the structural minimum).
+//   * the pivot chain r_k is restarted at every segment from a plan-time table r_{k0-1}(mode, s)
+//     (nx*ny*P doubles, 1/MROWS of a field) and recomputed in-register -- bit-identical to the
+//     sequential pivots;
+//   * d' and x are first-order linear recurrences: each segment runs them from a zero start while
+//     accumulating the propagation factor (prod of -a_k r_k, resp. -c_k r_k); a P-step scan over the
+//     segment ends in shared memory supplies the true start value, which is then propagated.
+// The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_column.
+#pragma once
+#include "common.cuh"
+
+namespace cans {
+
+struct ZArgs {
+    int nx, ny, nz;
+    int nseg;                 // P = ceil(nz / MROWS)
+    long ncols;               // nx * ny
+    double* p;                // field, solved in place
+    const double* lamx;       // [nx]  lam_x(position)/dx^2
+    const double* lamy;       // [ny]  lam_y(position)/dy^2
+    const double* az;         // [nseg*MROWS] sub-diagonal a_k        (0 beyond nz, a_0 = 0)
+    const double* bz;         // diagonal b_k with boundary rows folded in (1 beyond nz)
+    const double* cz;         // super-diagonal c_k                   (0 beyond nz, c_{nz-1} = 0)
+    const double* gz;         // a_k * c_{k-1}                        (0 for k = 0 and beyond nz)
+    const double* rstart;     // [nseg][ncols]  r_{s*MROWS-1}(column)  (0 for s = 0)
+    double scale;             // 1/(nx*ny): normalisation of the two unnormalised inverse FFTs
+    int singular;             // 1: column 0 is the singular mode, skipped here
+    const double* r00;        // [nz] pivots of the singular column (rows 0..nz-2), plan-time
+    const double* dzf;        // [nz]
+    double inv_lz;            // 1 / sum(dzf)
+};
+
+// one pivot step; shared by the plan-time table kernel and the solve so the values are identical
+CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) {
+    return 1.0 / ((bk + lam) - gk * rprev);
+}
+
+template <int MROWS>
+struct ZState {
+    double d[MROWS];
+    double r[MROWS];
+    double start;     // true d'_{k0-1}, later true x_{k0+MROWS}
+    long col;
+    bool active;
+};
+
+// shared memory: tables az,bz,cz,gz [4][nzp] then scan arrays end[TC*P], fac[TC*P]
+template <int MROWS, int TC>
+struct ZPass {
+    static CANS_HD size_t smem_doubles(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)2 * TC * nseg; }
+
+    static CANS_HD void load_tables(const ZArgs& a, double* sm, int tid, int nthreads) {
+        const int nzp = a.nseg * MROWS;
+        for (int i = tid; i < nzp; i += nthreads) {
+            sm[i] = a.az[i];
+            sm[nzp + i] = a.bz[i];
+            sm[2 * nzp + i] = a.cz[i];
+            sm[3 * nzp + i] = a.gz[i];
+        }
+    }
+
+    // phase 1: load the segment, pivots, local forward sweep from a zero start; publish (end, factor)
+    static CANS_HD void phase1(const ZArgs& a, double* sm, ZState<MROWS>& st, long tile, int tid) {
+        const int nzp = a.nseg * MROWS;
+        const double* saz = sm;
+        const double* sbz = sm + nzp;
+        const double* sgz = sm + 3 * nzp;
+        double* s_end = sm + 4 * nzp;
+        double* s_fac = s_end + TC * a.nseg;
+        const int c = tid % TC;
+        const int s = tid / TC;
+        const long col = tile * TC + c;
+        st.col = col;
+        st.active = (col < a.ncols) && !(a.singular && col == 0);
+        const int k0 = s * MROWS;
+        const size_t plane = (size_t)a.ncols;
+        if (col < a.ncols) {
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) {
+                const int k = k0 + r;
+                st.d[r] = (k < a.nz) ? a.p[(size_t)k * plane + col] * a.scale : 0.0;
+            }
+            const int i = (int)(col % a.nx);
+            const int j = (int)(col / a.nx);
+            const double lam = a.lamx[i] + a.lamy[j];
+            double rp = a.rstart[(size_t)s * a.ncols + col];
+            double dp = 0.0, fac = 1.0;
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) {
+                const int k = k0 + r;
+                rp = z_pivot(sbz[k], lam, sgz[k], rp);
+                st.r[r] = rp;
+                const double e = saz[k] * rp;
+                dp = st.d[r] * rp - e * dp;
+                st.d[r] = dp;
+                fac *= -e;
+            }
+            s_end[s * TC + c] = dp;
+            s_fac[s * TC + c] = fac;
+        } else {
+            s_end[s * TC + c] = 0.0;
+            s_fac[s * TC + c] = 0.0;
+        }
+    }
+
+    // phase 2: scan the segment ends -> true start; propagate; local backward sweep from a zero start; publish
+    static CANS_HD void phase2a(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
+        const int nzp = a.nseg * MROWS;
+        const double* s_end = sm + 4 * nzp;
+        const double* s_fac = s_end + TC * a.nseg;
+        const int c = tid % TC;
+        const int s = tid / TC;
+        double D = 0.0;                     // true d' at the end of segment s'-1
+        for (int q = 0; q < s; ++q) D = s_end[q * TC + c] + s_fac[q * TC + c] * D;
+        st.start = D;
+    }
+    // (a barrier separates 2a and 2b because 2b overwrites the scan arrays)
+    static CANS_HD void phase2b(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
+        const int nzp = a.nseg * MROWS;
+        const double* saz = sm;
+        const double* scz = sm + 2 * nzp;
+        double* s_end = sm + 4 * nzp;
+        double* s_fac = s_end + TC * a.nseg;
+        const int c = tid % TC;
+        const int s = tid / TC;
+        const int k0 = s * MROWS;
+        if (st.col < a.ncols) {
+            double fac = 1.0;
+            const double D = st.start;
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) {
+                fac *= -(saz[k0 + r] * st.r[r]);
+                st.d[r] += fac * D;
+            }
+            double xs = 0.0, g = 1.0;
+#pragma unroll
+            for (int r = MROWS - 1; r >= 0; --r) {
+                const double cp = scz[k0 + r] * st.r[r];
+                xs = st.d[r] - cp * xs;
+                st.d[r] = xs;
+                g *= -cp;
+            }
+            s_end[s * TC + c] = xs;     // x^0 at the top row of the segment
+            s_fac[s * TC + c] = g;
+        } else {
+            s_end[s * TC + c] = 0.0;
+            s_fac[s * TC + c] = 0.0;
+        }
+    }
+
+    // phase 3: scan from the bottom -> true x below the segment; propagate; store
+    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
+        const int nzp = a.nseg * MROWS;
+        const double* scz = sm + 2 * nzp;
+        const double* s_end = sm + 4 * nzp;
+        const double* s_fac = s_end + TC * a.nseg;
+        const int c = tid % TC;
+        const int s = tid / TC;
+        const int k0 = s * MROWS;
+        double X = 0.0;                     // true x at the top row of segment s'+1
+        for (int q = a.nseg - 1; q > s; --q) X = s_end[q * TC + c] + s_fac[q * TC + c] * X;
+        if (st.active) {
+            const size_t plane = (size_t)a.ncols;
+            double g = 1.0;
+#pragma unroll
+            for (int r = MROWS - 1; r >= 0; --r) {
+                g *= -(scz[k0 + r] * st.r[r]);
+                st.d[r] += g * X;
+            }
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) {
+                const int k = k0 + r;
+                if (k < a.nz) a.p[(size_t)k * plane + st.col] = st.d[r];
+            }
+        }
+    }
+};
+
+// plan-time: pivots at the segment boundaries of every column (thread per column, sequential in k)
+template <int MROWS>
+CANS_HD void z_setup_column(const ZArgs& a, double* rstart_out, double* r00_out, long col) {
+    const int i = (int)(col % a.nx);
+    const int j = (int)(col / a.nx);
+    const double lam = a.lamx[i] + a.lamy[j];
+    double rp = 0.0;
+    const int nzp = a.nseg * MROWS;
+    for (int k = 0; k < nzp; ++k) {
+        if (k % MROWS == 0) rstart_out[(size_t)(k / MROWS) * a.ncols + col] = rp;
+        rp = z_pivot(a.bz[k], lam, a.gz[k], rp);
+        if (col == 0 && k < a.nz && r00_out) r00_out[k] = rp;
+    }
+}
+
+// The singular column (reading S3 / oracle O4): forward sweep on rows 0..nz-2, x[nz-1] = 0,
+// back-substitute, subtract the dzf-weighted mean.  One thread; d is staged in shared memory.
+CANS_HD void z_singular_column(const ZArgs& a, double* sd /* nz doubles */) {
+    const size_t plane = (size_t)a.ncols;
+    const int nz = a.nz;
+    double dp = 0.0;
+    for (int k = 0; k < nz - 1; ++k) {
+        const double rk = a.r00[k];
+        dp = (sd[k] * a.scale - a.az[k] * dp) * rk;
+        sd[k] = dp;
+    }
+    double x = 0.0, acc = 0.0;
+    sd[nz - 1] = 0.0;
+    for (int k = nz - 2; k >= 0; --k) {
+        x = sd[k] - a.cz[k] * a.r00[k] * x;
+        sd[k] = x;
+        acc += x * a.dzf[k];
+    }
+    const double mean = acc * a.inv_lz;
+    for (int k = 0; k < nz; ++k) a.p[(size_t)k * plane] = sd[k] - mean;
+}
+
+}  // namespace cans

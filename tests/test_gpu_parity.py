@@ -1,0 +1,219 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Bar (BASELINE.json north_star): relative L2 <= 1e-11 on every output
+field and max-abs <= 1e-10 on O(1)-scaled fields (Phi for Poisson; u, v, w and dt*Phi for projection).
+"""
+import itertools
+import os
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import cans_oracle as orc
+from paper_2001_05234_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 1e-11
+MAX_ABS = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2001_05234_b200 import binding
+    return binding
+
+
+def np_of(t):
+    return t.detach().cpu().numpy()
+
+
+def dz_np(w):
+    if w.dzc is None:
+        return None, None
+    return w.dzc.numpy(), w.dzf.numpy()
+
+
+def check_field(got, ref, scale=1.0, what=""):
+    got = np.asarray(got)
+    diff = got - ref
+    nrm = np.linalg.norm(ref.ravel())
+    if nrm > 0:
+        rel = np.linalg.norm(diff.ravel()) / nrm
+        assert rel <= REL_L2, f"{what}: rel-L2 {rel:.3e}"
+    mabs = np.max(np.abs(diff)) * scale
+    assert mabs <= MAX_ABS, f"{what}: max-abs {mabs:.3e}"
+
+
+def gpu_poisson(B, w, f_dev):
+    plan = B.plan_for(w)
+    p = f_dev.clone()
+    plan.poisson_solve(p)
+    torch.cuda.synchronize()
+    plan.close()
+    return p
+
+
+def random_rhs(nx, ny, nz, bc, dzf, seed):
+    rng = np.random.default_rng(seed)
+    f = rng.uniform(-1, 1, (nz, ny, nx))
+    if orc.is_singular(bc):
+        wz = dzf if dzf is not None else np.ones(nz)
+        f -= np.sum(f * wz[:, None, None]) / (np.sum(wz) * nx * ny)
+    return f
+
+
+# ----------------------------------------------------------------------------------------------
+# BASELINE.json configs 1 and 2: full-size, element by element
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C1", "C2"])
+def test_config_full_parity(B, name):
+    w = wl.make_workload(name, device="cuda")
+    f = w.fields["f"]
+    phi = gpu_poisson(B, w, f)
+    dzc, dzf = dz_np(w)
+    ref = orc.poisson_solve(np_of(f), *w.lengths, w.bc, dzc, dzf)
+    check_field(np_of(phi), ref, what=name)
+    wz = dzf if dzf is not None else np.ones(w.n[2])
+    # zero dzf-weighted mean (reading S3)
+    assert abs(np.sum(np_of(phi) * wz[:, None, None])) <= 1e-12 * np.sum(np.abs(ref) * wz[:, None, None]) + 1e-12
+
+
+# ----------------------------------------------------------------------------------------------
+# every supported boundary combination, sizes that span several tiles with ragged tails
+# (nz = 33: three z segments, the last with one row; 48/96: radix-3 lengths; tiles of 16 columns)
+# ----------------------------------------------------------------------------------------------
+XY = ["PP", "NN", "DD"]
+ZP = ["NN", "DD", "ND", "DN"]
+
+
+@pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 96, 33, 1.6), (128, 32, 40, None), (16, 16, 2, None),
+                                               (192, 64, 17, 2.0)])
+def test_all_boundary_combinations(B, nx, ny, nz, stretch):
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    if stretch is None:
+        dzc = dzf = None
+    else:
+        dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, stretch)
+        dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    seed = 100
+    for px, py, pz in itertools.product(XY, XY, ZP):
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        seed += 1
+        f = random_rhs(nx, ny, nz, bc, dzf, seed)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        torch.cuda.synchronize()
+        plan.close()
+        ref = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        check_field(np_of(p), ref, what=f"{px}/{py}/{pz} {nx}x{ny}x{nz}")
+
+
+@pytest.mark.parametrize("n", [16, 32, 48, 64, 96, 128, 192, 256, 384, 512, 768, 1024, 1536, 2048])
+def test_every_transform_length_in_x_and_y(B, n):
+    lx, ly, lz = 1.0, 2.0, 0.5
+    nz = 18
+    for (nx, ny, bc) in [(n, 32, (("N", "N"), ("P", "P"), ("D", "N"))), (32, n, (("P", "P"), ("D", "D"), ("N", "N")))]:
+        f = random_rhs(nx, ny, nz, bc, None, n)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        torch.cuda.synchronize()
+        plan.close()
+        ref = orc.poisson_solve(f, lx, ly, lz, bc)
+        check_field(np_of(p), ref, what=f"n={n} {nx}x{ny}")
+
+
+# ----------------------------------------------------------------------------------------------
+# projection (eqs. 2b-2c) against the oracle, plus its invariants evaluated with the oracle's operators
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("px,py,pz", [("PP", "PP", "NN"), ("PP", "NN", "NN"), ("NN", "NN", "NN"),
+                                      ("PP", "PP", "ND"), ("NN", "PP", "NN")])
+def test_projection_parity_and_invariants(B, px, py, pz):
+    nx, ny, nz = 96, 64, 40
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+    rng = np.random.default_rng(7)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    if px[1] == "N":
+        u[:, :, -1] = 0
+    if py[1] == "N":
+        v[:, -1, :] = 0
+    if pz[1] == "N":
+        w[-1] = 0
+    dt = 1e-3
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+    pd = torch.full((nz, ny, nx), float("nan"), dtype=torch.float64, device="cuda")   # entry contents ignored
+    plan.projection(ud, vd, wd, pd, dt)
+    torch.cuda.synchronize()
+    un, vn, wn, phi, _ = orc.projection(u, v, w, dt, lx, ly, lz, bc, dzc, dzf)
+    check_field(np_of(ud), un, what="u")
+    check_field(np_of(vd), vn, what="v")
+    check_field(np_of(wd), wn, what="w")
+    check_field(np_of(pd), phi, scale=dt, what="dt*Phi")
+    # invariants of the GPU result, measured with the oracle's operators
+    div = orc.divergence(np_of(ud), np_of(vd), np_of(wd), lx, ly, lz, bc, dzc, dzf)
+    assert np.max(np.abs(div)) < 1e-11 * np.max(np.abs(u)) / min(lx / nx, ly / ny, dzf.min())
+    if px[1] == "N":
+        assert np.array_equal(np_of(ud)[:, :, -1], u[:, :, -1])
+    if py[1] == "N":
+        assert np.array_equal(np_of(vd)[:, -1, :], v[:, -1, :])
+    if pz[1] == "N":
+        assert np.array_equal(np_of(wd)[-1], w[-1])
+    # idempotence: projecting the projected field changes nothing
+    u1, v1, w1 = ud.clone(), vd.clone(), wd.clone()
+    plan.projection(ud, vd, wd, pd, dt)
+    torch.cuda.synchronize()
+    assert float((ud - u1).abs().max()) < 1e-11 and float((pd * dt).abs().max()) < 1e-11
+    plan.close()
+
+
+def test_error_codes_on_device(B):
+    bc = (("P", "P"), ("P", "P"), ("D", "N"))
+    plan = B.PoissonPlan(32, 32, 16, 1.0, 1.0, 1.0, bc)
+    z = torch.zeros((16, 32, 32), dtype=torch.float64, device="cuda")
+    with pytest.raises(B.CansError) as ei:
+        plan.projection(z, z.clone(), z.clone(), z.clone(), 1e-3)       # lower 'D' side in z
+    assert ei.value.status == B.CANS_ERR_NEEDS_FACE
+    with pytest.raises(B.CansError) as ei:
+        B.PoissonPlan(32, 32, 16, 1.0, 1.0, 1.0, (("P", "P"), ("P", "P"), ("N", "N"))).projection(
+            z, z.clone(), z.clone(), z.clone(), -1.0)
+    assert ei.value.status == B.CANS_ERR_INVALID_ARG
+    with pytest.raises(ValueError):
+        plan.poisson_solve(torch.zeros((16, 32, 31), dtype=torch.float64, device="cuda"))
+    plan.close()
+
+
+def test_solve_runs_on_a_side_stream_without_syncing(B):
+    w = wl.make_workload("C1", device="cuda")
+    plan = B.plan_for(w)
+    f = w.fields["f"]
+    s = torch.cuda.Stream()
+    p = f.clone()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        plan.poisson_solve(p, stream=s)
+    s.synchronize()
+    ref = gpu_poisson(B, w, f)
+    assert torch.equal(p, ref)          # deterministic: same bits on any stream
+    plan.close()
+
+
+def test_host_entry_point_matches_device_path(B):
+    w = wl.make_workload("C5", device="cuda", n_override=(64, 48, 32))
+    plan = B.plan_for(w)
+    u, v, ww = (w.fields[c] for c in "uvw")
+    ud, vd, wd = u.clone(), v.clone(), ww.clone()
+    pd = torch.empty_like(u)
+    plan.projection(ud, vd, wd, pd, w.dt)
+    torch.cuda.synchronize()
+    uh, vh, wh = (t.cpu().pin_memory() for t in (u, v, ww))
+    ph = torch.empty(u.shape, dtype=torch.float64).pin_memory()
+    plan.projection_host(uh, vh, wh, ph, w.dt)
+    assert torch.equal(uh, ud.cpu()) and torch.equal(wh, wd.cpu()) and torch.equal(ph, pd.cpu())
+    plan.close()
