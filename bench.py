@@ -1,0 +1,359 @@
+#!/usr/bin/env python
+"""bench.py -- FP64 pressure-projection throughput on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]            this repo's CUDA path
+  python bench.py --impl reference [--gpus N] [--steps K] ...    the CPU oracle on the host cores
+
+A "step" is one pass of the whole hot path (divergence -> x/y transforms -> z Thomas solve -> inverse
+transforms -> gradient correction) on the C5 workload of BASELINE.json: the 1024x768x512 channel grid,
+periodic x/y, Neumann z, tanh-stretched z (a = 1.6), seeded synthetic k^-5/3 + Poiseuille velocity
+fields (recipe: DESIGN.md "Synthetic inputs"; stands in for the paper's turbulent-channel data).
+One JSON line is printed by rank 0.  For N > 1 every rank runs an independent replica
+("replicas only": the path has no exchange step on one GPU).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fp64_projection_throughput"
+UNIT = "Gcells/s"
+WORKLOAD = "C5: projection step 1024x768x512, PP/PP/NN, tanh z (a=1.6), dt=1e-4"
+
+# algorithmic HBM bytes per cell of each kernel of the current launch sequence
+KERNEL_BYTES_PER_CELL = {
+    "x_fwd_div": 32.0,     # read u, v, w (24) + write f~ (8)
+    "x_fwd": 16.0,
+    "y_fwd": 16.0,
+    "z_solve": 16.0,
+    "y_inv": 16.0,
+    "x_inv": 16.0,
+    "grad_correct": 56.0,  # read Phi (8) + u, v, w (24), write u, v, w (24)
+}
+STEP_MIN_BYTES_PER_CELL = {"projection": 112.0, "poisson": 48.0}   # structural minimum, SURVEY.md 8(d)
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            with open(path) as fh:
+                mp = json.load(fh)
+            return float(mp["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, device copy)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clock / throttle-reason sampler running during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for l in self.lines:
+            parts = [p.strip() for p in l.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                smax = float(parts[1])
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        # median over the upper half of the samples = clocks under load (idle samples sit lower or equal)
+        med = sm[len(sm) // 2] if sm else None
+        return {"sm_mhz": med, "sm_max_mhz": smax, "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def cpu_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [d.get("num_threads", 1) for d in threadpool_info() if d.get("user_api") == "blas"]
+        if n:
+            return max(n)
+    except Exception:
+        pass
+    return os.cpu_count() or 1
+
+
+def time_oracle_sample(nz_sample: int, repeats: int):
+    """The CPU oracle, as it stands, on a bounded sample of C5: same nx, ny, domain, bc and stretching
+    recipe with nz_sample planes.  Returns (Gcells/s, seconds per step, cells)."""
+    import numpy as np
+    from oracle import cans_oracle as orc
+    from paper_2001_05234_b200 import workloads
+    w = workloads.make_workload("C5", device="cpu", n_override=(1024, 768, nz_sample))
+    u, v, ww = (w.fields[c].numpy() for c in "uvw")
+    dzc, dzf = w.dzc.numpy(), w.dzf.numpy()
+    times = []
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        orc.projection(u, v, ww, w.dt, *w.lengths, w.bc, dzc, dzf)
+        times.append(time.perf_counter() - t0)
+    return w.cells, times
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (rank 0 only)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    nz_sample = 8
+    cells, times = time_oracle_sample(nz_sample, args.warmup + args.steps)
+    timed = times[args.warmup:]
+    total = sum(timed)
+    value = cells * len(timed) / total / 1e9
+    sample = (f"oracle.projection on a {1024}x{768}x{nz_sample} slab of the C5 workload per step "
+              f"(same domain, bc, tanh recipe; {cells} cells)")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(timed),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def time_poisson_config(binding, workloads, torch, name, steps=10, warmup=3):
+    """Poisson-only timing of a BASELINE.json config (RHS values do not affect the timing)."""
+    w = workloads.make_workload(name, device="cuda", with_fields=False)
+    nx, ny, nz = w.n
+    plan = binding.plan_for(w)
+    f = torch.rand((nz, ny, nx), dtype=torch.float64, device="cuda")
+    p = torch.empty_like(f)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for _ in range(warmup):
+        p.copy_(f)
+        plan.poisson_solve(p)
+    for i in range(steps):
+        p.copy_(f)
+        ev[i][0].record()
+        plan.poisson_solve(p)
+        ev[i][1].record()
+    torch.cuda.synchronize()
+    ms = sorted(a.elapsed_time(b) for a, b in ev)
+    plan.close()
+    med = ms[len(ms) // 2]
+    cells = nx * ny * nz
+    return {"config": name, "grid": f"{nx}x{ny}x{nz}", "bc": w.bc_str, "ms_median": med, "ms_min": ms[0],
+            "gcells_per_s": cells / med / 1e6, "min_bytes": 48.0 * cells}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback "
+                         "(use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_2001_05234_b200 import binding, workloads   # raises if libcans_poisson.so is missing
+
+    peak_gbs, peak_src = load_peaks()
+    w = workloads.make_workload("C5", device="cuda")
+    nx, ny, nz = w.n
+    cells = w.cells
+    plan = binding.plan_for(w)
+    u0, v0, w0 = (w.fields[c] for c in "uvw")
+    u, v, ww = torch.empty_like(u0), torch.empty_like(u0), torch.empty_like(u0)
+    p = torch.empty_like(u0)
+
+    def restore():
+        u.copy_(u0); v.copy_(v0); ww.copy_(w0)
+
+    # ---- warm-up ----
+    for _ in range(max(args.warmup, 3)):
+        restore()
+        plan.projection(u, v, ww, p, w.dt)
+    torch.cuda.synchronize()
+
+    # ---- timed region: K steps, CUDA events on the launching stream, per-kernel events inside ----
+    plan.set_profiling(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kernel_ms = {}
+    sampler = ClockSampler(local_rank)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    for i in range(args.steps):
+        restore()                      # inputs (12.9 GB) are far larger than L2 (126 MB): every step starts cold
+        ev[i][0].record()
+        plan.projection(u, v, ww, p, w.dt)
+        ev[i][1].record()
+        for name, ms in plan.kernel_times():     # waits for this step's kernels only
+            kernel_ms.setdefault(name, []).append(ms)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    plan.set_profiling(False)
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * cells * args.steps / (total_ms * 1e-3) / 1e9
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (largest share of the step) ----
+    kavg = {k: sum(vv) / len(vv) for k, vv in kernel_ms.items()}
+    dom = max(kavg, key=kavg.get)
+    dom_bytes = KERNEL_BYTES_PER_CELL[dom] * cells
+    dom_gbs = dom_bytes / (kavg[dom] * 1e-3) / 1e9
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "traffic.json")     # per-launch DRAM bytes from the committed ncu capture
+    if os.path.exists(tpath):
+        try:
+            with open(tpath) as fh:
+                traffic = json.load(fh).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": dom_gbs, "peak": peak_gbs, "unit": "GB/s",
+                "frac": dom_gbs / peak_gbs, "traffic": traffic, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": kavg[dom]}
+    step_gbs = STEP_MIN_BYTES_PER_CELL["projection"] * cells / (ms_per_step * 1e-3) / 1e9
+    kernels = {k: {"ms": kavg[k], "share": kavg[k] / sum(kavg.values()),
+                   "achieved_gbs": KERNEL_BYTES_PER_CELL[k] * cells / (kavg[k] * 1e-3) / 1e9} for k in kavg}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        n_e2e = min(args.steps, 3)
+        hu, hv, hw = (t.cpu().pin_memory() for t in (u0, v0, w0))
+        hu0 = hu.clone()
+        hp = torch.empty(u0.shape, dtype=torch.float64).pin_memory()
+        plan.projection_host(hu, hv, hw, hp, w.dt)          # warm-up (allocates the plan's device buffers)
+        t_e2e = 0.0
+        for _ in range(n_e2e):
+            hu.copy_(hu0)                                     # host-side restore of one field, outside the timing
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            plan.projection_host(hu, hv, hw, hp, w.dt)       # H2D of u,v,w + kernels + D2H of u,v,w,Phi + sync
+            t_e2e += time.perf_counter() - t0
+        e2e = {"value": cells * n_e2e / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": 3 * 8 * cells,
+               "d2h_bytes_per_step": 4 * 8 * cells, "steps": n_e2e, "ms_per_step": 1e3 * t_e2e / n_e2e,
+               "api": "cans_projection_host (pinned host buffers)"}
+        del hu, hv, hw, hp, hu0
+
+    # ---- Poisson-only timings of the other configs (context; parity-test cases, not bench lines) ----
+    poisson = []
+    if not args.no_extra:
+        del u, v, ww, p
+        torch.cuda.empty_cache()
+        for name in ("C2", "C3", "C4", "C5"):
+            r = time_poisson_config(binding, workloads, torch, name)
+            r["frac_of_peak"] = r["min_bytes"] / (r["ms_median"] * 1e-3) / 1e9 / peak_gbs
+            poisson.append(r)
+
+    # ---- CPU baseline: the oracle on a bounded sample, host cores of this box ----
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu:
+        nz_sample = 32
+        ccells, times = time_oracle_sample(nz_sample, 1)
+        cpu_baseline = {"value": ccells / times[0] / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+                        "sample": f"oracle.projection on a 1024x768x{nz_sample} slab of C5 (same domain, bc, "
+                                  f"tanh recipe), {ccells} cells, {times[0]:.1f} s wall"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": WORKLOAD, "cells": cells, "l2_policy": "inputs (12.9 GB) larger than L2; "
+                   "u,v,w restored by device copies between timed steps", "parallelism": f"replicas x{world}"},
+        "roofline": roofline,
+        "roofline_step": {"bound": "hbm", "achieved": step_gbs, "peak": peak_gbs, "unit": "GB/s",
+                          "frac": step_gbs / peak_gbs, "frac_of_nominal_8TBs": step_gbs / 8000.0,
+                          "min_bytes_per_cell": STEP_MIN_BYTES_PER_CELL["projection"]},
+        "kernels": kernels,
+        "cpu_baseline": cpu_baseline,
+        "e2e": e2e,
+        "gpu_launches": plan.launches_per_projection * args.steps,
+        "clocks": clocks,
+        "poisson_configs": poisson,
+        "paper_context": "PAPER.md Table 1 (P:L274-284): 0.1404 s per full RK3 time step (3 projections + momentum), "
+                         "1536x768x576, 16x V100 DGX-2 -- whole time step on other hardware, not this metric",
+    }
+    print(json.dumps(line), flush=True)
+    plan.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
+    ap.add_argument("--no-extra", action="store_true", help="skip the Poisson-only timings of C2..C5")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

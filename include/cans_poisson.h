@@ -120,6 +120,17 @@ int cans_last_status(void);
 int cans_plan_launches_per_solve(const cans_poisson_plan* plan);
 int cans_plan_launches_per_projection(const cans_poisson_plan* plan);
 
+/*
+ * Optional per-kernel timing for bench.py.  With profiling enabled every kernel launch of the next
+ * cans_poisson_solve / cans_projection call is bracketed by a cudaEvent pair on the caller's stream.
+ * cans_plan_kernel_times waits for those events and writes the duration (ms) of each launch of the
+ * LAST call, in launch order, into ms[0..capacity); returns the number written, or -1 on error.
+ * cans_plan_kernel_name returns the name of launch idx of the last call ("" if out of range).
+ */
+int cans_plan_set_profiling(cans_poisson_plan* plan, int enable);
+int cans_plan_kernel_times(cans_poisson_plan* plan, float* ms, int capacity);
+const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
+
 /* "x.y" version string of the library. */
 const char* cans_version(void);
 

@@ -274,7 +274,7 @@ def poisson_solve(f, lx, ly, lz, bc, dzc=None, dzf=None):
         # O4: the exactly-zero eigenvalue sits at q = r = 0 for both PP and NN tables
         assert lam[0, 0] == 0.0
         d00 = fh[:, 0, 0].copy()
-        bfull[:, 0, 0] = 1.0           # placeholder so the vectorised sweep stays finite
+        bfull[:, 0, 0] = b - 1.0       # placeholder (non-singular, result discarded) so the vectorised sweep stays finite
     ph = solver(a, bfull, c, fh)
     if singular:
         if pz == "PP":

@@ -27,6 +27,7 @@ EXPORTED_SYMBOLS = (
     "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
+    "cans_plan_set_profiling", "cans_plan_kernel_times", "cans_plan_kernel_name",
 )
 
 
@@ -65,6 +66,12 @@ def _load() -> ctypes.CDLL:
     lib.cans_plan_launches_per_solve.argtypes = [vp]
     lib.cans_plan_launches_per_projection.restype = i32
     lib.cans_plan_launches_per_projection.argtypes = [vp]
+    lib.cans_plan_set_profiling.restype = i32
+    lib.cans_plan_set_profiling.argtypes = [vp, i32]
+    lib.cans_plan_kernel_times.restype = i32
+    lib.cans_plan_kernel_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32]
+    lib.cans_plan_kernel_name.restype = ctypes.c_char_p
+    lib.cans_plan_kernel_name.argtypes = [vp, i32]
     lib.cans_version.restype = ctypes.c_char_p
     lib.cans_version.argtypes = []
     return lib
@@ -167,6 +174,17 @@ class PoissonPlan:
         _check(_lib.cans_projection_host(self._h, _host_ptr(u, self.shape), _host_ptr(v, self.shape),
                                          _host_ptr(w, self.shape), _host_ptr(p, self.shape), float(dt),
                                          _stream_ptr(stream)))
+
+    def set_profiling(self, enable: bool):
+        _check(_lib.cans_plan_set_profiling(self._h, 1 if enable else 0))
+
+    def kernel_times(self):
+        """[(kernel name, ms)] of the last call, in launch order (profiling must be enabled)."""
+        buf = (ctypes.c_float * 8)()
+        n = _lib.cans_plan_kernel_times(self._h, buf, 8)
+        if n < 0:
+            raise CansError(_lib.cans_last_status(), last_error())
+        return [(_lib.cans_plan_kernel_name(self._h, i).decode(), float(buf[i])) for i in range(n)]
 
     @property
     def launches_per_solve(self) -> int:

@@ -106,6 +106,23 @@ struct cans_poisson_plan {
     double inv_lz;
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
+    // optional per-kernel timing (cans_plan_set_profiling): event pair around every launch
+    int prof;
+    int nrec;
+    cudaEvent_t ev[2 * 8];
+    const char* kname[8];
+};
+
+// bracket one kernel launch with events when profiling is on
+struct LaunchScope {
+    cans_poisson_plan* pl;
+    cudaStream_t st;
+    LaunchScope(cans_poisson_plan* p, cudaStream_t s, const char* name) : pl(p), st(s) {
+        if (pl->prof && pl->nrec < 8) { pl->kname[pl->nrec] = name; cudaEventRecord(pl->ev[2 * pl->nrec], st); }
+    }
+    ~LaunchScope() {
+        if (pl->prof && pl->nrec < 8) { cudaEventRecord(pl->ev[2 * pl->nrec + 1], st); pl->nrec++; }
+    }
 };
 
 static int kind_of(char lo, char up, int* kind) {
@@ -153,6 +170,7 @@ void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
     if (!plan) return;
     for (void* d : plan->dev_allocs) cudaFree(d);
     for (int i = 0; i < 4; ++i) if (plan->hostbuf[i]) cudaFree(plan->hostbuf[i]);
+    if (plan->prof) for (int i = 0; i < 16; ++i) cudaEventDestroy(plan->ev[i]);
     delete plan;
 }
 
@@ -197,6 +215,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->kind_x = kx; pl->kind_y = ky;
     pl->nseg = nseg; pl->nzp = nseg * Z_MROWS;
     for (int i = 0; i < 4; ++i) pl->hostbuf[i] = nullptr;
+    pl->prof = 0; pl->nrec = 0;
     pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
     int dev = 0;
     cudaGetDevice(&dev);
@@ -266,8 +285,11 @@ static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
     return a;
 }
 
-static int launch_xy_any(int n, int op, const XYArgs& a, cudaStream_t st) {
+static const char* const XY_NAMES[5] = {"x_fwd", "x_fwd_div", "x_inv", "y_fwd", "y_inv"};
+
+static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, cudaStream_t st) {
     cudaError_t err = cudaSuccess;
+    LaunchScope scope(pl, st, XY_NAMES[op]);
     if (launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||
         launch_xy_group_c(n, op, a, st, &err) || launch_xy_group_d(n, op, a, st, &err)) {
         if (err != cudaSuccess) return fail_cuda(err, "x/y transform launch");
@@ -276,8 +298,9 @@ static int launch_xy_any(int n, int op, const XYArgs& a, cudaStream_t st) {
     return fail(CANS_ERR_UNSUPPORTED_SIZE, "transform length not instantiated");
 }
 
-static int launch_z(const cans_poisson_plan* pl, double* p, cudaStream_t st) {
+static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
     ZArgs z = make_zargs(pl, p);
+    LaunchScope scope(pl, st, "z_solve");
     const int tc = z_tc_for(pl->nseg);
     const long ntiles = (z.ncols + tc - 1) / tc;
     const unsigned grid = (unsigned)(ntiles + (pl->singular ? 1 : 0));
@@ -294,13 +317,14 @@ static int launch_z(const cans_poisson_plan* pl, double* p, cudaStream_t st) {
 // the transform/solve/transform core shared by both entry points; `div` selects the fused-divergence load
 static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, cudaStream_t st) {
     int rc;
-    if (divargs) rc = launch_xy_any(pl->nx, OP_X_FWD_DIV, *divargs, st);
-    else rc = launch_xy_any(pl->nx, OP_X_FWD, make_xyargs(pl, p, true), st);
+    pl->nrec = 0;
+    if (divargs) rc = launch_xy_any(pl, pl->nx, OP_X_FWD_DIV, *divargs, st);
+    else rc = launch_xy_any(pl, pl->nx, OP_X_FWD, make_xyargs(pl, p, true), st);
     if (rc) return rc;
-    if ((rc = launch_xy_any(pl->ny, OP_Y_FWD, make_xyargs(pl, p, false), st))) return rc;
+    if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, make_xyargs(pl, p, false), st))) return rc;
     if ((rc = launch_z(pl, p, st))) return rc;
-    if ((rc = launch_xy_any(pl->ny, OP_Y_INV, make_xyargs(pl, p, false), st))) return rc;
-    if ((rc = launch_xy_any(pl->nx, OP_X_INV, make_xyargs(pl, p, true), st))) return rc;
+    if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, make_xyargs(pl, p, false), st))) return rc;
+    if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, make_xyargs(pl, p, true), st))) return rc;
     return CANS_OK;
 }
 
@@ -355,10 +379,49 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     size_t blocks = (npair + 255) / 256;
     const size_t cap = (size_t)plan->num_sms * 32;
     if (blocks > cap) blocks = cap;
-    grad_correct_kernel<<<(unsigned)blocks, 256, 0, st>>>(g);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e;
+    {
+        LaunchScope scope(plan, st, "grad_correct");
+        grad_correct_kernel<<<(unsigned)blocks, 256, 0, st>>>(g);
+        e = cudaGetLastError();
+    }
     if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
     return CANS_OK;
+}
+
+int cans_plan_set_profiling(cans_poisson_plan* plan, int enable) {
+    g_status = CANS_OK;
+    if (!plan) return fail(CANS_ERR_INVALID_ARG, "plan is NULL");
+    if (enable && !plan->prof) {
+        for (int i = 0; i < 16; ++i) {
+            cudaError_t e = cudaEventCreate(&plan->ev[i]);
+            if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
+        }
+        plan->prof = 1;
+    } else if (!enable && plan->prof) {
+        for (int i = 0; i < 16; ++i) cudaEventDestroy(plan->ev[i]);
+        plan->prof = 0;
+    }
+    plan->nrec = 0;
+    return CANS_OK;
+}
+
+int cans_plan_kernel_times(cans_poisson_plan* plan, float* ms, int capacity) {
+    g_status = CANS_OK;
+    if (!plan || !ms) { fail(CANS_ERR_INVALID_ARG, "NULL argument"); return -1; }
+    if (!plan->prof) { fail(CANS_ERR_INVALID_ARG, "profiling is not enabled"); return -1; }
+    int n = plan->nrec < capacity ? plan->nrec : capacity;
+    for (int i = 0; i < n; ++i) {
+        cudaError_t e = cudaEventSynchronize(plan->ev[2 * i + 1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms[i], plan->ev[2 * i], plan->ev[2 * i + 1]);
+        if (e != cudaSuccess) { fail_cuda(e, "kernel timing"); return -1; }
+    }
+    return n;
+}
+
+const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx) {
+    if (!plan || idx < 0 || idx >= plan->nrec) return "";
+    return plan->kname[idx];
 }
 
 int cans_projection_set_lower_face(cans_poisson_plan* plan, int dir, double* face_plane) {
