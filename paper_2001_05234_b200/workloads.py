@@ -75,6 +75,18 @@ def kolmogorov_field(shape, lengths, seed: int, device="cpu") -> torch.Tensor:
     nz, ny, nx = shape
     lx, ly, lz = lengths
     x = gaussian_field(shape, seed, device)
+    if torch.device(device).type == "cpu":
+        # numpy's FFT on the host (torch's CPU irfftn aborted with heap corruption on the 16-core GPU box)
+        import numpy as np
+        xh = np.fft.rfftn(x.numpy())
+        kx = 2.0 * math.pi * np.fft.rfftfreq(nx, d=lx / nx)
+        ky = 2.0 * math.pi * np.fft.fftfreq(ny, d=ly / ny)
+        kz = 2.0 * math.pi * np.fft.fftfreq(nz, d=lz / nz)
+        k2 = kz[:, None, None] ** 2 + ky[None, :, None] ** 2 + kx[None, None, :] ** 2
+        filt = np.where(k2 > 0, np.maximum(k2, 1e-300) ** (-11.0 / 12.0), 0.0)
+        y = np.fft.irfftn(xh * filt, s=shape, axes=(0, 1, 2))
+        y /= np.sqrt(np.mean(y * y))
+        return torch.from_numpy(np.ascontiguousarray(y))
     xh = torch.fft.rfftn(x)
     del x
     kx = 2.0 * math.pi * torch.fft.rfftfreq(nx, d=lx / nx).to(device)
