@@ -32,7 +32,9 @@ def B():
 
 
 def rel_l2(a, b):
-    return np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel())
+    nb = np.linalg.norm(b.ravel())
+    d = np.linalg.norm((a - b).ravel())
+    return d / nb if nb > 0 else d        # absolute form when the reference vanishes (e.g. the wall plane of w)
 
 
 def op_norm_inf(w):
