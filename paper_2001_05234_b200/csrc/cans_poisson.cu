@@ -19,7 +19,7 @@
 #include "../../include/cans_poisson.h"
 #include "plan_tables.hpp"
 #include "xy_kernels.cuh"
-#include "z_pass.cuh"
+#include "z_kernels.cuh"
 #include "grad_pass.cuh"
 
 namespace cans {
@@ -34,45 +34,6 @@ static int fail(int code, const std::string& msg) {
 }
 static int fail_cuda(cudaError_t e, const char* where) {
     return fail(CANS_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
-}
-
-constexpr int Z_MROWS = 16;   // rows per thread in the z solve
-// columns per CTA: 16 consecutive x-indices (128 B per row) while the CTA stays <= 512 threads
-// (nz <= 512), else 8 (nz <= 1024)
-static int z_tc_for(int nseg) { return nseg <= 32 ? 16 : 8; }
-
-// ------------------------------------------------------------------------------------------------
-// z kernels
-// ------------------------------------------------------------------------------------------------
-template <int MROWS, int TC>
-__global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a) {
-    extern __shared__ __align__(16) double zsm[];
-    typedef ZPass<MROWS, TC> Z;
-    const int tid = threadIdx.x;
-    const int nthreads = blockDim.x;
-    if (a.singular && blockIdx.x == gridDim.x - 1) {
-        // extra CTA: the singular (0,0) column, staged in shared memory, solved by one thread
-        for (int k = tid; k < a.nz; k += nthreads) zsm[k] = a.p[(size_t)k * a.ncols];
-        __syncthreads();
-        if (tid == 0) z_singular_column(a, zsm);
-        return;
-    }
-    Z::load_tables(a, zsm, tid, nthreads);
-    __syncthreads();
-    ZState<MROWS> st;
-    Z::phase1(a, zsm, st, (long)blockIdx.x, tid);
-    __syncthreads();
-    Z::phase2a(a, zsm, st, tid);
-    __syncthreads();
-    Z::phase2b(a, zsm, st, tid);
-    __syncthreads();
-    Z::phase3(a, zsm, st, tid);
-}
-
-template <int MROWS>
-__global__ void z_setup_kernel(const ZArgs a, double* rstart, double* r00) {
-    const long col = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (col < a.ncols) z_setup_column<MROWS>(a, rstart, r00, col);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -99,6 +60,10 @@ struct cans_poisson_plan {
     int singular;
     int nseg, nzp;
     int num_sms;
+    int z_grid;               // persistent grid of the z solve
+    size_t z_smem;
+    unsigned int* sched;      // scheduler state (tickets, per-plane counters), zeroed at the start of every call
+    size_t sched_bytes;
     std::vector<void*> dev_allocs;
     // device tables
     double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc, *rstart, *r00;
@@ -143,6 +108,9 @@ static cudaError_t upload(cans_poisson_plan* pl, const std::vector<double>& h, T
     return e;
 }
 
+// layout of the scheduler state (unsigned ints)
+enum { SCHED_Z_TICKET = 0, SCHED_A_TICKET = 1, SCHED_C_TICKET = 2, SCHED_ERR = 3, SCHED_PLANES = 8 };
+
 static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
     ZArgs z;
     z.nx = pl->nx; z.ny = pl->ny; z.nz = pl->nz;
@@ -157,6 +125,9 @@ static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
     z.r00 = pl->r00;
     z.dzf = pl->dzf;
     z.inv_lz = pl->inv_lz;
+    const int tc = z_tc_for(pl->nseg);
+    z.ntiles = (z.ncols + tc - 1) / tc;
+    z.ticket = pl->sched + SCHED_Z_TICKET;
     return z;
 }
 
@@ -249,20 +220,16 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->r00 = (double*)d; }
     }
     if (e == cudaSuccess) {
-        ZArgs z = make_zargs(pl, nullptr);
-        const long ncols = z.ncols;
-        z_setup_kernel<Z_MROWS><<<(unsigned)((ncols + 127) / 128), 128>>>(z, pl->rstart, pl->r00);
-        e = cudaGetLastError();
-        if (e == cudaSuccess) e = cudaDeviceSynchronize();
+        pl->sched_bytes = sizeof(unsigned int) * (size_t)(SCHED_PLANES + 4 * (nz + 4));
+        void* d = nullptr;
+        e = cudaMalloc(&d, pl->sched_bytes);
+        if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->sched = (unsigned int*)d; e = cudaMemset(d, 0, pl->sched_bytes); }
     }
     if (e == cudaSuccess) {
-        size_t zsmem = sizeof(double) * ZPass<Z_MROWS, 16>::smem_doubles(nseg);
-        if (sizeof(double) * (size_t)nz > zsmem) zsmem = sizeof(double) * (size_t)nz;
-        if (z_tc_for(nseg) == 16)
-            e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zsmem);
-        else
-            e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)zsmem);
+        ZArgs z = make_zargs(pl, nullptr);
+        e = z_setup_launch(z, pl->rstart, pl->r00);
     }
+    if (e == cudaSuccess) e = z_solve_configure(nseg, nz, pl->num_sms, &pl->z_grid, &pl->z_smem);
     if (e != cudaSuccess) {
         const bool oom = (e == cudaErrorMemoryAllocation);
         std::string msg = std::string("plan creation: ") + cudaGetErrorString(e);
@@ -301,15 +268,7 @@ static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, 
 static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
     ZArgs z = make_zargs(pl, p);
     LaunchScope scope(pl, st, "z_solve");
-    const int tc = z_tc_for(pl->nseg);
-    const long ntiles = (z.ncols + tc - 1) / tc;
-    const unsigned grid = (unsigned)(ntiles + (pl->singular ? 1 : 0));
-    size_t smem = sizeof(double) * (tc == 16 ? ZPass<Z_MROWS, 16>::smem_doubles(pl->nseg)
-                                             : ZPass<Z_MROWS, 8>::smem_doubles(pl->nseg));
-    if (pl->singular && sizeof(double) * (size_t)pl->nz > smem) smem = sizeof(double) * (size_t)pl->nz;
-    if (tc == 16) z_solve_kernel<Z_MROWS, 16><<<grid, 16 * pl->nseg, smem, st>>>(z);
-    else z_solve_kernel<Z_MROWS, 8><<<grid, 8 * pl->nseg, smem, st>>>(z);
-    cudaError_t e = cudaGetLastError();
+    cudaError_t e = z_solve_launch(z, pl->z_grid, pl->z_smem, st);
     if (e != cudaSuccess) return fail_cuda(e, "z solve launch");
     return CANS_OK;
 }
@@ -318,6 +277,8 @@ static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
 static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, cudaStream_t st) {
     int rc;
     pl->nrec = 0;
+    cudaError_t me = cudaMemsetAsync(pl->sched, 0, pl->sched_bytes, st);
+    if (me != cudaSuccess) return fail_cuda(me, "scheduler reset");
     if (divargs) rc = launch_xy_any(pl, pl->nx, OP_X_FWD_DIV, *divargs, st);
     else rc = launch_xy_any(pl, pl->nx, OP_X_FWD, make_xyargs(pl, p, true), st);
     if (rc) return rc;

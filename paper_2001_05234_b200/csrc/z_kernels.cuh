@@ -1,0 +1,20 @@
+// z_kernels.cuh -- host-callable launchers of the z-solve kernels (defined in z_solve.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include "z_pass.cuh"
+
+namespace cans {
+
+constexpr int Z_MROWS = 16;   // rows per thread in the z solve
+
+// columns per CTA for a given segment count (threads = TC * nseg <= 512)
+inline int z_tc_for(int nseg) { return nseg <= 16 ? 32 : (nseg <= 32 ? 16 : 8); }
+
+// plan time: opt in to the dynamic shared memory of the solve kernel and compute the persistent grid
+cudaError_t z_solve_configure(int nseg, int nz, int num_sms, int* grid_out, size_t* smem_out);
+// enqueue the solve (a.ticket must point at a zeroed counter)
+cudaError_t z_solve_launch(const ZArgs& a, int grid, size_t smem, cudaStream_t st);
+// plan time: fill rstart / r00 (synchronous)
+cudaError_t z_setup_launch(const ZArgs& a, double* rstart, double* r00);
+
+}  // namespace cans

@@ -6,17 +6,23 @@
 // Thomas recurrence (same algebra as the sequential algorithm):
 //   r_k = 1 / (b_k + lam - a_k c_{k-1} r_{k-1}),  d'_k = (d_k - a_k d'_{k-1}) r_k,  x_k = d'_k - c_k r_k x_{k+1}
 //
-// B200 mapping ("register-resident partitioned Thomas"): a column is cut into P segments of MROWS rows;
-// thread (c, s) owns segment s of column c with its MROWS right-hand sides in registers, so a warp
-// reads/writes 16-32 consecutive x-indices per row (coalesced) and the whole column never leaves the
-// SM between the forward and backward sweeps (16 B/cell of HBM traffic, the structural minimum).
+// B200 mapping ("register-resident partitioned Thomas", fed by an asynchronous tile pipeline):
+//   * a CTA is persistent and draws tiles of TC consecutive columns (x fastest => TC*8 contiguous
+//     bytes per row) from a global ticket counter; the tile of the NEXT ticket is copied global ->
+//     shared with cp.async (LDGSTS, 16 B per thread, no register staging) while the current tile is
+//     being solved, so HBM reads stay in flight during the whole arithmetic phase;
+//   * a column is cut into P segments of MROWS rows; thread (c, s) owns segment s of column c with
+//     its MROWS right-hand sides in registers; the whole column never leaves the SM between the
+//     forward and backward sweeps (16 B/cell of HBM traffic, the structural minimum);
 //   * the pivot chain r_k is restarted at every segment from a plan-time table r_{k0-1}(mode, s)
 //     (nx*ny*P doubles, 1/MROWS of a field) and recomputed in-register -- bit-identical to the
 //     sequential pivots;
 //   * d' and x are first-order linear recurrences: each segment runs them from a zero start while
 //     accumulating the propagation factor (prod of -a_k r_k, resp. -c_k r_k); a P-step scan over the
-//     segment ends in shared memory supplies the true start value, which is then propagated.
-// The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_column.
+//     segment ends in shared memory supplies the true start value, which is then propagated;
+//   * results go straight from registers to global memory (coalesced rows).
+// The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_column
+// (CTA 0, before it joins the tile loop).
 #pragma once
 #include "common.cuh"
 
@@ -26,6 +32,7 @@ struct ZArgs {
     int nx, ny, nz;
     int nseg;                 // P = ceil(nz / MROWS)
     long ncols;               // nx * ny
+    long ntiles;              // ceil(ncols / TC)
     double* p;                // field, solved in place
     const double* lamx;       // [nx]  lam_x(position)/dx^2
     const double* lamy;       // [ny]  lam_y(position)/dy^2
@@ -35,16 +42,27 @@ struct ZArgs {
     const double* gz;         // a_k * c_{k-1}                        (0 for k = 0 and beyond nz)
     const double* rstart;     // [nseg][ncols]  r_{s*MROWS-1}(column)  (0 for s = 0)
     double scale;             // 1/(nx*ny): normalisation of the two unnormalised inverse FFTs
-    int singular;             // 1: column 0 is the singular mode, skipped here
+    int singular;             // 1: column 0 is the singular mode, skipped by the tile path
     const double* r00;        // [nz] pivots of the singular column (rows 0..nz-2), plan-time
     const double* dzf;        // [nz]
     double inv_lz;            // 1 / sum(dzf)
+    unsigned int* ticket;     // tile ticket counter (zeroed before the launch)
 };
 
 // one pivot step; shared by the plan-time table kernel and the solve so the values are identical
 CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) {
     return 1.0 / ((bk + lam) - gk * rprev);
 }
+
+#if defined(__CUDACC__)
+CANS_D void cp_async16(void* smem_dst, const void* gmem_src) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem_src) : "memory");
+}
+CANS_D void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+CANS_D void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+#endif
 
 template <int MROWS>
 struct ZState {
@@ -55,10 +73,13 @@ struct ZState {
     bool active;
 };
 
-// shared memory: tables az,bz,cz,gz [4][nzp] then scan arrays end[TC*P], fac[TC*P]
+// shared memory (doubles): tables az,bz,cz,gz [4][nzp]; scan arrays end[TC*P], fac[TC*P];
+// two tile buffers [nzp][TC]
 template <int MROWS, int TC>
 struct ZPass {
-    static CANS_HD size_t smem_doubles(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)2 * TC * nseg; }
+    static CANS_HD size_t table_doubles(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)2 * TC * nseg; }
+    static CANS_HD size_t tile_doubles(int nseg) { return (size_t)nseg * MROWS * TC; }
+    static CANS_HD size_t smem_doubles(int nseg) { return table_doubles(nseg) + 2 * tile_doubles(nseg); }
 
     static CANS_HD void load_tables(const ZArgs& a, double* sm, int tid, int nthreads) {
         const int nzp = a.nseg * MROWS;
@@ -70,8 +91,33 @@ struct ZPass {
         }
     }
 
-    // phase 1: load the segment, pivots, local forward sweep from a zero start; publish (end, factor)
-    static CANS_HD void phase1(const ZArgs& a, double* sm, ZState<MROWS>& st, long tile, int tid) {
+#if defined(__CUDACC__)
+    // asynchronous copy of tile `tile` (rows 0..nz-1, TC columns) into buf[k*TC + c]
+    static CANS_D void prefetch_tile(const ZArgs& a, double* buf, long tile, int tid, int nthreads) {
+        constexpr int CH = TC / 2;                      // 16-byte chunks per row
+        const long col0 = tile * TC;
+        const size_t plane = (size_t)a.ncols;
+        const int nchunks = a.nz * CH;
+        if (col0 + TC <= a.ncols) {
+            for (int id = tid; id < nchunks; id += nthreads) {
+                const int k = id / CH;
+                const int q = id - k * CH;
+                cp_async16(buf + (size_t)k * TC + 2 * q, a.p + (size_t)k * plane + col0 + 2 * q);
+            }
+        } else {                                        // ragged last tile: plain guarded loads
+            for (int id = tid; id < a.nz * TC; id += nthreads) {
+                const int k = id / TC;
+                const int c = id - k * TC;
+                buf[(size_t)k * TC + c] = (col0 + c < a.ncols) ? a.p[(size_t)k * plane + col0 + c] : 0.0;
+            }
+        }
+    }
+#endif
+
+    // phase 1: take the segment from the tile buffer, pivots, local forward sweep from a zero start;
+    // publish (end, factor)
+    static CANS_HD void phase1(const ZArgs& a, double* sm, const double* buf, ZState<MROWS>& st, long tile,
+                               double rstart_val, double lam, int tid) {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
         const double* sbz = sm + nzp;
@@ -84,17 +130,13 @@ struct ZPass {
         st.col = col;
         st.active = (col < a.ncols) && !(a.singular && col == 0);
         const int k0 = s * MROWS;
-        const size_t plane = (size_t)a.ncols;
         if (col < a.ncols) {
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
                 const int k = k0 + r;
-                st.d[r] = (k < a.nz) ? a.p[(size_t)k * plane + col] * a.scale : 0.0;
+                st.d[r] = (k < a.nz) ? buf[(size_t)k * TC + c] * a.scale : 0.0;
             }
-            const int i = (int)(col % a.nx);
-            const int j = (int)(col / a.nx);
-            const double lam = a.lamx[i] + a.lamy[j];
-            double rp = a.rstart[(size_t)s * a.ncols + col];
+            double rp = rstart_val;
             double dp = 0.0, fac = 1.0;
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
