@@ -38,6 +38,11 @@ KERNEL_BYTES_PER_CELL = {
     "y_inv": 16.0,
     "x_inv": 16.0,
     "grad_correct": 56.0,  # read Phi (8) + u, v, w (24), write u, v, w (24)
+    # fused persistent kernels (intermediate plane stays in L2)
+    "xy_fwd_div": 32.0,    # pass A: read u, v, w (24) + write f^ (8)
+    "xy_fwd": 16.0,
+    "xy_inv": 16.0,
+    "xy_inv_grad": 64.0,   # pass C: read Phi^ (8) + u, v, w (24), write Phi (8) + u, v, w (24)
 }
 STEP_MIN_BYTES_PER_CELL = {"projection": 112.0, "poisson": 48.0}   # structural minimum, SURVEY.md 8(d)
 

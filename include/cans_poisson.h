@@ -131,6 +131,18 @@ int cans_plan_set_profiling(cans_poisson_plan* plan, int enable);
 int cans_plan_kernel_times(cans_poisson_plan* plan, float* ms, int capacity);
 const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
 
+/*
+ * cans_plan_set_fusion -- switch between the two launch sequences of a plan (both are this library's
+ * CUDA kernels and run the same phase functions, so results are bit-identical):
+ *   fused   (default when nx and ny are both in {256,384,512,768,1024}): pass A = divergence + x + y
+ *           forward transforms and pass C = y + x inverse transforms + gradient correction, each one
+ *           persistent kernel whose intermediate plane stays in L2 (3 launches per call);
+ *   unfused one kernel per step of SURVEY 8(a) (5 launches per solve, 6 per projection).
+ * Returns the resulting state (1 fused, 0 unfused); a NULL plan sets the thread's status to
+ * CANS_ERR_INVALID_ARG and returns 0.
+ */
+int cans_plan_set_fusion(cans_poisson_plan* plan, int enable);
+
 /* "x.y" version string of the library. */
 const char* cans_version(void);
 

@@ -28,6 +28,7 @@ EXPORTED_SYMBOLS = (
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
     "cans_plan_set_profiling", "cans_plan_kernel_times", "cans_plan_kernel_name",
+    "cans_plan_set_fusion",
 )
 
 
@@ -68,6 +69,8 @@ def _load() -> ctypes.CDLL:
     lib.cans_plan_launches_per_projection.argtypes = [vp]
     lib.cans_plan_set_profiling.restype = i32
     lib.cans_plan_set_profiling.argtypes = [vp, i32]
+    lib.cans_plan_set_fusion.restype = i32
+    lib.cans_plan_set_fusion.argtypes = [vp, i32]
     lib.cans_plan_kernel_times.restype = i32
     lib.cans_plan_kernel_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32]
     lib.cans_plan_kernel_name.restype = ctypes.c_char_p
@@ -177,6 +180,10 @@ class PoissonPlan:
 
     def set_profiling(self, enable: bool):
         _check(_lib.cans_plan_set_profiling(self._h, 1 if enable else 0))
+
+    def set_fusion(self, enable: bool) -> bool:
+        """Select the fused (3 launches) or unfused launch sequence; returns the resulting state."""
+        return bool(_lib.cans_plan_set_fusion(self._h, 1 if enable else 0))
 
     def kernel_times(self):
         """[(kernel name, ms)] of the last call, in launch order (profiling must be enabled)."""

@@ -15,7 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libcans_poisson.so")
-SOURCES = ["cans_poisson.cu", "z_solve.cu", "xy_group_a.cu", "xy_group_b.cu", "xy_group_c.cu", "xy_group_d.cu"]
+SOURCES = ["fused_x1024.cu", "fused_x768.cu", "fused_x512.cu", "fused_x384.cu", "fused_x256.cu", "cans_poisson.cu", "z_solve.cu",
+           "xy_group_a.cu", "xy_group_b.cu", "xy_group_c.cu", "xy_group_d.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v", "-I", os.path.join(ROOT, "include"),
@@ -56,7 +57,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError(f"nvcc failed on {src}:\n{r.stdout}\n{r.stderr}")
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+    with ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(compile_one, SOURCES))
     cmd = [nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
     r = subprocess.run(cmd, capture_output=True, text=True)

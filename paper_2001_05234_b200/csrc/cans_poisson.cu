@@ -21,6 +21,7 @@
 #include "xy_kernels.cuh"
 #include "z_kernels.cuh"
 #include "grad_pass.cuh"
+#include "fused_kernels.cuh"
 
 namespace cans {
 
@@ -45,6 +46,58 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
         grad_correct_pair(a, t);
 }
 
+bool fused_dispatch(int nx, int ny, int what, const FusedArgs* a, int num_sms, int* grid, size_t* smem,
+                    cudaStream_t st, cudaError_t* err) {
+    switch (nx) {
+        case 256: return fused_dispatch_256(ny, what, a, num_sms, grid, smem, st, err);
+        case 384: return fused_dispatch_384(ny, what, a, num_sms, grid, smem, st, err);
+        case 512: return fused_dispatch_512(ny, what, a, num_sms, grid, smem, st, err);
+        case 768: return fused_dispatch_768(ny, what, a, num_sms, grid, smem, st, err);
+        case 1024: return fused_dispatch_1024(ny, what, a, num_sms, grid, smem, st, err);
+        default: return false;
+    }
+}
+
+// Ticket order of the fused passes (fused_pass.cuh).  Counter indices: pass A x-done [0, nz);
+// pass C y-done [nz+4, 2nz+4), x-done [2(nz+4), 3nz+8).  LAG planes separate a producer from its consumer in
+// the ticket order so that the consumer rarely has to spin.
+static std::vector<Segment> build_segments(int nz, int nxt, int nyt, int ngt, bool inv, bool grad, unsigned* total) {
+    std::vector<Segment> v;
+    unsigned first = 0;
+    auto add = [&](int type, int k, unsigned count, int dep0, unsigned t0, int dep1, unsigned t1, int signal) {
+        Segment s;
+        s.first = first; s.count = count; s.type = type; s.k = k;
+        s.dep0 = dep0; s.target0 = t0; s.dep1 = dep1; s.target1 = t1; s.signal = signal; s.pad = 0;
+        v.push_back(s);
+        first += count;
+    };
+    const int stride = nz + 4;
+    if (!inv) {
+        const int LAG = 2;
+        for (int k = 0; k < LAG && k < nz; ++k) add(TASK_X, k, nxt, -1, 0, -1, 0, k);
+        for (int k = 0; k < nz; ++k) {
+            if (k + LAG < nz) add(TASK_X, k + LAG, nxt, -1, 0, -1, 0, k + LAG);
+            add(TASK_Y, k, nyt, k, nxt, -1, 0, -1);
+        }
+    } else {
+        const int LAG = 1;
+        for (int r = 0; r < nz + 2 * LAG + 1; ++r) {
+            if (r < nz) add(TASK_Y, r, nyt, -1, 0, -1, 0, stride + r);
+            const int kx = r - LAG;
+            if (kx >= 0 && kx < nz) add(TASK_X, kx, nxt, stride + kx, nyt, -1, 0, 2 * stride + kx);
+            const int kg = r - 2 * LAG - 1;
+            if (grad && kg >= 0 && kg < nz)
+                add(TASK_G, kg, ngt, 2 * stride + kg, nxt, (kg + 1 < nz) ? 2 * stride + kg + 1 : -1, nxt, -1);
+        }
+    }
+    *total = first;
+    Segment s;
+    s.first = first; s.count = 0xffffffffu; s.type = -1; s.k = 0;
+    s.dep0 = s.dep1 = s.signal = -1; s.target0 = s.target1 = 0; s.pad = 0;
+    v.push_back(s);
+    return v;
+}
+
 }  // namespace cans
 
 using namespace cans;
@@ -62,6 +115,12 @@ struct cans_poisson_plan {
     int num_sms;
     int z_grid;               // persistent grid of the z solve
     size_t z_smem;
+    // fused passes A / C (fused_pass.cuh): persistent grid, ticket tables
+    int fused;                // 1: (nx, ny) has fused kernels and fusion is enabled
+    int fused_grid;
+    size_t fused_smem;
+    Segment *seg_a, *seg_c, *seg_cg;      // pass A; pass C without / with gradient tasks
+    unsigned tot_a, tot_c, tot_cg;
     unsigned int* sched;      // scheduler state (tickets, per-plane counters), zeroed at the start of every call
     size_t sched_bytes;
     std::vector<void*> dev_allocs;
@@ -187,6 +246,8 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->nseg = nseg; pl->nzp = nseg * Z_MROWS;
     for (int i = 0; i < 4; ++i) pl->hostbuf[i] = nullptr;
     pl->prof = 0; pl->nrec = 0;
+    pl->seg_a = pl->seg_c = pl->seg_cg = nullptr;
+    pl->fused = 0;
     pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
     int dev = 0;
     cudaGetDevice(&dev);
@@ -230,6 +291,29 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         e = z_setup_launch(z, pl->rstart, pl->r00);
     }
     if (e == cudaSuccess) e = z_solve_configure(nseg, nz, pl->num_sms, &pl->z_grid, &pl->z_smem);
+    pl->fused = 0;
+    if (e == cudaSuccess && fused_supported(nx, ny)) {
+        cudaError_t fe = cudaSuccess;
+        if (fused_dispatch(nx, ny, 0, nullptr, pl->num_sms, &pl->fused_grid, &pl->fused_smem, 0, &fe)) e = fe;
+        if (e == cudaSuccess) {
+            const int nxt = (ny / 2 + fused_nfx(nx) - 1) / fused_nfx(nx);
+            const int nyt = (nx / 2) / fused_txc(ny);
+            const int ngt = (ny + FUSED_GROWS - 1) / FUSED_GROWS;
+            auto upseg = [&](const std::vector<Segment>& h, Segment** d) {
+                if (e != cudaSuccess) return;
+                void* dv = nullptr;
+                e = cudaMalloc(&dv, h.size() * sizeof(Segment));
+                if (e != cudaSuccess) return;
+                pl->dev_allocs.push_back(dv);
+                e = cudaMemcpy(dv, h.data(), h.size() * sizeof(Segment), cudaMemcpyHostToDevice);
+                *d = (Segment*)dv;
+            };
+            upseg(build_segments(nz, nxt, nyt, ngt, false, false, &pl->tot_a), &pl->seg_a);
+            upseg(build_segments(nz, nxt, nyt, ngt, true, false, &pl->tot_c), &pl->seg_c);
+            upseg(build_segments(nz, nxt, nyt, ngt, true, true, &pl->tot_cg), &pl->seg_cg);
+            pl->fused = 1;
+        }
+    }
     if (e != cudaSuccess) {
         const bool oom = (e == cudaErrorMemoryAllocation);
         std::string msg = std::string("plan creation: ") + cudaGetErrorString(e);
@@ -273,12 +357,59 @@ static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
     return CANS_OK;
 }
 
-// the transform/solve/transform core shared by both entry points; `div` selects the fused-divergence load
-static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, cudaStream_t st) {
+static int launch_fused(cans_poisson_plan* pl, bool inv, double* p, const XYArgs* divargs, const GradArgs* grad,
+                        cudaStream_t st) {
+    FusedArgs f;
+    std::memset(&f, 0, sizeof(f));
+    f.ax = (divargs && !inv) ? *divargs : make_xyargs(pl, p, true);
+    f.ay = make_xyargs(pl, p, false);
+    if (grad) f.g = *grad;
+    f.counters = pl->sched + SCHED_PLANES;
+    f.lookahead = (unsigned)pl->fused_grid;
+    f.grows = FUSED_GROWS;
+    const char* name;
+    if (!inv) {
+        f.segs = pl->seg_a; f.total = pl->tot_a; f.ticket = pl->sched + SCHED_A_TICKET;
+        f.mode = divargs ? 1 : 0;
+        name = divargs ? "xy_fwd_div" : "xy_fwd";
+    } else {
+        f.segs = grad ? pl->seg_cg : pl->seg_c; f.total = grad ? pl->tot_cg : pl->tot_c;
+        f.ticket = pl->sched + SCHED_C_TICKET;
+        f.mode = grad ? 1 : 0;
+        name = grad ? "xy_inv_grad" : "xy_inv";
+    }
+    LaunchScope scope(pl, st, name);
+    cudaError_t err = cudaSuccess;
+    if (!fused_dispatch(pl->nx, pl->ny, inv ? 2 : 1, &f, pl->num_sms, &pl->fused_grid, &pl->fused_smem, st, &err))
+        return fail(CANS_ERR_UNSUPPORTED_SIZE, "fused kernels not instantiated for this (nx, ny)");
+    if (err != cudaSuccess) return fail_cuda(err, "fused x/y launch");
+    return CANS_OK;
+}
+
+static int launch_grad(cans_poisson_plan* pl, const GradArgs& g, cudaStream_t st) {
+    const size_t npair = (size_t)pl->nx / 2 * pl->ny * pl->nz;
+    size_t blocks = (npair + 255) / 256;
+    const size_t cap = (size_t)pl->num_sms * 32;
+    if (blocks > cap) blocks = cap;
+    LaunchScope scope(pl, st, "grad_correct");
+    grad_correct_kernel<<<(unsigned)blocks, 256, 0, st>>>(g);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
+    return CANS_OK;
+}
+
+// the whole path shared by both entry points; `divargs` selects the fused-divergence load (a1),
+// `grad` the velocity correction (a7)
+static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st) {
     int rc;
     pl->nrec = 0;
     cudaError_t me = cudaMemsetAsync(pl->sched, 0, pl->sched_bytes, st);
     if (me != cudaSuccess) return fail_cuda(me, "scheduler reset");
+    if (pl->fused) {
+        if ((rc = launch_fused(pl, false, p, divargs, nullptr, st))) return rc;
+        if ((rc = launch_z(pl, p, st))) return rc;
+        return launch_fused(pl, true, p, nullptr, grad, st);
+    }
     if (divargs) rc = launch_xy_any(pl, pl->nx, OP_X_FWD_DIV, *divargs, st);
     else rc = launch_xy_any(pl, pl->nx, OP_X_FWD, make_xyargs(pl, p, true), st);
     if (rc) return rc;
@@ -286,17 +417,25 @@ static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, cud
     if ((rc = launch_z(pl, p, st))) return rc;
     if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, make_xyargs(pl, p, false), st))) return rc;
     if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, make_xyargs(pl, p, true), st))) return rc;
+    if (grad) return launch_grad(pl, *grad, st);
     return CANS_OK;
 }
 
-int cans_plan_launches_per_solve(const cans_poisson_plan*) { return 5; }
-int cans_plan_launches_per_projection(const cans_poisson_plan*) { return 6; }
+int cans_plan_set_fusion(cans_poisson_plan* plan, int enable) {
+    g_status = CANS_OK;
+    if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
+    plan->fused = (enable && plan->seg_a != nullptr) ? 1 : 0;
+    return plan->fused;
+}
+
+int cans_plan_launches_per_solve(const cans_poisson_plan* plan) { return (plan && plan->fused) ? 3 : 5; }
+int cans_plan_launches_per_projection(const cans_poisson_plan* plan) { return (plan && plan->fused) ? 3 : 6; }
 
 int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream) {
     g_status = CANS_OK;
     if (!plan || !p) return fail(CANS_ERR_INVALID_ARG, "plan and p must be non-NULL");
     if ((reinterpret_cast<size_t>(p) & 15) != 0) return fail(CANS_ERR_INVALID_ARG, "p must be 16-byte aligned");
-    return run_core(plan, p, nullptr, (cudaStream_t)stream);
+    return run_core(plan, p, nullptr, nullptr, (cudaStream_t)stream);
 }
 
 int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double dt, void* stream) {
@@ -319,8 +458,6 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     a.wrap_x = plan->bc[0][0] == 'P';
     a.wrap_y = plan->bc[1][0] == 'P';
     a.wrap_z = plan->bc[2][0] == 'P';
-    int rc = run_core(plan, p, &a, st);
-    if (rc) return rc;
     GradArgs g;
     g.nx = plan->nx; g.ny = plan->ny; g.nz = plan->nz;
     g.u = u; g.v = v; g.w = w; g.phi = p;
@@ -336,18 +473,7 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     ghost(plan->bc[0][1], plan->nx, &g.gx_idx, &g.gx_sgn);
     ghost(plan->bc[1][1], plan->ny, &g.gy_idx, &g.gy_sgn);
     ghost(plan->bc[2][1], plan->nz, &g.gz_idx, &g.gz_sgn);
-    const size_t npair = (size_t)plan->nx / 2 * plan->ny * plan->nz;
-    size_t blocks = (npair + 255) / 256;
-    const size_t cap = (size_t)plan->num_sms * 32;
-    if (blocks > cap) blocks = cap;
-    cudaError_t e;
-    {
-        LaunchScope scope(plan, st, "grad_correct");
-        grad_correct_kernel<<<(unsigned)blocks, 256, 0, st>>>(g);
-        e = cudaGetLastError();
-    }
-    if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
-    return CANS_OK;
+    return run_core(plan, p, &a, &g, st);
 }
 
 int cans_plan_set_profiling(cans_poisson_plan* plan, int enable) {

@@ -38,6 +38,17 @@ CANS_HD cplx cmulc(cplx a, cplx b) {
 CANS_HD cplx cmul_mi(cplx a) { return make_double2(a.y, -a.x); }
 CANS_HD cplx cmul_pi(cplx a) { return make_double2(-a.y, a.x); }
 
+// 16-byte load of the field being transformed in place.  L2-only (ld.global.cg): inside the fused
+// persistent kernels the same addresses are rewritten by other CTAs between two reads of one SM, and
+// L1 is not coherent; the data is streamed once per task, so L1 would not help anyway.
+CANS_HD double2 ld_p2(const double* p) {
+#if defined(__CUDA_ARCH__)
+    return __ldcg(reinterpret_cast<const double2*>(p));
+#else
+    return *reinterpret_cast<const double2*>(p);
+#endif
+}
+
 // Transform kind of one direction (pressure boundary pair), see DESIGN.md "Transforms".
 enum Kind : int { KIND_PP = 0, KIND_NN = 1, KIND_DD = 2 };
 

@@ -73,13 +73,16 @@ CANS_HD void pre_inverse(double A0, double A1, double B0, double B1, cplx wq, in
 // =================================================================================================
 // x pass.  One CTA handles NF row pairs; shared memory: NF lines of P::NPAD cplx.
 // =================================================================================================
-template <class P, int NF, int NT>
+template <class P, int NF, int NT, int TWOFF = NF * P::NPAD>
 struct XPass {
     static constexpr int N = P::N;
     static constexpr int H = N / 2;
+    static constexpr int WORK_CPLX = NF * P::NPAD;             // line buffers
     static constexpr int SMEM_CPLX = NF * P::NPAD + P::TW_TOTAL;
 
-    static CANS_HD cplx* tw_smem(cplx* sm) { return sm + NF * P::NPAD; }
+    // TWOFF: where this direction's twiddles live relative to the work buffer (the fused kernels
+    // of fused_pass.cuh keep one work buffer and both directions' tables behind it)
+    static CANS_HD cplx* tw_smem(cplx* sm) { return sm + TWOFF; }
 
     static CANS_HD void load_twiddles(const XYArgs& a, cplx* sm, int tid) {
         cplx* t = tw_smem(sm);
@@ -106,8 +109,8 @@ struct XPass {
             const size_t ro = row_offset(a, pr, j, k);
             double2 va, vb;
             if (!DIV) {
-                va = *reinterpret_cast<const double2*>(a.p + ro + 2 * e2);
-                vb = *reinterpret_cast<const double2*>(a.p + ro + a.nx + 2 * e2);
+                va = ld_p2(a.p + ro + 2 * e2);
+                vb = ld_p2(a.p + ro + a.nx + 2 * e2);
             } else {
                 const size_t plane = (size_t)a.nx * a.ny;
                 const int i0 = 2 * e2;
@@ -210,8 +213,8 @@ struct XPass {
             int j, k;
             const size_t ro = row_offset(a, pr, j, k);
             cplx* line = sm + f * P::NPAD;
-            const double2 ia = *reinterpret_cast<const double2*>(a.p + ro + 2 * s);
-            const double2 ib = *reinterpret_cast<const double2*>(a.p + ro + a.nx + 2 * s);
+            const double2 ia = ld_p2(a.p + ro + 2 * s);
+            const double2 ib = ld_p2(a.p + ro + a.nx + 2 * s);
             if (s == 0) {
                 const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
                 line[P::pad(P::loc_of_freq(0))] = make_double2(ia.x, ib.x);
@@ -253,13 +256,14 @@ struct XPass {
 // y pass.  One CTA handles TXC complex columns (2*TXC real columns) of one k-plane, all ny rows;
 // shared memory: element (e, f) at e*TXC + f, so every access of 8 consecutive threads is contiguous.
 // =================================================================================================
-template <class P, int TXC, int NT>
+template <class P, int TXC, int NT, int TWOFF = P::N * TXC>
 struct YPass {
     static constexpr int N = P::N;
     static constexpr int H = N / 2;
+    static constexpr int WORK_CPLX = N * TXC;
     static constexpr int SMEM_CPLX = N * TXC + P::TW_TOTAL;
 
-    static CANS_HD cplx* tw_smem(cplx* sm) { return sm + N * TXC; }
+    static CANS_HD cplx* tw_smem(cplx* sm) { return sm + TWOFF; }
     static CANS_HD void load_twiddles(const XYArgs& a, cplx* sm, int tid) {
         cplx* t = tw_smem(sm);
         for (int i = tid; i < P::TW_TOTAL; i += NT) t[i] = a.tw[i];
@@ -274,7 +278,7 @@ struct YPass {
         for (int idx = tid; idx < N * TXC; idx += NT) {
             const int j = idx / TXC;
             const int f = idx - j * TXC;
-            cplx z = *reinterpret_cast<const double2*>(base + (size_t)j * a.nx + 2 * f);
+            cplx z = ld_p2(base + (size_t)j * a.nx + 2 * f);
             const int e = elem_of_index<N>(j, a.kind);
             if (a.kind == KIND_DD && (j & 1)) z = cneg(z);
             sm[e * TXC + f] = z;
@@ -329,8 +333,8 @@ struct YPass {
         for (int idx = tid; idx < H * TXC; idx += NT) {
             const int s = idx / TXC;
             const int f = idx - s * TXC;
-            const double2 r0 = *reinterpret_cast<const double2*>(base + (size_t)(2 * s) * a.nx + 2 * f);
-            const double2 r1 = *reinterpret_cast<const double2*>(base + (size_t)(2 * s + 1) * a.nx + 2 * f);
+            const double2 r0 = ld_p2(base + (size_t)(2 * s) * a.nx + 2 * f);
+            const double2 r1 = ld_p2(base + (size_t)(2 * s + 1) * a.nx + 2 * f);
             if (s == 0) {
                 const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
                 sm[P::loc_of_freq(0) * TXC + f] = make_double2(r0.x, r0.y);
