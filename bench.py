@@ -222,6 +222,8 @@ def run_ours(args):
     nx, ny, nz = w.n
     cells = w.cells
     plan = binding.plan_for(w)
+    if args.no_fuse:
+        plan.set_fusion(False)
     u0, v0, w0 = (w.fields[c] for c in "uvw")
     u, v, ww = torch.empty_like(u0), torch.empty_like(u0), torch.empty_like(u0)
     p = torch.empty_like(u0)
@@ -366,6 +368,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
+    ap.add_argument("--no-fuse", action="store_true", help="time the unfused launch sequence (one kernel per step)")
     ap.add_argument("--no-extra", action="store_true", help="skip the Poisson-only timings of C2..C5")
     args = ap.parse_args()
     if args.impl == "reference":

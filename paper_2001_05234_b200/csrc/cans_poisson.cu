@@ -58,46 +58,6 @@ bool fused_dispatch(int nx, int ny, int what, const FusedArgs* a, int num_sms, i
     }
 }
 
-// Ticket order of the fused passes (fused_pass.cuh).  Counter indices: pass A x-done [0, nz);
-// pass C y-done [nz+4, 2nz+4), x-done [2(nz+4), 3nz+8).  LAG planes separate a producer from its consumer in
-// the ticket order so that the consumer rarely has to spin.
-static std::vector<Segment> build_segments(int nz, int nxt, int nyt, int ngt, bool inv, bool grad, unsigned* total) {
-    std::vector<Segment> v;
-    unsigned first = 0;
-    auto add = [&](int type, int k, unsigned count, int dep0, unsigned t0, int dep1, unsigned t1, int signal) {
-        Segment s;
-        s.first = first; s.count = count; s.type = type; s.k = k;
-        s.dep0 = dep0; s.target0 = t0; s.dep1 = dep1; s.target1 = t1; s.signal = signal; s.pad = 0;
-        v.push_back(s);
-        first += count;
-    };
-    const int stride = nz + 4;
-    if (!inv) {
-        const int LAG = 2;
-        for (int k = 0; k < LAG && k < nz; ++k) add(TASK_X, k, nxt, -1, 0, -1, 0, k);
-        for (int k = 0; k < nz; ++k) {
-            if (k + LAG < nz) add(TASK_X, k + LAG, nxt, -1, 0, -1, 0, k + LAG);
-            add(TASK_Y, k, nyt, k, nxt, -1, 0, -1);
-        }
-    } else {
-        const int LAG = 1;
-        for (int r = 0; r < nz + 2 * LAG + 1; ++r) {
-            if (r < nz) add(TASK_Y, r, nyt, -1, 0, -1, 0, stride + r);
-            const int kx = r - LAG;
-            if (kx >= 0 && kx < nz) add(TASK_X, kx, nxt, stride + kx, nyt, -1, 0, 2 * stride + kx);
-            const int kg = r - 2 * LAG - 1;
-            if (grad && kg >= 0 && kg < nz)
-                add(TASK_G, kg, ngt, 2 * stride + kg, nxt, (kg + 1 < nz) ? 2 * stride + kg + 1 : -1, nxt, -1);
-        }
-    }
-    *total = first;
-    Segment s;
-    s.first = first; s.count = 0xffffffffu; s.type = -1; s.k = 0;
-    s.dep0 = s.dep1 = s.signal = -1; s.target0 = s.target1 = 0; s.pad = 0;
-    v.push_back(s);
-    return v;
-}
-
 }  // namespace cans
 
 using namespace cans;
@@ -117,10 +77,9 @@ struct cans_poisson_plan {
     size_t z_smem;
     // fused passes A / C (fused_pass.cuh): persistent grid, ticket tables
     int fused;                // 1: (nx, ny) has fused kernels and fusion is enabled
+    int fused_ok;             // 1: (nx, ny) has fused kernels
     int fused_grid;
     size_t fused_smem;
-    Segment *seg_a, *seg_c, *seg_cg;      // pass A; pass C without / with gradient tasks
-    unsigned tot_a, tot_c, tot_cg;
     unsigned int* sched;      // scheduler state (tickets, per-plane counters), zeroed at the start of every call
     size_t sched_bytes;
     std::vector<void*> dev_allocs;
@@ -246,8 +205,8 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->nseg = nseg; pl->nzp = nseg * Z_MROWS;
     for (int i = 0; i < 4; ++i) pl->hostbuf[i] = nullptr;
     pl->prof = 0; pl->nrec = 0;
-    pl->seg_a = pl->seg_c = pl->seg_cg = nullptr;
     pl->fused = 0;
+    pl->fused_ok = 0;
     pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
     int dev = 0;
     cudaGetDevice(&dev);
@@ -281,7 +240,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->r00 = (double*)d; }
     }
     if (e == cudaSuccess) {
-        pl->sched_bytes = sizeof(unsigned int) * (size_t)(SCHED_PLANES + 4 * (nz + 4));
+        pl->sched_bytes = sizeof(unsigned int) * (size_t)(SCHED_PLANES + 6 * (nz + 4));
         void* d = nullptr;
         e = cudaMalloc(&d, pl->sched_bytes);
         if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->sched = (unsigned int*)d; e = cudaMemset(d, 0, pl->sched_bytes); }
@@ -296,22 +255,8 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         cudaError_t fe = cudaSuccess;
         if (fused_dispatch(nx, ny, 0, nullptr, pl->num_sms, &pl->fused_grid, &pl->fused_smem, 0, &fe)) e = fe;
         if (e == cudaSuccess) {
-            const int nxt = (ny / 2 + fused_nfx(nx) - 1) / fused_nfx(nx);
-            const int nyt = (nx / 2) / fused_txc(ny);
-            const int ngt = (ny + FUSED_GROWS - 1) / FUSED_GROWS;
-            auto upseg = [&](const std::vector<Segment>& h, Segment** d) {
-                if (e != cudaSuccess) return;
-                void* dv = nullptr;
-                e = cudaMalloc(&dv, h.size() * sizeof(Segment));
-                if (e != cudaSuccess) return;
-                pl->dev_allocs.push_back(dv);
-                e = cudaMemcpy(dv, h.data(), h.size() * sizeof(Segment), cudaMemcpyHostToDevice);
-                *d = (Segment*)dv;
-            };
-            upseg(build_segments(nz, nxt, nyt, ngt, false, false, &pl->tot_a), &pl->seg_a);
-            upseg(build_segments(nz, nxt, nyt, ngt, true, false, &pl->tot_c), &pl->seg_c);
-            upseg(build_segments(nz, nxt, nyt, ngt, true, true, &pl->tot_cg), &pl->seg_cg);
             pl->fused = 1;
+            pl->fused_ok = 1;
         }
     }
     if (e != cudaSuccess) {
@@ -364,20 +309,35 @@ static int launch_fused(cans_poisson_plan* pl, bool inv, double* p, const XYArgs
     f.ax = (divargs && !inv) ? *divargs : make_xyargs(pl, p, true);
     f.ay = make_xyargs(pl, p, false);
     if (grad) f.g = *grad;
-    f.counters = pl->sched + SCHED_PLANES;
-    f.lookahead = (unsigned)pl->fused_grid;
+    const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
+    const unsigned nxt = (unsigned)((ny / 2) / fused_nfx(nx));
+    const unsigned nyt = (unsigned)((nx / 2) / fused_txc(ny));
+    f.cstride = nz + 4;
+    f.drows = FUSED_DROWS;
     f.grows = FUSED_GROWS;
+    const unsigned ndt = (unsigned)((ny + FUSED_DROWS - 1) / FUSED_DROWS);
+    const unsigned ngt = (unsigned)((ny + FUSED_GROWS - 1) / FUSED_GROWS);
+    auto slot = [&](int type, int off, unsigned count) {
+        f.slot_type[f.nslots] = type; f.slot_off[f.nslots] = off; f.slot_count[f.nslots] = count;
+        f.per_round += count;
+        ++f.nslots;
+    };
     const char* name;
+    int maxoff;
     if (!inv) {
-        f.segs = pl->seg_a; f.total = pl->tot_a; f.ticket = pl->sched + SCHED_A_TICKET;
-        f.mode = divargs ? 1 : 0;
+        f.counters = pl->sched + SCHED_PLANES;
+        f.ticket = pl->sched + SCHED_A_TICKET;
+        if (divargs) { slot(TASK_D, 0, ndt); slot(TASK_X, 1, nxt); slot(TASK_Y, 2, nyt); maxoff = 2; }
+        else { slot(TASK_X, 0, nxt); slot(TASK_Y, 1, nyt); maxoff = 1; }
         name = divargs ? "xy_fwd_div" : "xy_fwd";
     } else {
-        f.segs = grad ? pl->seg_cg : pl->seg_c; f.total = grad ? pl->tot_cg : pl->tot_c;
+        f.counters = pl->sched + SCHED_PLANES + 3 * (nz + 4);
         f.ticket = pl->sched + SCHED_C_TICKET;
-        f.mode = grad ? 1 : 0;
+        slot(TASK_Y, 0, nyt); slot(TASK_X, 1, nxt); maxoff = 1;
+        if (grad) { slot(TASK_G, 3, ngt); maxoff = 3; }
         name = grad ? "xy_inv_grad" : "xy_inv";
     }
+    f.total = (unsigned)(nz + maxoff) * f.per_round;
     LaunchScope scope(pl, st, name);
     cudaError_t err = cudaSuccess;
     if (!fused_dispatch(pl->nx, pl->ny, inv ? 2 : 1, &f, pl->num_sms, &pl->fused_grid, &pl->fused_smem, st, &err))
@@ -424,7 +384,7 @@ static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, con
 int cans_plan_set_fusion(cans_poisson_plan* plan, int enable) {
     g_status = CANS_OK;
     if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
-    plan->fused = (enable && plan->seg_a != nullptr) ? 1 : 0;
+    plan->fused = (enable && plan->fused_ok) ? 1 : 0;
     return plan->fused;
 }
 

@@ -17,10 +17,10 @@ template <int NX>
 bool fused_dispatch_nx(int ny, int what, const FusedArgs* a, int num_sms, int* grid, size_t* smem,
                        cudaStream_t st, cudaError_t* err) {
     typedef typename PlanOf<NX>::type PX;
-    constexpr int NFX = NX <= 384 ? 8 : 4;      // == fused_nfx(NX)
+    constexpr int NFX = fused_nfx(NX);
     switch (ny) {
 #define CANS_FY(NY) \
-        case NY: *err = fused_run<PX, typename PlanOf<NY>::type, NFX, (NY <= 512 ? 8 : 4), FUSED_NT>( \
+        case NY: *err = fused_run<PX, typename PlanOf<NY>::type, NFX, fused_txc(NY), FUSED_NT>( \
                             what, a, num_sms, grid, smem, st); return true;
         CANS_FY(256) CANS_FY(384) CANS_FY(512) CANS_FY(768) CANS_FY(1024)
 #undef CANS_FY

@@ -18,8 +18,17 @@ struct GradArgs {
     double gx_sgn, gy_sgn, gz_sgn;
 };
 
-// one pair of x-adjacent cells (t = pair index, x fastest)
-CANS_HD void grad_correct_pair(const GradArgs& a, size_t t) {
+// inputs of one pair of x-adjacent cells (t = pair index, x fastest), fetched before any of them is
+// used so that a caller can keep several pairs' loads in flight
+struct GradIn {
+    double2 ph, phy, phz, uu, vv, ww;
+    double phx;
+    size_t o;
+    int k;
+};
+
+CANS_HD GradIn grad_load(const GradArgs& a, size_t t) {
+    GradIn in;
     const size_t plane = (size_t)a.nx * a.ny;
     const int hx = a.nx / 2;
     const int i = 2 * (int)(t % hx);
@@ -27,35 +36,46 @@ CANS_HD void grad_correct_pair(const GradArgs& a, size_t t) {
     const int j = (int)(row % a.ny);
     const int k = (int)(row / a.ny);
     const size_t o = (size_t)k * plane + (size_t)j * a.nx + i;
-    const double2 ph = *reinterpret_cast<const double2*>(a.phi + o);
+    in.o = o;
+    in.k = k;
+    in.ph = *reinterpret_cast<const double2*>(a.phi + o);
     // x neighbour of the second cell
-    double phx = (i + 2 < a.nx) ? a.phi[o + 2] : a.gx_sgn * a.phi[o - i + a.gx_idx];
+    in.phx = (i + 2 < a.nx) ? a.phi[o + 2] : a.gx_sgn * a.phi[o - i + a.gx_idx];
     // y neighbours
-    double2 phy;
-    if (j + 1 < a.ny) phy = *reinterpret_cast<const double2*>(a.phi + o + a.nx);
+    if (j + 1 < a.ny) in.phy = *reinterpret_cast<const double2*>(a.phi + o + a.nx);
     else {
-        phy = *reinterpret_cast<const double2*>(a.phi + (size_t)k * plane + (size_t)a.gy_idx * a.nx + i);
-        phy.x *= a.gy_sgn; phy.y *= a.gy_sgn;
+        in.phy = *reinterpret_cast<const double2*>(a.phi + (size_t)k * plane + (size_t)a.gy_idx * a.nx + i);
+        in.phy.x *= a.gy_sgn; in.phy.y *= a.gy_sgn;
     }
-    double2 phz;
-    if (k + 1 < a.nz) phz = *reinterpret_cast<const double2*>(a.phi + o + plane);
+    if (k + 1 < a.nz) in.phz = *reinterpret_cast<const double2*>(a.phi + o + plane);
     else {
-        phz = *reinterpret_cast<const double2*>(a.phi + (size_t)a.gz_idx * plane + (size_t)j * a.nx + i);
-        phz.x *= a.gz_sgn; phz.y *= a.gz_sgn;
+        in.phz = *reinterpret_cast<const double2*>(a.phi + (size_t)a.gz_idx * plane + (size_t)j * a.nx + i);
+        in.phz.x *= a.gz_sgn; in.phz.y *= a.gz_sgn;
     }
-    double2 uu = *reinterpret_cast<double2*>(a.u + o);
-    double2 vv = *reinterpret_cast<double2*>(a.v + o);
-    double2 ww = *reinterpret_cast<double2*>(a.w + o);
+    in.uu = *reinterpret_cast<const double2*>(a.u + o);
+    in.vv = *reinterpret_cast<const double2*>(a.v + o);
+    in.ww = *reinterpret_cast<const double2*>(a.w + o);
+    return in;
+}
+
+CANS_HD void grad_apply(const GradArgs& a, const GradIn& in) {
+    double2 uu = in.uu, vv = in.vv, ww = in.ww;
+    const double2 ph = in.ph;
     uu.x -= a.dt_rdx * (ph.y - ph.x);
-    uu.y -= a.dt_rdx * (phx - ph.y);
-    vv.x -= a.dt_rdy * (phy.x - ph.x);
-    vv.y -= a.dt_rdy * (phy.y - ph.y);
-    const double dz = a.dt * a.rdzc[k];
-    ww.x -= dz * (phz.x - ph.x);
-    ww.y -= dz * (phz.y - ph.y);
-    *reinterpret_cast<double2*>(a.u + o) = uu;
-    *reinterpret_cast<double2*>(a.v + o) = vv;
-    *reinterpret_cast<double2*>(a.w + o) = ww;
+    uu.y -= a.dt_rdx * (in.phx - ph.y);
+    vv.x -= a.dt_rdy * (in.phy.x - ph.x);
+    vv.y -= a.dt_rdy * (in.phy.y - ph.y);
+    const double dz = a.dt * a.rdzc[in.k];
+    ww.x -= dz * (in.phz.x - ph.x);
+    ww.y -= dz * (in.phz.y - ph.y);
+    *reinterpret_cast<double2*>(a.u + in.o) = uu;
+    *reinterpret_cast<double2*>(a.v + in.o) = vv;
+    *reinterpret_cast<double2*>(a.w + in.o) = ww;
+}
+
+CANS_HD void grad_correct_pair(const GradArgs& a, size_t t) {
+    const GradIn in = grad_load(a, t);
+    grad_apply(a, in);
 }
 
 }  // namespace cans

@@ -12,7 +12,7 @@ enum XYOp : int { OP_X_FWD = 0, OP_X_FWD_DIV = 1, OP_X_INV = 2, OP_Y_FWD = 3, OP
 extern __shared__ __align__(16) unsigned char cans_dyn_smem[];
 
 template <class P, int NF, int NT, int MODE>   // MODE: 0 fwd, 1 fwd+div, 2 inv
-__global__ void __launch_bounds__(NT) x_pass_kernel(const XYArgs a, long npairs) {
+__global__ void __launch_bounds__(NT, 2) x_pass_kernel(const XYArgs a, long npairs) {
     typedef XPass<P, NF, NT> X;
     cplx* sm = reinterpret_cast<cplx*>(cans_dyn_smem);
     const int tid = threadIdx.x;
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(NT) x_pass_kernel(const XYArgs a, long npairs)
 }
 
 template <class P, int TXC, int NT, bool INV>
-__global__ void __launch_bounds__(NT) y_pass_kernel(const XYArgs a) {
+__global__ void __launch_bounds__(NT, 2) y_pass_kernel(const XYArgs a) {
     typedef YPass<P, TXC, NT> Y;
     cplx* sm = reinterpret_cast<cplx*>(cans_dyn_smem);
     const int tid = threadIdx.x;

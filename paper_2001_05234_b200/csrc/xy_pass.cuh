@@ -70,6 +70,12 @@ CANS_HD void pre_inverse(double A0, double A1, double B0, double B1, cplx wq, in
 
 #define CANS_SQRT_HALF 0.70710678118654752440
 
+// eq. 2b at one cell from the three face differences; one definition so that every kernel
+// that evaluates the divergence rounds identically
+CANS_HD double div_value(double du, double dv, double dw, double rdx, double rdy, double rz, double rdt) {
+    return (du * rdx + dv * rdy + dw * rz) * rdt;
+}
+
 // =================================================================================================
 // x pass.  One CTA handles NF row pairs; shared memory: NF lines of P::NPAD cplx.
 // =================================================================================================
@@ -98,61 +104,98 @@ struct XPass {
     }
 
     // ---- forward load (optionally computing the divergence on the fly) ----
+    // Loads are issued in batches of UB iterations before the first use, so that every thread keeps
+    // 2*UB (22*UB/11 with the divergence) independent 16-byte loads in flight: the load phase is then
+    // bound by bandwidth rather than by one memory latency per iteration.
+    static constexpr int ITERS = (NF * H + NT - 1) / NT;
+
+    template <bool DIV>
+    static CANS_HD void fetch_forward(const XYArgs& a, size_t ro, int j, int k, int e2, double2& va, double2& vb) {
+        if (!DIV) {
+            va = ld_p2(a.p + ro + 2 * e2);
+            vb = ld_p2(a.p + ro + a.nx + 2 * e2);
+        } else {
+            const size_t plane = (size_t)a.nx * a.ny;
+            const int i0 = 2 * e2;
+            // u: x differences on rows a and b
+            const double2 ua = *reinterpret_cast<const double2*>(a.u + ro + i0);
+            const double2 ub = *reinterpret_cast<const double2*>(a.u + ro + a.nx + i0);
+            double ula, ulb;
+            if (i0 > 0) { ula = a.u[ro + i0 - 1]; ulb = a.u[ro + a.nx + i0 - 1]; }
+            else if (a.wrap_x) { ula = a.u[ro + a.nx - 1]; ulb = a.u[ro + 2 * (size_t)a.nx - 1]; }
+            else { ula = 0.0; ulb = 0.0; }
+            // v: rows j-1, j, j+1
+            const double2 v1 = *reinterpret_cast<const double2*>(a.v + ro + i0);
+            const double2 v2 = *reinterpret_cast<const double2*>(a.v + ro + a.nx + i0);
+            double2 v0;
+            if (j > 0) v0 = *reinterpret_cast<const double2*>(a.v + ro - a.nx + i0);
+            else if (a.wrap_y) v0 = *reinterpret_cast<const double2*>(a.v + ro + (size_t)(a.ny - 1) * a.nx + i0);
+            else v0 = make_double2(0.0, 0.0);
+            // w: planes k-1, k
+            const double2 wa = *reinterpret_cast<const double2*>(a.w + ro + i0);
+            const double2 wb = *reinterpret_cast<const double2*>(a.w + ro + a.nx + i0);
+            double2 wla, wlb;
+            if (k > 0) {
+                wla = *reinterpret_cast<const double2*>(a.w + ro - plane + i0);
+                wlb = *reinterpret_cast<const double2*>(a.w + ro - plane + a.nx + i0);
+            } else if (a.wrap_z) {
+                wla = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + i0);
+                wlb = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + a.nx + i0);
+            } else { wla = make_double2(0.0, 0.0); wlb = wla; }
+            const double rz = a.rdzf[k];
+            va.x = div_value(ua.x - ula, v1.x - v0.x, wa.x - wla.x, a.rdx, a.rdy, rz, a.rdt);
+            va.y = div_value(ua.y - ua.x, v1.y - v0.y, wa.y - wla.y, a.rdx, a.rdy, rz, a.rdt);
+            vb.x = div_value(ub.x - ulb, v2.x - v1.x, wb.x - wlb.x, a.rdx, a.rdy, rz, a.rdt);
+            vb.y = div_value(ub.y - ub.x, v2.y - v1.y, wb.y - wlb.y, a.rdx, a.rdy, rz, a.rdt);
+        }
+    }
+
     template <bool DIV>
     static CANS_HD void load_forward(const XYArgs& a, cplx* sm, long pair0, long npairs, int tid) {
+        constexpr int UB = DIV ? (ITERS < 2 ? ITERS : 2) : (ITERS < 8 ? ITERS : 8);
+        for (int it0 = 0; it0 < ITERS; it0 += UB) {
+            double2 va[UB], vb[UB];
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int f = idx / H;
+                const int e2 = idx - f * H;
+                const long pr = pair0 + f;
+                if (idx < NF * H && pr < npairs) {
+                    int j, k;
+                    const size_t ro = row_offset(a, pr, j, k);
+                    fetch_forward<DIV>(a, ro, j, k, e2, va[u], vb[u]);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int f = idx / H;
+                const int e2 = idx - f * H;
+                if (idx < NF * H && pair0 + f < npairs) put_forward(sm + f * P::NPAD, e2, va[u], vb[u], a.kind);
+            }
+        }
+    }
+
+    // samples (2*e2, 2*e2+1) of rows a and b -> FFT input elements of the packed line z = a + i b
+    static CANS_HD void put_forward(cplx* line, int e2, double2 va, double2 vb, int kind) {
+        cplx z0 = make_double2(va.x, vb.x);      // index 2*e2
+        cplx z1 = make_double2(va.y, vb.y);      // index 2*e2+1
+        int d0, d1;
+        if (kind == KIND_PP) { d0 = 2 * e2; d1 = 2 * e2 + 1; }
+        else { d0 = e2; d1 = N - 1 - e2; if (kind == KIND_DD) z1 = cneg(z1); }
+        line[P::pad(d0)] = z0;
+        line[P::pad(d1)] = z1;
+    }
+
+    // forward "load" from a staged copy of the 2*NF rows in shared memory (row stride N doubles)
+    static CANS_HD void unpack_forward(const XYArgs& a, cplx* sm, const double* S, int tid) {
         for (int idx = tid; idx < NF * H; idx += NT) {
             const int f = idx / H;
             const int e2 = idx - f * H;
-            const long pr = pair0 + f;
-            if (pr >= npairs) continue;
-            int j, k;
-            const size_t ro = row_offset(a, pr, j, k);
-            double2 va, vb;
-            if (!DIV) {
-                va = ld_p2(a.p + ro + 2 * e2);
-                vb = ld_p2(a.p + ro + a.nx + 2 * e2);
-            } else {
-                const size_t plane = (size_t)a.nx * a.ny;
-                const int i0 = 2 * e2;
-                // u: x differences on rows a and b
-                const double2 ua = *reinterpret_cast<const double2*>(a.u + ro + i0);
-                const double2 ub = *reinterpret_cast<const double2*>(a.u + ro + a.nx + i0);
-                double ula, ulb;
-                if (i0 > 0) { ula = a.u[ro + i0 - 1]; ulb = a.u[ro + a.nx + i0 - 1]; }
-                else if (a.wrap_x) { ula = a.u[ro + a.nx - 1]; ulb = a.u[ro + 2 * (size_t)a.nx - 1]; }
-                else { ula = 0.0; ulb = 0.0; }
-                // v: rows j-1, j, j+1
-                const double2 v1 = *reinterpret_cast<const double2*>(a.v + ro + i0);
-                const double2 v2 = *reinterpret_cast<const double2*>(a.v + ro + a.nx + i0);
-                double2 v0;
-                if (j > 0) v0 = *reinterpret_cast<const double2*>(a.v + ro - a.nx + i0);
-                else if (a.wrap_y) v0 = *reinterpret_cast<const double2*>(a.v + ro + (size_t)(a.ny - 1) * a.nx + i0);
-                else v0 = make_double2(0.0, 0.0);
-                // w: planes k-1, k
-                const double2 wa = *reinterpret_cast<const double2*>(a.w + ro + i0);
-                const double2 wb = *reinterpret_cast<const double2*>(a.w + ro + a.nx + i0);
-                double2 wla, wlb;
-                if (k > 0) {
-                    wla = *reinterpret_cast<const double2*>(a.w + ro - plane + i0);
-                    wlb = *reinterpret_cast<const double2*>(a.w + ro - plane + a.nx + i0);
-                } else if (a.wrap_z) {
-                    wla = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + i0);
-                    wlb = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + a.nx + i0);
-                } else { wla = make_double2(0.0, 0.0); wlb = wla; }
-                const double rz = a.rdzf[k];
-                va.x = ((ua.x - ula) * a.rdx + (v1.x - v0.x) * a.rdy + (wa.x - wla.x) * rz) * a.rdt;
-                va.y = ((ua.y - ua.x) * a.rdx + (v1.y - v0.y) * a.rdy + (wa.y - wla.y) * rz) * a.rdt;
-                vb.x = ((ub.x - ulb) * a.rdx + (v2.x - v1.x) * a.rdy + (wb.x - wlb.x) * rz) * a.rdt;
-                vb.y = ((ub.y - ub.x) * a.rdx + (v2.y - v1.y) * a.rdy + (wb.y - wlb.y) * rz) * a.rdt;
-            }
-            cplx z0 = make_double2(va.x, vb.x);      // index 2*e2
-            cplx z1 = make_double2(va.y, vb.y);      // index 2*e2+1
-            int d0, d1;
-            if (a.kind == KIND_PP) { d0 = 2 * e2; d1 = 2 * e2 + 1; }
-            else { d0 = e2; d1 = N - 1 - e2; if (a.kind == KIND_DD) z1 = cneg(z1); }
-            cplx* line = sm + f * P::NPAD;
-            line[P::pad(d0)] = z0;
-            line[P::pad(d1)] = z1;
+            const double* ra = S + (size_t)(2 * f) * N + 2 * e2;
+            put_forward(sm + f * P::NPAD, e2, *reinterpret_cast<const double2*>(ra),
+                        *reinterpret_cast<const double2*>(ra + N), a.kind);
         }
     }
 
@@ -203,30 +246,57 @@ struct XPass {
         }
     }
 
-    // ---- inverse load: slots -> Z at digit-reversed locations ----
+    // ---- inverse load: slots -> Z at digit-reversed locations (batched like load_forward) ----
     static CANS_HD void load_inverse(const XYArgs& a, cplx* sm, long pair0, long npairs, int tid) {
+        constexpr int UB = ITERS < 8 ? ITERS : 8;
+        for (int it0 = 0; it0 < ITERS; it0 += UB) {
+            double2 ia[UB], ib[UB];
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int f = idx / H;
+                const int s = idx - f * H;
+                const long pr = pair0 + f;
+                if (idx < NF * H && pr < npairs) {
+                    int j, k;
+                    const size_t ro = row_offset(a, pr, j, k);
+                    ia[u] = ld_p2(a.p + ro + 2 * s);
+                    ib[u] = ld_p2(a.p + ro + a.nx + 2 * s);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int f = idx / H;
+                const int s = idx - f * H;
+                if (idx < NF * H && pair0 + f < npairs) put_inverse(a, sm + f * P::NPAD, s, ia[u], ib[u]);
+            }
+        }
+    }
+
+    // slot s of rows a and b -> Z at the digit-reversed locations
+    static CANS_HD void put_inverse(const XYArgs& a, cplx* line, int s, double2 ia, double2 ib) {
+        if (s == 0) {
+            const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
+            line[P::pad(P::loc_of_freq(0))] = make_double2(ia.x, ib.x);
+            line[P::pad(P::loc_of_freq(H))] = make_double2(c * ia.y, c * ib.y);
+        } else {
+            cplx wq = make_double2(1.0, 0.0);
+            if (a.kind != KIND_PP) wq = a.wpost[s];
+            cplx Zq, Zm;
+            pre_inverse(ia.x, ia.y, ib.x, ib.y, wq, a.kind, Zq, Zm);
+            line[P::pad(P::loc_of_freq(s))] = Zq;
+            line[P::pad(P::loc_of_freq(N - s))] = Zm;
+        }
+    }
+
+    static CANS_HD void unpack_inverse(const XYArgs& a, cplx* sm, const double* S, int tid) {
         for (int idx = tid; idx < NF * H; idx += NT) {
             const int f = idx / H;
             const int s = idx - f * H;
-            const long pr = pair0 + f;
-            if (pr >= npairs) continue;
-            int j, k;
-            const size_t ro = row_offset(a, pr, j, k);
-            cplx* line = sm + f * P::NPAD;
-            const double2 ia = ld_p2(a.p + ro + 2 * s);
-            const double2 ib = ld_p2(a.p + ro + a.nx + 2 * s);
-            if (s == 0) {
-                const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
-                line[P::pad(P::loc_of_freq(0))] = make_double2(ia.x, ib.x);
-                line[P::pad(P::loc_of_freq(H))] = make_double2(c * ia.y, c * ib.y);
-            } else {
-                cplx wq = make_double2(1.0, 0.0);
-                if (a.kind != KIND_PP) wq = a.wpost[s];
-                cplx Zq, Zm;
-                pre_inverse(ia.x, ia.y, ib.x, ib.y, wq, a.kind, Zq, Zm);
-                line[P::pad(P::loc_of_freq(s))] = Zq;
-                line[P::pad(P::loc_of_freq(N - s))] = Zm;
-            }
+            const double* ra = S + (size_t)(2 * f) * N + 2 * s;
+            put_inverse(a, sm + f * P::NPAD, s, *reinterpret_cast<const double2*>(ra),
+                        *reinterpret_cast<const double2*>(ra + N));
         }
     }
 
@@ -275,13 +345,39 @@ struct YPass {
 
     static CANS_HD void load_forward(const XYArgs& a, cplx* sm, int ctile, int k, int tid) {
         const double* base = tile_base(a, ctile, k);
+        constexpr int ITERS = (N * TXC + NT - 1) / NT;
+        constexpr int UB = ITERS < 12 ? ITERS : 12;        // independent 16-byte loads in flight per thread
+        for (int it0 = 0; it0 < ITERS; it0 += UB) {
+            cplx z[UB];
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int j = idx / TXC;
+                const int f = idx - j * TXC;
+                if (idx < N * TXC) z[u] = ld_p2(base + (size_t)j * a.nx + 2 * f);
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int j = idx / TXC;
+                const int f = idx - j * TXC;
+                if (idx < N * TXC) put_forward(a, sm, j, f, z[u]);
+            }
+        }
+    }
+
+    static CANS_HD void put_forward(const XYArgs& a, cplx* sm, int j, int f, cplx z) {
+        const int e = elem_of_index<N>(j, a.kind);
+        if (a.kind == KIND_DD && (j & 1)) z = cneg(z);
+        sm[e * TXC + f] = z;
+    }
+
+    // forward "load" from a staged dense copy of the tile in shared memory (row stride 2*TXC doubles)
+    static CANS_HD void unpack_forward(const XYArgs& a, cplx* sm, const double* S, int tid) {
         for (int idx = tid; idx < N * TXC; idx += NT) {
             const int j = idx / TXC;
             const int f = idx - j * TXC;
-            cplx z = ld_p2(base + (size_t)j * a.nx + 2 * f);
-            const int e = elem_of_index<N>(j, a.kind);
-            if (a.kind == KIND_DD && (j & 1)) z = cneg(z);
-            sm[e * TXC + f] = z;
+            put_forward(a, sm, j, f, *reinterpret_cast<const double2*>(S + 2 * (size_t)idx));
         }
     }
 
@@ -330,23 +426,51 @@ struct YPass {
 
     static CANS_HD void load_inverse(const XYArgs& a, cplx* sm, int ctile, int k, int tid) {
         const double* base = tile_base(a, ctile, k);
+        constexpr int ITERS = (H * TXC + NT - 1) / NT;
+        constexpr int UB = ITERS < 6 ? ITERS : 6;
+        for (int it0 = 0; it0 < ITERS; it0 += UB) {
+            double2 r0[UB], r1[UB];
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int s = idx / TXC;
+                const int f = idx - s * TXC;
+                if (idx < H * TXC) {
+                    r0[u] = ld_p2(base + (size_t)(2 * s) * a.nx + 2 * f);
+                    r1[u] = ld_p2(base + (size_t)(2 * s + 1) * a.nx + 2 * f);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UB; ++u) {
+                const int idx = tid + (it0 + u) * NT;
+                const int s = idx / TXC;
+                const int f = idx - s * TXC;
+                if (idx < H * TXC) put_inverse(a, sm, s, f, r0[u], r1[u]);
+            }
+        }
+    }
+
+    static CANS_HD void put_inverse(const XYArgs& a, cplx* sm, int s, int f, double2 r0, double2 r1) {
+        if (s == 0) {
+            const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
+            sm[P::loc_of_freq(0) * TXC + f] = make_double2(r0.x, r0.y);
+            sm[P::loc_of_freq(H) * TXC + f] = make_double2(c * r1.x, c * r1.y);
+        } else {
+            cplx wq = make_double2(1.0, 0.0);
+            if (a.kind != KIND_PP) wq = a.wpost[s];
+            cplx Zq, Zm;
+            pre_inverse(r0.x, r1.x, r0.y, r1.y, wq, a.kind, Zq, Zm);
+            sm[P::loc_of_freq(s) * TXC + f] = Zq;
+            sm[P::loc_of_freq(N - s) * TXC + f] = Zm;
+        }
+    }
+
+    static CANS_HD void unpack_inverse(const XYArgs& a, cplx* sm, const double* S, int tid) {
         for (int idx = tid; idx < H * TXC; idx += NT) {
             const int s = idx / TXC;
             const int f = idx - s * TXC;
-            const double2 r0 = ld_p2(base + (size_t)(2 * s) * a.nx + 2 * f);
-            const double2 r1 = ld_p2(base + (size_t)(2 * s + 1) * a.nx + 2 * f);
-            if (s == 0) {
-                const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
-                sm[P::loc_of_freq(0) * TXC + f] = make_double2(r0.x, r0.y);
-                sm[P::loc_of_freq(H) * TXC + f] = make_double2(c * r1.x, c * r1.y);
-            } else {
-                cplx wq = make_double2(1.0, 0.0);
-                if (a.kind != KIND_PP) wq = a.wpost[s];
-                cplx Zq, Zm;
-                pre_inverse(r0.x, r1.x, r0.y, r1.y, wq, a.kind, Zq, Zm);
-                sm[P::loc_of_freq(s) * TXC + f] = Zq;
-                sm[P::loc_of_freq(N - s) * TXC + f] = Zm;
-            }
+            put_inverse(a, sm, s, f, *reinterpret_cast<const double2*>(S + ((size_t)(2 * s) * TXC + f) * 2),
+                        *reinterpret_cast<const double2*>(S + ((size_t)(2 * s + 1) * TXC + f) * 2));
         }
     }
 
