@@ -47,6 +47,7 @@ struct ZArgs {
     const double* dzf;        // [nz]
     double inv_lz;            // 1 / sum(dzf)
     unsigned int* ticket;     // tile ticket counter (zeroed before the launch)
+    int nbox, box_rows;       // TMA tiling of a column tile: nbox boxes of box_rows rows (set by z_solve_launch)
 };
 
 // one pivot step; shared by the plan-time table kernel and the solve so the values are identical
@@ -92,17 +93,25 @@ struct ZPass {
     }
 
 #if defined(__CUDACC__)
-    // asynchronous copy of tile `tile` (rows 0..nz-1, TC columns) into buf[k*TC + c]
+    // asynchronous copy of tile `tile` (rows 0..nz-1, TC columns) into buf[k*TC + c].
+    // nthreads is a multiple of the CH = TC/2 chunks of a row, so a thread keeps its chunk column and
+    // walks down the rows with a constant stride: no per-copy index arithmetic.
     static CANS_D void prefetch_tile(const ZArgs& a, double* buf, long tile, int tid, int nthreads) {
         constexpr int CH = TC / 2;                      // 16-byte chunks per row
         const long col0 = tile * TC;
         const size_t plane = (size_t)a.ncols;
-        const int nchunks = a.nz * CH;
         if (col0 + TC <= a.ncols) {
-            for (int id = tid; id < nchunks; id += nthreads) {
-                const int k = id / CH;
-                const int q = id - k * CH;
-                cp_async16(buf + (size_t)k * TC + 2 * q, a.p + (size_t)k * plane + col0 + 2 * q);
+            const int q = tid % CH;
+            const int kstep = nthreads / CH;
+            const double* src = a.p + (size_t)(tid / CH) * plane + col0 + 2 * q;
+            double* dst = buf + (size_t)(tid / CH) * TC + 2 * q;
+            const size_t sstep = (size_t)kstep * plane;
+            const int dstep = kstep * TC;
+#pragma unroll 4
+            for (int k = tid / CH; k < a.nz; k += kstep) {
+                cp_async16(dst, src);
+                src += sstep;
+                dst += dstep;
             }
         } else {                                        // ragged last tile: plain guarded loads
             for (int id = tid; id < a.nz * TC; id += nthreads) {
