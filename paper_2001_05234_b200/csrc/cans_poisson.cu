@@ -255,7 +255,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         cudaError_t fe = cudaSuccess;
         if (fused_dispatch(nx, ny, 0, nullptr, pl->num_sms, &pl->fused_grid, &pl->fused_smem, 0, &fe)) e = fe;
         if (e == cudaSuccess) {
-            pl->fused = 1;
+            pl->fused = 0;        // opt-in (cans_plan_set_fusion): the unfused sequence is currently faster
             pl->fused_ok = 1;
         }
     }
@@ -313,9 +313,7 @@ static int launch_fused(cans_poisson_plan* pl, bool inv, double* p, const XYArgs
     const unsigned nxt = (unsigned)((ny / 2) / fused_nfx(nx));
     const unsigned nyt = (unsigned)((nx / 2) / fused_txc(ny));
     f.cstride = nz + 4;
-    f.drows = FUSED_DROWS;
     f.grows = FUSED_GROWS;
-    const unsigned ndt = (unsigned)((ny + FUSED_DROWS - 1) / FUSED_DROWS);
     const unsigned ngt = (unsigned)((ny + FUSED_GROWS - 1) / FUSED_GROWS);
     auto slot = [&](int type, int off, unsigned count) {
         f.slot_type[f.nslots] = type; f.slot_off[f.nslots] = off; f.slot_count[f.nslots] = count;
@@ -327,14 +325,14 @@ static int launch_fused(cans_poisson_plan* pl, bool inv, double* p, const XYArgs
     if (!inv) {
         f.counters = pl->sched + SCHED_PLANES;
         f.ticket = pl->sched + SCHED_A_TICKET;
-        if (divargs) { slot(TASK_D, 0, ndt); slot(TASK_X, 1, nxt); slot(TASK_Y, 2, nyt); maxoff = 2; }
-        else { slot(TASK_X, 0, nxt); slot(TASK_Y, 1, nyt); maxoff = 1; }
+        slot(TASK_X, 0, nxt); slot(TASK_Y, 2, nyt); maxoff = 2;
+        f.mode = divargs ? 1 : 0;
         name = divargs ? "xy_fwd_div" : "xy_fwd";
     } else {
         f.counters = pl->sched + SCHED_PLANES + 3 * (nz + 4);
         f.ticket = pl->sched + SCHED_C_TICKET;
-        slot(TASK_Y, 0, nyt); slot(TASK_X, 1, nxt); maxoff = 1;
-        if (grad) { slot(TASK_G, 3, ngt); maxoff = 3; }
+        slot(TASK_Y, 0, nyt); slot(TASK_X, 2, nxt); maxoff = 2;
+        if (grad) { slot(TASK_G, 5, ngt); maxoff = 5; }
         name = grad ? "xy_inv_grad" : "xy_inv";
     }
     f.total = (unsigned)(nz + maxoff) * f.per_round;

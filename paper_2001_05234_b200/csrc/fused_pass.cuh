@@ -25,7 +25,7 @@
 
 namespace cans {
 
-enum TaskType : int { TASK_END = -2, TASK_NONE = -1, TASK_X = 0, TASK_Y = 1, TASK_G = 2, TASK_D = 3 };
+enum TaskType : int { TASK_END = -2, TASK_NONE = -1, TASK_X = 0, TASK_Y = 1, TASK_G = 2 };
 
 struct FusedArgs {
     XYArgs ax, ay;              // x / y direction (ax carries u, v, w and the divergence factors)
@@ -39,17 +39,18 @@ struct FusedArgs {
     unsigned* ticket;
     unsigned* counters;         // [slot][cstride]
     int cstride;
-    int drows, grows;           // rows per divergence / gradient task
+    int grows;                  // rows per gradient task
+    int mode;                   // pass A: 1 = divergence fused into the x load
 };
 
 struct Task { int type, k, idx, slot; };
 
 // tiling of the fused kernels per transform length (host and device agree through these)
-constexpr int FUSED_NT = 512;
-constexpr int FUSED_DROWS = 8;
+constexpr int FUSED_NT = 256;
 constexpr int FUSED_GROWS = 8;
-constexpr int fused_nfx(int nx) { return nx >= 768 ? 4 : 8; }       // row pairs per x task
-constexpr int fused_txc(int ny) { return ny <= 768 ? 8 : 4; }       // complex columns per y task
+// the work buffer of a CTA stays <= 67 KB so that two CTAs (with both twiddle tables each) share an SM
+constexpr int fused_nfx(int nx) { return nx >= 512 ? 4 : 8; }        // row pairs per x task
+constexpr int fused_txc(int ny) { return ny >= 768 ? 4 : 8; }        // complex columns per y task
 inline bool fused_supported(int nx, int ny) {
     auto ok = [](int n) { return n == 256 || n == 384 || n == 512 || n == 768 || n == 1024; };
     return ok(nx) && ok(ny);
@@ -114,50 +115,6 @@ CANS_D int task_deps(const FusedArgs& a, const Task& tk, const unsigned* (&c)[2]
 
 // ---- streaming tasks: several items' loads are issued before the first use (memory-level parallelism) ----
 
-// a1: divergence of rows [j0, j1) of plane k -> p (eq. 2b; same arithmetic as XPass::load_forward<true>)
-template <int NT, int U>
-CANS_D void div_rows(const XYArgs& a, int k, int j0, int j1, int tid) {
-    const int hx = a.nx >> 1;
-    const int nitems = (j1 - j0) * hx;
-    const size_t plane = (size_t)a.nx * a.ny;
-    const double rz = a.rdzf[k];
-    const double2 zero2 = make_double2(0.0, 0.0);
-    for (int base = tid; base < nitems; base += U * NT) {
-        double2 ua[U], v1[U], v0[U], wa[U], wl[U];
-        double ul[U];
-        size_t off[U];
-#pragma unroll
-        for (int q = 0; q < U; ++q) {
-            const int it = base + q * NT;
-            if (it < nitems) {
-                const int r = it / hx;
-                const int i0 = 2 * (it - r * hx);
-                const int j = j0 + r;
-                const size_t o = (size_t)k * plane + (size_t)j * a.nx + i0;
-                off[q] = o;
-                ua[q] = *reinterpret_cast<const double2*>(a.u + o);
-                ul[q] = (i0 > 0) ? a.u[o - 1] : (a.wrap_x ? a.u[o + a.nx - 1] : 0.0);
-                v1[q] = *reinterpret_cast<const double2*>(a.v + o);
-                v0[q] = (j > 0) ? *reinterpret_cast<const double2*>(a.v + o - a.nx)
-                                : (a.wrap_y ? *reinterpret_cast<const double2*>(a.v + o + (size_t)(a.ny - 1) * a.nx) : zero2);
-                wa[q] = *reinterpret_cast<const double2*>(a.w + o);
-                wl[q] = (k > 0) ? *reinterpret_cast<const double2*>(a.w + o - plane)
-                                : (a.wrap_z ? *reinterpret_cast<const double2*>(a.w + o + (size_t)(a.nz - 1) * plane) : zero2);
-            }
-        }
-#pragma unroll
-        for (int q = 0; q < U; ++q) {
-            const int it = base + q * NT;
-            if (it < nitems) {
-                double2 f;
-                f.x = div_value(ua[q].x - ul[q], v1[q].x - v0[q].x, wa[q].x - wl[q].x, a.rdx, a.rdy, rz, a.rdt);
-                f.y = div_value(ua[q].y - ua[q].x, v1[q].y - v0[q].y, wa[q].y - wl[q].y, a.rdx, a.rdy, rz, a.rdt);
-                *reinterpret_cast<double2*>(a.p + off[q]) = f;
-            }
-        }
-    }
-}
-
 // a7: gradient correction of rows [j0, j1) of plane k (eq. 2c; grad_pass.cuh)
 template <int NT, int U>
 CANS_D void grad_rows(const GradArgs& g, int k, int j0, int j1, int tid) {
@@ -179,67 +136,55 @@ extern __shared__ __align__(16) unsigned char cans_dyn_smem[];
 
 template <int A, int B> struct MaxOf { static constexpr int value = A > B ? A : B; };
 
-// shared-memory plan of one (PX, PY) pair; sizes in cplx (16 B) units
+// shared-memory plan of one (PX, PY) pair; sizes in cplx (16 B) units: one FFT work buffer shared by the
+// x and y tasks of the CTA, followed by both twiddle tables
 template <class PX, class PY, int NFX, int TXC>
 struct FusedSmem {
-    static constexpr int WORK = MaxOf<NFX * PX::NPAD, PY::N * TXC>::value;     // FFT work buffer
-    static constexpr int TW = PX::TW_TOTAL + PY::TW_TOTAL;                     // both twiddle tables
-    static constexpr int STAGE = MaxOf<NFX * PX::N, PY::N * TXC>::value;       // raw input of the next task
-    static constexpr size_t BYTES = sizeof(cplx) * (size_t)(WORK + TW + STAGE);
+    static constexpr int WORK = MaxOf<NFX * PX::NPAD, PY::N * TXC>::value;
+    static constexpr int TW = PX::TW_TOTAL + PY::TW_TOTAL;
+    static constexpr size_t BYTES = sizeof(cplx) * (size_t)(WORK + TW);
 };
 
-
-// INV = false: pass A (D = divergence rows, X = forward x transform, Y = forward y transform)
+// INV = false: pass A (X = [divergence +] forward x transform, Y = forward y transform)
 // INV = true : pass C (Y = inverse y transform, X = inverse x transform, G = gradient rows)
 template <class PX, class PY, int NFX, int TXC, int NT, bool INV>
-__global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
+__global__ void __launch_bounds__(NT, 2) fused_xy_kernel(const FusedArgs a) {
     typedef FusedSmem<PX, PY, NFX, TXC> L;
     typedef XPass<PX, NFX, NT, L::WORK> X;
     typedef YPass<PY, TXC, NT, L::WORK + PX::TW_TOTAL> Y;
-    cplx* sm = reinterpret_cast<cplx*>(cans_dyn_smem);
-    double* S = reinterpret_cast<double*>(sm + L::WORK + L::TW);
+    cplx* const sm = reinterpret_cast<cplx*>(cans_dyn_smem);
     __shared__ unsigned s_next;
-    __shared__ int s_ready;
     const int tid = threadIdx.x;
     const int nx = a.ax.nx, ny = a.ax.ny;
+    const unsigned rowb = (unsigned)(nx * sizeof(double));
 
-    // copy the raw input of a transform task into the staging buffer (asynchronously), or prefetch the
-    // HBM rows of a streaming task into L2.  Requires the task's dependencies to be satisfied.
-    auto stage_in = [&](const Task& tk) {
-        if (tk.type == TASK_X) {
-            const double* src = a.ax.p + ((size_t)tk.k * ny + (size_t)2 * NFX * tk.idx) * (size_t)nx;
-            for (int c = tid; c < NFX * PX::N; c += NT) fx_cp_async16(S + 2 * c, src + 2 * c);
-        } else if (tk.type == TASK_Y) {
-            const double* src = a.ay.p + (size_t)tk.k * ny * (size_t)nx + 2 * (size_t)tk.idx * TXC;
-            for (int c = tid; c < PY::N * TXC; c += NT) {
-                const int j = c / TXC;
-                const int q = c - j * TXC;
-                fx_cp_async16(S + 2 * c, src + (size_t)j * nx + 2 * q);
+    // L2 prefetch of the HBM-resident input rows of a task (issued one task ahead of its loads)
+    auto prefetch = [&](const Task& tk) {
+        if (!INV && tk.type == TASK_X) {
+            const int nr = 2 * NFX;
+            const size_t ro = ((size_t)tk.k * ny + (size_t)nr * tk.idx) * (size_t)nx;
+            if (a.mode) {
+                if (tid < 3 * nr) {
+                    const int fld = tid / nr, r = tid - fld * nr;
+                    l2_prefetch_bulk((fld == 0 ? a.ax.u : (fld == 1 ? a.ax.v : a.ax.w)) + ro + (size_t)r * nx, rowb);
+                }
+            } else if (tid < nr) {
+                l2_prefetch_bulk(a.ax.p + ro + (size_t)tid * nx, rowb);
             }
-        } else if (tk.type == TASK_D || tk.type == TASK_G) {
-            const int rows = (tk.type == TASK_D) ? a.drows : a.grows;
-            const int j0 = tk.idx * rows;
-            const int nr = min(rows, ny - j0);
+        } else if (INV && tk.type == TASK_Y) {
+            // the y tiles of a plane together read the whole plane: each prefetches its share of rows
+            const int nyt = (int)a.slot_count[tk.slot];
+            const int j0 = (int)(((long)tk.idx * ny) / nyt);
+            const int j1 = (int)(((long)(tk.idx + 1) * ny) / nyt);
+            if (tid < j1 - j0) l2_prefetch_bulk(a.ay.p + ((size_t)tk.k * ny + j0 + tid) * (size_t)nx, rowb);
+        } else if (INV && tk.type == TASK_G) {
+            const int j0 = tk.idx * a.grows;
+            const int nr = min(a.grows, ny - j0);
             if (tid < 3 * nr) {
                 const int fld = tid / nr, r = tid - fld * nr;
-                const double* u = (tk.type == TASK_D) ? a.ax.u : a.g.u;
-                const double* v = (tk.type == TASK_D) ? a.ax.v : a.g.v;
-                const double* w = (tk.type == TASK_D) ? a.ax.w : a.g.w;
-                const double* src = (fld == 0 ? u : (fld == 1 ? v : w)) + ((size_t)tk.k * ny + j0 + r) * (size_t)nx;
-                l2_prefetch_bulk(src, (unsigned)(nx * sizeof(double)));
+                l2_prefetch_bulk((fld == 0 ? a.g.u : (fld == 1 ? a.g.v : a.g.w)) + ((size_t)tk.k * ny + j0 + r) * (size_t)nx, rowb);
             }
         }
-        fx_cp_async_commit();
-    };
-    auto block_wait = [&](const Task& tk) {
-        if (tid == 0) {
-            const unsigned* c[2];
-            unsigned target = 0;
-            const int nd = task_deps(a, tk, c, target);
-            for (int d = 0; d < nd; ++d) wait_counter(c[d], target);
-            if (nd) __threadfence();
-        }
-        __syncthreads();
     };
 
     X::load_twiddles(a.ax, sm, tid);
@@ -251,49 +196,31 @@ __global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
     }
     __syncthreads();
     Task cur = decode_ticket(a, s_next);
-    if (cur.type == TASK_END) return;
-    block_wait(cur);                                     // (also orders the read of s_next before its rewrite)
-    stage_in(cur);
+    __syncthreads();
 
-    while (true) {
-        // thread 0 publishes the next ticket, draws the one after it (latency hidden behind this task)
-        // and probes the next task's dependencies; the answers are used after the unpack
-        unsigned c0 = 0, c1 = 0, target = 0;
-        int nd = 0;
+    while (cur.type != TASK_END) {
+        // thread 0 publishes the next ticket and draws the one after it (its latency hides behind this task),
+        // then waits for the planes this task reads; the barrier publishes both to the CTA
         if (tid == 0) {
-            const unsigned tn = t2;
-            s_next = tn;
+            s_next = t2;
             t2 = atomicAdd(a.ticket, 1u);
-            const Task nt = decode_ticket(a, tn);
             const unsigned* c[2];
-            nd = task_deps(a, nt, c, target);
-            if (nd > 0) c0 = ld_relaxed_u32(c[0]);
-            if (nd > 1) c1 = ld_relaxed_u32(c[1]);
+            unsigned target = 0;
+            const int nd = task_deps(a, cur, c, target);
+            for (int d = 0; d < nd; ++d) wait_counter(c[d], target);
+            if (nd) __threadfence();
         }
-        // the staged input of the current transform task has landed: unpack it into the work buffer
-        if (cur.type == TASK_X || cur.type == TASK_Y) {
-            fx_cp_async_wait_all();
-            __syncthreads();
-            if (cur.type == TASK_X) {
-                if (!INV) X::unpack_forward(a.ax, sm, S, tid); else X::unpack_inverse(a.ax, sm, S, tid);
-            } else {
-                if (!INV) Y::unpack_forward(a.ay, sm, S, tid); else Y::unpack_inverse(a.ay, sm, S, tid);
-            }
-        }
-        if (tid == 0) {
-            const int ready = (nd < 1 || c0 >= target) && (nd < 2 || c1 >= target);
-            if (ready && nd) __threadfence();             // relaxed load + fence = acquire
-            s_ready = ready;
-        }
-        __syncthreads();                                   // staging buffer free, work buffer filled
+        __syncthreads();
         const Task nxt = decode_ticket(a, s_next);
-        const bool ready = s_ready != 0;
-        if (ready) stage_in(nxt);                          // overlaps the whole computation below
+        prefetch(nxt);
 
         if (cur.type == TASK_X) {
             const long pair0 = (long)cur.k * (ny >> 1) + (long)cur.idx * NFX;
             const long lim = (long)(cur.k + 1) * (ny >> 1);
             if (!INV) {
+                if (a.mode) X::template load_forward<true>(a.ax, sm, pair0, lim, tid);
+                else X::template load_forward<false>(a.ax, sm, pair0, lim, tid);
+                __syncthreads();
                 X::pass1_fwd(sm, tid);
                 __syncthreads();
                 if (PX::R2 > 1) { X::pass2_fwd(sm, tid); __syncthreads(); }
@@ -301,6 +228,8 @@ __global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
                 __syncthreads();
                 X::store_forward(a.ax, sm, pair0, lim, tid);
             } else {
+                X::load_inverse(a.ax, sm, pair0, lim, tid);
+                __syncthreads();
                 X::pass3_inv(sm, tid);
                 __syncthreads();
                 if (PX::R2 > 1) { X::pass2_inv(sm, tid); __syncthreads(); }
@@ -310,6 +239,8 @@ __global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
             }
         } else if (cur.type == TASK_Y) {
             if (!INV) {
+                Y::load_forward(a.ay, sm, cur.idx, cur.k, tid);
+                __syncthreads();
                 Y::pass1_fwd(sm, tid);
                 __syncthreads();
                 if (PY::R2 > 1) { Y::pass2_fwd(sm, tid); __syncthreads(); }
@@ -317,6 +248,8 @@ __global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
                 __syncthreads();
                 Y::store_forward(a.ay, sm, cur.idx, cur.k, tid);
             } else {
+                Y::load_inverse(a.ay, sm, cur.idx, cur.k, tid);
+                __syncthreads();
                 Y::pass3_inv(sm, tid);
                 __syncthreads();
                 if (PY::R2 > 1) { Y::pass2_inv(sm, tid); __syncthreads(); }
@@ -324,9 +257,6 @@ __global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
                 __syncthreads();
                 Y::store_inverse(a.ay, sm, cur.idx, cur.k, tid);
             }
-        } else if (!INV && cur.type == TASK_D) {
-            const int j0 = cur.idx * a.drows;
-            div_rows<NT, 2>(a.ax, cur.k, j0, min(j0 + a.drows, ny), tid);
         } else if (INV && cur.type == TASK_G) {
             const int j0 = cur.idx * a.grows;
             grad_rows<NT, 2>(a.g, cur.k, j0, min(j0 + a.grows, ny), tid);
@@ -337,14 +267,8 @@ __global__ void __launch_bounds__(NT, 1) fused_xy_kernel(const FusedArgs a) {
             __threadfence();                               // ... and visible before the count moves
             atomicAdd(a.counters + (size_t)cur.slot * a.cstride + cur.k, 1u);
         }
-        if (nxt.type == TASK_END) break;
-        if (!ready) {
-            block_wait(nxt);
-            stage_in(nxt);
-        }
         cur = nxt;
     }
-    fx_cp_async_wait_all();
 }
 
 template <class K>
@@ -366,8 +290,9 @@ cudaError_t fused_run(int what, const FusedArgs* a, int num_sms, int* grid, size
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&oa, ka, NT, bytes);
         if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&oc, kc, NT, bytes);
         if (e != cudaSuccess) return e;
-        if (oa < 1 || oc < 1) return cudaErrorLaunchOutOfResources;
-        *grid = num_sms;                                   // one persistent CTA per SM
+        const int occ = oa < oc ? oa : oc;
+        if (occ < 1) return cudaErrorLaunchOutOfResources;
+        *grid = occ * num_sms;                             // persistent: every CTA resident
         *smem = bytes;
         return cudaSuccess;
     }

@@ -216,6 +216,12 @@ struct XPass {
     static CANS_HD void pass1_inv(cplx* sm, int tid) { pass<N, P::R1, true>(sm, tw_smem(sm), tid); }
     static CANS_HD void pass2_inv(cplx* sm, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw_smem(sm) + P::TW1, tid); }
     static CANS_HD void pass3_inv(cplx* sm, int tid) { pass<P::R3, P::R3, true>(sm, nullptr, tid); }
+    // the same passes with this direction's twiddle table given explicitly (fused kernels: one table shared
+    // by the warp groups of a CTA)
+    static CANS_HD void pass1_fwd(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, false>(sm, tw, tid); }
+    static CANS_HD void pass2_fwd(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, false>(sm, tw + P::TW1, tid); }
+    static CANS_HD void pass1_inv(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, true>(sm, tw, tid); }
+    static CANS_HD void pass2_inv(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw + P::TW1, tid); }
 
     // ---- forward store: separate the two lines and write slots ----
     static CANS_HD void store_forward(const XYArgs& a, const cplx* sm, long pair0, long npairs, int tid) {
@@ -396,6 +402,12 @@ struct YPass {
     static CANS_HD void pass1_inv(cplx* sm, int tid) { pass<N, P::R1, true>(sm, tw_smem(sm), tid); }
     static CANS_HD void pass2_inv(cplx* sm, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw_smem(sm) + P::TW1, tid); }
     static CANS_HD void pass3_inv(cplx* sm, int tid) { pass<P::R3, P::R3, true>(sm, nullptr, tid); }
+    // the same passes with this direction's twiddle table given explicitly (fused kernels: one table shared
+    // by the warp groups of a CTA)
+    static CANS_HD void pass1_fwd(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, false>(sm, tw, tid); }
+    static CANS_HD void pass2_fwd(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, false>(sm, tw + P::TW1, tid); }
+    static CANS_HD void pass1_inv(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, true>(sm, tw, tid); }
+    static CANS_HD void pass2_inv(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw + P::TW1, tid); }
 
     static CANS_HD void store_forward(const XYArgs& a, const cplx* sm, int ctile, int k, int tid) {
         double* base = tile_base(a, ctile, k);

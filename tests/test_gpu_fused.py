@@ -144,3 +144,11 @@ def test_fused_projection_against_oracle(B):
     check(wd.cpu().numpy(), wn, what="w")
     check(pd.cpu().numpy(), phi, scale=dt, what="dt*Phi")
     assert np.array_equal(wd.cpu().numpy()[-1], w[-1])
+
+
+def test_unfused_only_sizes_report_it(B):
+    bc = make_bc("PP", "PP", "NN")
+    plan = B.PoissonPlan(256, 128, 4, 1.0, 1.0, 1.0, bc)        # ny = 128 has no fused kernels
+    assert plan.set_fusion(True) is False
+    assert plan.launches_per_solve == 5
+    plan.close()
