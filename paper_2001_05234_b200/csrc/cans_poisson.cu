@@ -38,12 +38,50 @@ static int fail_cuda(cudaError_t e, const char* where) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// a7: velocity correction u -= dt G Phi (eq. 2c): grid-stride loop over pairs of x-adjacent cells
+// a7: velocity correction u -= dt G Phi (eq. 2c).  A thread owns one pair of x-adjacent cells of a row
+// and marches up GRAD_KC planes, carrying Phi(k+1) in registers to become the centre value of the next
+// plane: every Phi value is read from HBM once (the row above comes from L2, it is the neighbour thread's
+// carry), so the kernel moves its algorithmic 56 B/cell.  The CTAs resident at one time sweep the planes
+// together, which keeps the seven streams (Phi, u, v, w in; u, v, w out) sequential in DRAM.
 // ------------------------------------------------------------------------------------------------
+constexpr int GRAD_KC = 32;
+
 __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
-    const size_t npair = (size_t)a.nx / 2 * a.ny * a.nz;
-    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < npair; t += (size_t)gridDim.x * blockDim.x)
-        grad_correct_pair(a, t);
+    const int hx = a.nx / 2;
+    const size_t cols = (size_t)hx * a.ny;
+    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= cols) return;
+    const int k0 = (int)blockIdx.y * GRAD_KC;
+    const int k1 = (k0 + GRAD_KC < a.nz) ? k0 + GRAD_KC : a.nz;
+    const int i = 2 * (int)(c % hx);
+    const int j = (int)(c / hx);
+    const size_t plane = (size_t)a.nx * a.ny;
+    const size_t rowo = (size_t)j * a.nx + i;
+    size_t o = (size_t)k0 * plane + rowo;
+    double2 ph = *reinterpret_cast<const double2*>(a.phi + o);
+    for (int k = k0; k < k1; ++k, o += plane) {
+        GradIn in;
+        in.o = o;
+        in.k = k;
+        in.ph = ph;
+        in.phx = (i + 2 < a.nx) ? a.phi[o + 2] : a.gx_sgn * a.phi[o - i + a.gx_idx];
+        if (j + 1 < a.ny) in.phy = *reinterpret_cast<const double2*>(a.phi + o + a.nx);
+        else {
+            in.phy = *reinterpret_cast<const double2*>(a.phi + (size_t)k * plane + (size_t)a.gy_idx * a.nx + i);
+            in.phy.x *= a.gy_sgn; in.phy.y *= a.gy_sgn;
+        }
+        if (k + 1 < a.nz) {
+            in.phz = *reinterpret_cast<const double2*>(a.phi + o + plane);
+            ph = in.phz;                       // centre value of the next plane
+        } else {
+            in.phz = *reinterpret_cast<const double2*>(a.phi + (size_t)a.gz_idx * plane + rowo);
+            in.phz.x *= a.gz_sgn; in.phz.y *= a.gz_sgn;
+        }
+        in.uu = *reinterpret_cast<const double2*>(a.u + o);
+        in.vv = *reinterpret_cast<const double2*>(a.v + o);
+        in.ww = *reinterpret_cast<const double2*>(a.w + o);
+        grad_apply(a, in);
+    }
 }
 
 bool fused_dispatch(int nx, int ny, int what, const FusedArgs* a, int num_sms, int* grid, size_t* smem,
@@ -345,12 +383,10 @@ static int launch_fused(cans_poisson_plan* pl, bool inv, double* p, const XYArgs
 }
 
 static int launch_grad(cans_poisson_plan* pl, const GradArgs& g, cudaStream_t st) {
-    const size_t npair = (size_t)pl->nx / 2 * pl->ny * pl->nz;
-    size_t blocks = (npair + 255) / 256;
-    const size_t cap = (size_t)pl->num_sms * 32;
-    if (blocks > cap) blocks = cap;
+    const size_t cols = (size_t)pl->nx / 2 * pl->ny;
+    dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((pl->nz + GRAD_KC - 1) / GRAD_KC));
     LaunchScope scope(pl, st, "grad_correct");
-    grad_correct_kernel<<<(unsigned)blocks, 256, 0, st>>>(g);
+    grad_correct_kernel<<<grid, 256, 0, st>>>(g);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
     return CANS_OK;
