@@ -157,7 +157,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    nz_sample = 8
+    nz_sample = 32
     cells, times = time_oracle_sample(nz_sample, args.warmup + args.steps)
     timed = times[args.warmup:]
     total = sum(timed)
@@ -328,7 +328,7 @@ def run_ours(args):
     # ---- CPU baseline: the oracle on a bounded sample, host cores of this box ----
     cpu_baseline = None
     if world == 1 and not args.no_cpu:
-        nz_sample = 32
+        nz_sample = 256
         ccells, times = time_oracle_sample(nz_sample, 1)
         cpu_baseline = {"value": ccells / times[0] / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
                         "sample": f"oracle.projection on a 1024x768x{nz_sample} slab of C5 (same domain, bc, "
