@@ -22,6 +22,7 @@
 #include "z_kernels.cuh"
 #include "grad_pass.cuh"
 #include "fused_kernels.cuh"
+#include "xw_kernels.cuh"
 
 namespace cans {
 
@@ -124,6 +125,8 @@ struct cans_poisson_plan {
     // device tables
     double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc, *rstart, *r00;
     cplx *tw_x, *tw_y, *wpost_x, *wpost_y;
+    cplx* tw2_x;              // W_nx^(p k1), [nx/32][32]: warp-per-line x kernels (xw_pass.cuh), or NULL
+    int use_xw;               // 1: x transforms run the warp-per-line kernels
     double inv_lz;
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
@@ -267,6 +270,12 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     up(make_pass_twiddles(fy), &pl->tw_y);
     up(make_post_twiddles(nx), &pl->wpost_x);
     up(make_post_twiddles(ny), &pl->wpost_y);
+    pl->tw2_x = nullptr;
+    pl->use_xw = 0;
+    if (xw_supported(nx)) {
+        up(make_two_pass_twiddles(nx), &pl->tw2_x);
+        pl->use_xw = 1;
+    }
     if (e == cudaSuccess) {
         void* d = nullptr;
         e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
@@ -324,6 +333,11 @@ static const char* const XY_NAMES[5] = {"x_fwd", "x_fwd_div", "x_inv", "y_fwd", 
 static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, cudaStream_t st) {
     cudaError_t err = cudaSuccess;
     LaunchScope scope(pl, st, XY_NAMES[op]);
+    if (pl->use_xw && !pl->fused && (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV) &&
+        xw_launch(n, op, a, pl->tw2_x, st, &err)) {
+        if (err != cudaSuccess) return fail_cuda(err, "x transform launch");
+        return CANS_OK;
+    }
     if (launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||
         launch_xy_group_c(n, op, a, st, &err) || launch_xy_group_d(n, op, a, st, &err)) {
         if (err != cudaSuccess) return fail_cuda(err, "x/y transform launch");

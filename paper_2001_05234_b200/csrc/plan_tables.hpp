@@ -75,6 +75,18 @@ inline std::vector<double> make_pass_twiddles(const FftRadices& f) {
     return t;
 }
 
+// twiddles between the two passes of the warp-per-line transform (xw_pass.cuh): [k1][p] = W_n^(p k1), p < 32, k1 < n/32
+inline std::vector<double> make_two_pass_twiddles(int n) {
+    std::vector<double> t;
+    for (int k1 = 0; k1 < n / 32; ++k1)
+        for (int p = 0; p < 32; ++p) {
+            double re, im;
+            unit_root((long long)p * k1, n, &re, &im);
+            t.push_back(re); t.push_back(im);
+        }
+    return t;
+}
+
 // w^q = exp(-i pi q / (2n)) = exp(-2 pi i q / (4n)), q = 0..n/2-1
 inline std::vector<double> make_post_twiddles(int n) {
     std::vector<double> t;

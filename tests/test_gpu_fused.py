@@ -1,7 +1,9 @@
 """GPU tests of the fused launch sequence (persistent pass-A / pass-C kernels, fused_pass.cuh).
 
-The fused and the unfused sequence run the same phase functions, so their results must be BIT-identical;
-the fused sequence is additionally compared with the CPU oracle (same bar as test_gpu_parity.py).
+The fused sequence runs the 3-pass phase functions of xy_pass.cuh.  Where the unfused sequence runs the same
+functions (nx not in {512, 768, 1024}) the two results must be BIT-identical; for the long x lines the unfused
+sequence uses the warp-per-line kernels (xw_pass.cuh, another factorisation) and the two must agree to rounding
+(relative L2 <= 1e-13).  The fused sequence is additionally compared with the CPU oracle (bar of test_gpu_parity.py).
 Small nz values exercise the ramp-up / ramp-down of the ticket order (planes fewer than the lag).
 """
 import itertools
@@ -23,6 +25,14 @@ MAX_ABS = 1e-10
 def B():
     from paper_2001_05234_b200 import binding
     return binding
+
+
+def same(a, b, nx):
+    """fused vs unfused: identical bits when both run the same phase functions, else equal to rounding"""
+    if nx not in (512, 768, 1024):
+        return torch.equal(a, b)
+    den = float(b.norm())
+    return float((a - b).norm()) <= 1e-13 * den if den > 0 else float((a - b).abs().max()) <= 1e-13
 
 
 def make_bc(px, py, pz):
@@ -78,8 +88,8 @@ def test_fused_equals_unfused_bitwise_poisson(B, nx, ny, nz, stretch):
         plan.poisson_solve(p0)
         torch.cuda.synchronize()
         plan.close()
-        assert torch.equal(p1, p0), f"{px}/{py}/{pz} {nx}x{ny}x{nz}"
-        assert torch.equal(p1b, p0)
+        assert same(p1, p0, nx), f"{px}/{py}/{pz} {nx}x{ny}x{nz}"
+        assert torch.equal(p1b, p1)
 
 
 @pytest.mark.parametrize("nx,ny,nz", [(256, 256, 6), (512, 768, 9), (1024, 384, 2), (384, 256, 1 + 32)])
@@ -102,7 +112,7 @@ def test_fused_equals_unfused_bitwise_projection(B, nx, ny, nz):
             out.append((uu, vv, ww, p))
         plan.close()
         for a, b, nm in zip(out[0], out[1], "uvwp"):
-            assert torch.equal(a, b), f"{nm}: {px}/{py}/{pz} {nx}x{ny}x{nz}"
+            assert same(a, b, nx), f"{nm}: {px}/{py}/{pz} {nx}x{ny}x{nz}"
 
 
 def test_fused_poisson_against_oracle(B):
