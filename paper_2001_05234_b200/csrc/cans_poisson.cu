@@ -23,6 +23,7 @@
 #include "grad_pass.cuh"
 #include "fused_kernels.cuh"
 #include "xw_kernels.cuh"
+#include "yw_kernels.cuh"
 
 namespace cans {
 
@@ -127,6 +128,8 @@ struct cans_poisson_plan {
     cplx *tw_x, *tw_y, *wpost_x, *wpost_y;
     cplx* tw2_x;              // W_nx^(p k1), [nx/32][32]: warp-per-line x kernels (xw_pass.cuh), or NULL
     int use_xw;               // 1: x transforms run the warp-per-line kernels
+    cplx* tw2_y;              // the same for ny (yw_pass.cuh), or NULL
+    int use_yw;
     double inv_lz;
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
@@ -276,6 +279,12 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         up(make_two_pass_twiddles(nx), &pl->tw2_x);
         pl->use_xw = 1;
     }
+    pl->tw2_y = nullptr;
+    pl->use_yw = 0;
+    if (yw_supported(ny) && (nx / 2) % YW_TXC == 0) {
+        up(make_two_pass_twiddles(ny), &pl->tw2_y);
+        pl->use_yw = 1;
+    }
     if (e == cudaSuccess) {
         void* d = nullptr;
         e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
@@ -336,6 +345,10 @@ static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, 
     if (pl->use_xw && !pl->fused && (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV) &&
         xw_launch(n, op, a, pl->tw2_x, st, &err)) {
         if (err != cudaSuccess) return fail_cuda(err, "x transform launch");
+        return CANS_OK;
+    }
+    if (pl->use_yw && !pl->fused && (op == OP_Y_FWD || op == OP_Y_INV) && yw_launch(n, op, a, pl->tw2_y, st, &err)) {
+        if (err != cudaSuccess) return fail_cuda(err, "y transform launch");
         return CANS_OK;
     }
     if (launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||

@@ -102,10 +102,11 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
         tile_scalars(nxt, rs_n, l1_n, l2_n);   // consumed in the next iteration
         mbar_wait(&s_bar[b], (phases >> b) & 1u);   // the current tile has landed (the next may still fly)
         phases ^= 1u << b;
-        if (tid == 0 && nxt < a.ntiles) s_next = (long)atomicAdd(a.ticket, 1u);
         ZState<MROWS> st;
         Z::phase1(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2, tid);
         __syncthreads();
+        // every thread has read s_next (before the barrier above): thread 0 may now draw the ticket after next
+        if (tid == 0 && nxt < a.ntiles) s_next = (long)atomicAdd(a.ticket, 1u);
         Z::phase2a(a, zsm, st, tid);
         __syncthreads();
         Z::phase2b(a, zsm, st, tid);
