@@ -35,6 +35,24 @@ struct YWPass {
         return a.p + (size_t)k * a.nx * a.ny + 2 * (size_t)ctile * YW_TXC;
     }
 
+    // W_N^(lane k1), k1 = 1..R1-1, applied to v (conjugated for the inverse).  Two CTAs' tiles leave almost no
+    // L1, so only every 8th root is read from the plan's table (exact); the ones between are products with
+    // W_N^lane -- at most 7 roundings, far inside the 1e-11 parity bar.
+    template <bool INV>
+    static CANS_D void apply_twiddles(cplx (&v)[R1], const cplx* __restrict__ tw, int lane) {
+        cplx anchor[R1 / 8];
+#pragma unroll
+        for (int g = 0; g < R1 / 8; ++g) anchor[g] = __ldg(tw + (g == 0 ? 1 : 8 * g) * 32 + lane);
+        const cplx w1 = anchor[0];
+        cplx wk = w1;
+#pragma unroll
+        for (int k1 = 1; k1 < R1; ++k1) {
+            if ((k1 & 7) == 0) wk = anchor[k1 / 8];
+            else if (k1 > 1) wk = cmul(wk, w1);
+            v[k1] = INV ? cmulc(v[k1], wk) : cmul(v[k1], wk);
+        }
+    }
+
     // ---- in-place column transforms (one warp; col = &tile[f], element e at col[e * RS]) ----
     // natural-order input, natural-order output, unnormalised; exchange rows k1*32 + (p ^ k1)
     static CANS_D void column_forward(cplx* col, const cplx* __restrict__ tw, int lane) {
@@ -42,8 +60,7 @@ struct YWPass {
 #pragma unroll
         for (int m = 0; m < R1; ++m) v[m] = col[(lane + 32 * m) * RS];
         Dft<R1, false>::run(v);
-#pragma unroll
-        for (int k1 = 1; k1 < R1; ++k1) v[k1] = cmul(v[k1], __ldg(tw + k1 * 32 + lane));
+        apply_twiddles<false>(v, tw, lane);
         __syncwarp();                                   // every lane has read its rows
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) col[(k1 * 32 + (lane ^ k1)) * RS] = v[k1];
@@ -76,8 +93,7 @@ struct YWPass {
         cplx v[R1];
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) v[k1] = col[(k1 * 32 + (lane ^ k1)) * RS];
-#pragma unroll
-        for (int k1 = 1; k1 < R1; ++k1) v[k1] = cmulc(v[k1], __ldg(tw + k1 * 32 + lane));
+        apply_twiddles<true>(v, tw, lane);
         Dft<R1, true>::run(v);
         __syncwarp();
 #pragma unroll
