@@ -47,7 +47,8 @@ typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the li
  * cans_poisson_plan_create -- build the plan for L Phi = f (eqs. 5-6).
  *
  *   nx, ny, nz   cells per direction (x, y uniform: "uniformly-spaced in two directions").
- *                nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048;
+ *                nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048
+ *                (512, 768 and 1024 run the warp-level 2-pass kernels, the others the 3-pass kernels);
  *                2 <= nz <= 1024.
  *   lx, ly, lz   domain lengths (> 0); dx = lx/nx, dy = ly/ny.
  *   bc           bc[d][0] / bc[d][1] = PRESSURE boundary condition on the lower / upper face of
@@ -133,11 +134,12 @@ const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
 
 /*
  * cans_plan_set_fusion -- switch between the two launch sequences of a plan (both are this library's
- * CUDA kernels and run the same phase functions, so results are bit-identical):
- *   fused   (default when nx and ny are both in {256,384,512,768,1024}): pass A = divergence + x + y
- *           forward transforms and pass C = y + x inverse transforms + gradient correction, each one
- *           persistent kernel whose intermediate plane stays in L2 (3 launches per call);
- *   unfused one kernel per step of SURVEY 8(a) (5 launches per solve, 6 per projection).
+ * CUDA kernels; their results agree to rounding, and bit for bit where both run the same transform code):
+ *   unfused (default) one kernel per step of SURVEY 8(a): 5 launches per solve, 6 per projection
+ *           (the divergence is fused into the forward x transform's load);
+ *   fused   (opt-in, nx and ny both in {256,384,512,768,1024}): pass A = divergence + x + y forward
+ *           transforms and pass C = y + x inverse transforms + gradient correction, each one persistent
+ *           kernel whose intermediate plane stays in L2 (3 launches per call).  Currently slower.
  * Returns the resulting state (1 fused, 0 unfused); a NULL plan sets the thread's status to
  * CANS_ERR_INVALID_ARG and returns 0.
  */

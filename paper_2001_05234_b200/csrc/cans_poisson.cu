@@ -1,13 +1,15 @@
 // cans_poisson.cu -- the C ABI of include/cans_poisson.h: plan creation (tables), the z-solve and
 // gradient-correction kernels, and the launch sequences of cans_poisson_solve / cans_projection.
 //
-// Hot path (eqs. 2b, 5, 6, 2c):
-//   a1+a2  x_pass_kernel<fwd, DIV>   divergence fused into the forward x transform
-//   a3     y_pass_kernel<fwd>        forward y transform (strided, staged in shared memory)
-//   a4     z_solve_kernel            Thomas solve per (kx, ky) mode, singular mode pinned
-//   a5     y_pass_kernel<inv>
-//   a6     x_pass_kernel<inv>
-//   a7     grad_correct_kernel       u -= dt G Phi
+// Hot path (eqs. 2b, 5, 6, 2c), default launch sequence:
+//   a1+a2  xw_kernel<fwd, DIV> / x_pass_kernel   divergence fused into the forward x transform
+//   a3     yw_kernel<fwd>      / y_pass_kernel   forward y transform (strided, tile staged in shared memory)
+//   a4     z_solve_kernel                        Thomas solve per (kx, ky) mode (TMA tiles), singular mode pinned
+//   a5     yw_kernel<inv>      / y_pass_kernel
+//   a6     xw_kernel<inv>      / x_pass_kernel
+//   a7     grad_correct_kernel                   u -= dt G Phi
+// (xw / yw: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
+//  FFTs for the other lengths.)  Opt-in: the fused persistent passes of fused_pass.cuh.
 #include <cuda_runtime.h>
 
 #include <cstdio>

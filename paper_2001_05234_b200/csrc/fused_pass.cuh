@@ -4,20 +4,22 @@
 //   pass C = a5 + a6 + a7 : inverse y -> inverse x (eq. 6) -> u -= dt G Phi (eq. 2c)
 //
 // A k-plane (C5: 6.3 MB) does not fit one SM's shared memory but fits the 126 MB L2 many times, so the
-// intermediate planes of a pass never have to reach HBM.  One persistent CTA per SM draws TICKETS from a
+// intermediate planes of a pass never have to reach HBM.  Persistent CTAs (two per SM) draw TICKETS from a
 // global counter.  Tickets are ordered in ROUNDS; round r holds, in this order, the tasks of up to three
 // SLOTS, slot s working on plane k = r - off[s]:
-//     pass A (projection):  D(r)  divergence rows     X(r-1)  x transforms     Y(r-2)  y transforms
-//     pass A (Poisson):     X(r)                      Y(r-1)
-//     pass C:               Y(r)  inverse y           X(r-1)  inverse x        G(r-3)  gradient rows
+//     pass A:  X(r)  [divergence +] x transforms     Y(r-2)  y transforms
+//     pass C:  Y(r)  inverse y      X(r-2)  inverse x      G(r-5)  gradient rows   (Poisson only: no G)
 // A task of slot s waits until every task of slot s-1 on its plane has signalled (G also waits for the
 // plane above, whose Phi it reads).  A task therefore only ever waits for tasks with SMALLER tickets,
 // which are finished or held by a running CTA: no deadlock, no co-residency requirement.
+// The HBM-resident input rows of the next task are prefetched into L2 (cp.async.bulk.prefetch.L2) while
+// the current task runs; the task bodies are the 3-pass phase functions of xy_pass.cuh.
 //
-// Latency hiding: the input of the NEXT transform task is copied global -> shared (cp.async.cg, no
-// register staging, L2-coherent) into a staging buffer while the CURRENT task computes in the work
-// buffer; divergence / gradient tasks stream through registers with several pairs of loads in flight
-// and have their HBM rows prefetched into L2 (cp.async.bulk.prefetch.L2) one task ahead.
+// STATUS (round 1): correct and parity-tested, but slower than the unfused sequence (19.9 ms vs 11.9 ms
+// per C5 projection): the CTA-synchronous phases serialise on an SM and a plane lag long enough to avoid
+// spinning pushes dirty intermediate planes out of L2.  Opt-in through cans_plan_set_fusion; see
+// DESIGN.md section 7 for the measurements of the three variants that were tried and the plan
+// (warp-level x tasks of xw_pass.cuh inside the persistent kernel).
 #pragma once
 #include <cuda_runtime.h>
 #include "xy_pass.cuh"

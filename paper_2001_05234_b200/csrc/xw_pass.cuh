@@ -76,6 +76,24 @@ struct XWPass {
     }
 
 #if defined(__CUDACC__)
+    // W_N^(lane k1), k1 = 1..R1-1, applied to v (conjugated for the inverse): every 8th root is read from the
+    // plan's table (exact), the ones between are products with W_N^lane (at most 7 roundings) -- 4 table
+    // reads per lane instead of R1 - 1 keep the L1 data pipe for the exchange
+    template <bool INV>
+    static CANS_D void apply_twiddles(cplx (&v)[R1], const cplx* __restrict__ tw, int lane) {
+        cplx anchor[R1 / 8];
+#pragma unroll
+        for (int g = 0; g < R1 / 8; ++g) anchor[g] = __ldg(tw + (g == 0 ? 1 : 8 * g) * 32 + lane);
+        const cplx w1 = anchor[0];
+        cplx wk = w1;
+#pragma unroll
+        for (int k1 = 1; k1 < R1; ++k1) {
+            if ((k1 & 7) == 0) wk = anchor[k1 / 8];
+            else if (k1 > 1) wk = cmul(wk, w1);
+            v[k1] = INV ? cmulc(v[k1], wk) : cmul(v[k1], wk);
+        }
+    }
+
     // ---- forward: rows (ro, ro + nx) of the field (or the divergence at those rows) -> slots ----
     template <bool DIV>
     static CANS_D void forward(const XYArgs& a, const cplx* __restrict__ tw, cplx* buf, size_t ro, int j, int k, int lane) {
@@ -154,8 +172,7 @@ struct XWPass {
         }
         __syncwarp();                                   // natural-order rows fully read: reuse the buffer for the exchange
         Dft<R1, false>::run(v);
-#pragma unroll
-        for (int k1 = 1; k1 < R1; ++k1) v[k1] = cmul(v[k1], __ldg(tw + k1 * 32 + lane));
+        apply_twiddles<false>(v, tw, lane);
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) buf[k1 * XSTRIDE + lane] = v[k1];
         __syncwarp();
@@ -233,8 +250,7 @@ struct XWPass {
         cplx v[R1];
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) v[k1] = buf[k1 * XSTRIDE + lane];
-#pragma unroll
-        for (int k1 = 1; k1 < R1; ++k1) v[k1] = cmulc(v[k1], __ldg(tw + k1 * 32 + lane));
+        apply_twiddles<true>(v, tw, lane);
         Dft<R1, true>::run(v);
         __syncwarp();                                   // exchange buffer fully read: reuse it in natural order
 #pragma unroll
