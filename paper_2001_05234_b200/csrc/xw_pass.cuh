@@ -102,8 +102,17 @@ struct XWPass {
         const size_t plane = (size_t)a.nx * a.ny;
         constexpr int NQ = H / 32;                       // column pairs per lane
         constexpr int UB = DIV ? 2 : (NQ < 16 ? NQ : 16);
+        cplx v[R1];
+        const bool direct = !DIV && a.kind == KIND_PP;   // periodic rows of a stored field: no staging needed
+        if (direct) {
+            // lane p takes x[p + 32 m] of both rows straight into registers: 2*R1 independent 8-byte loads,
+            // every load instruction of the warp reads 256 contiguous bytes
+#pragma unroll
+            for (int m = 0; m < R1; ++m)
+                v[m] = make_double2(__ldcg(a.p + ro + lane + 32 * m), __ldcg(a.p + ro + a.nx + lane + 32 * m));
+        }
 #pragma unroll 1
-        for (int m0 = 0; m0 < NQ; m0 += UB) {
+        for (int m0 = 0; m0 < (direct ? 0 : NQ); m0 += UB) {
             double2 fa[UB], fb[UB];
             if (!DIV) {
 #pragma unroll
@@ -163,12 +172,13 @@ struct XWPass {
             }
         }
         __syncwarp();
-        cplx v[R1];
+        if (!direct) {
 #pragma unroll
-        for (int m = 0; m < R1; ++m) {
-            const int i = index_of_elem(lane + 32 * m, a.kind);
-            v[m] = buf[i];
-            if (a.kind == KIND_DD && (i & 1)) v[m] = cneg(v[m]);
+            for (int m = 0; m < R1; ++m) {
+                const int i = index_of_elem(lane + 32 * m, a.kind);
+                v[m] = buf[i];
+                if (a.kind == KIND_DD && (i & 1)) v[m] = cneg(v[m]);
+            }
         }
         __syncwarp();                                   // natural-order rows fully read: reuse the buffer for the exchange
         Dft<R1, false>::run(v);
@@ -252,6 +262,17 @@ struct XWPass {
         for (int k1 = 0; k1 < R1; ++k1) v[k1] = buf[k1 * XSTRIDE + lane];
         apply_twiddles<true>(v, tw, lane);
         Dft<R1, true>::run(v);
+        if (a.kind == KIND_PP) {
+            // periodic lines need no permutation: lane p holds x[p + 32 m], so every store instruction of the
+            // warp writes 256 contiguous bytes of a row straight from registers
+#pragma unroll
+            for (int m = 0; m < R1; ++m) {
+                a.p[ro + lane + 32 * m] = v[m].x;
+                a.p[ro + a.nx + lane + 32 * m] = v[m].y;
+            }
+            __syncwarp();
+            return;
+        }
         __syncwarp();                                   // exchange buffer fully read: reuse it in natural order
 #pragma unroll
         for (int m = 0; m < R1; ++m) {
