@@ -201,6 +201,47 @@ def time_poisson_config(binding, workloads, torch, name, steps=10, warmup=3):
             "gcells_per_s": cells / med / 1e6, "min_bytes": 48.0 * cells}
 
 
+def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
+    """Every supported boundary-condition combination on the C5 grid (BASELINE.json: "for every supported
+    boundary-condition combination"): Poisson solve for {PP,NN,DD}^2 x {NN,DN,ND,DD}; projection step for the
+    combinations without a lower 'D' side ({PP,NN}^2 x {NN,ND}).  Median ms per call, CUDA events."""
+    w = workloads.make_workload("C5", device="cuda", with_fields=False)
+    nx, ny, nz = w.n
+    lx, ly, lz = w.lengths
+    f = torch.rand((nz, ny, nx), dtype=torch.float64, device="cuda")
+    bufs = [torch.empty_like(f) for _ in range(4)]
+    out = {"grid": f"{nx}x{ny}x{nz}", "poisson_ms": {}, "projection_ms": {}}
+
+    def med(fn, reset):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for _ in range(warmup):
+            reset(); fn()
+        for a, b in ev:
+            reset(); a.record(); fn(); b.record()
+        torch.cuda.synchronize()
+        ms = sorted(a.elapsed_time(b) for a, b in ev)
+        return ms[len(ms) // 2]
+
+    for px in ("PP", "NN", "DD"):
+        for py in ("PP", "NN", "DD"):
+            for pz in ("NN", "DN", "ND", "DD"):
+                bc = (tuple(px), tuple(py), tuple(pz))
+                plan = binding.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, w.dzc, w.dzf)
+                key = f"{px}/{py}/{pz}"
+                out["poisson_ms"][key] = med(lambda: plan.poisson_solve(bufs[3]), lambda: bufs[3].copy_(f))
+                if px != "DD" and py != "DD" and pz[0] == "N":
+                    def reset():
+                        for b in bufs[:3]:
+                            b.copy_(f)
+                    out["projection_ms"][key] = med(
+                        lambda: plan.projection(bufs[0], bufs[1], bufs[2], bufs[3], 1e-4), reset)
+                plan.close()
+    pv, jv = list(out["poisson_ms"].values()), list(out["projection_ms"].values())
+    out["poisson_ms_min_max"] = [min(pv), max(pv)]
+    out["projection_ms_min_max"] = [min(jv), max(jv)]
+    return out
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -317,6 +358,7 @@ def run_ours(args):
 
     # ---- Poisson-only timings of the other configs (context; parity-test cases, not bench lines) ----
     poisson = []
+    sweep = None
     if not args.no_extra:
         del u, v, ww, p
         torch.cuda.empty_cache()
@@ -324,6 +366,7 @@ def run_ours(args):
             r = time_poisson_config(binding, workloads, torch, name)
             r["frac_of_peak"] = r["min_bytes"] / (r["ms_median"] * 1e-3) / 1e9 / peak_gbs
             poisson.append(r)
+        sweep = bc_sweep(binding, workloads, torch)
 
     # ---- CPU baseline: the oracle on a bounded sample, host cores of this box ----
     cpu_baseline = None
@@ -350,6 +393,7 @@ def run_ours(args):
         "gpu_launches": plan.launches_per_projection * args.steps,
         "clocks": clocks,
         "poisson_configs": poisson,
+        "bc_sweep": sweep,
         "paper_context": "PAPER.md Table 1 (P:L274-284): 0.1404 s per full RK3 time step (3 projections + momentum), "
                          "1536x768x576, 16x V100 DGX-2 -- whole time step on other hardware, not this metric",
     }

@@ -188,17 +188,6 @@ struct XPass {
         line[P::pad(d1)] = z1;
     }
 
-    // forward "load" from a staged copy of the 2*NF rows in shared memory (row stride N doubles)
-    static CANS_HD void unpack_forward(const XYArgs& a, cplx* sm, const double* S, int tid) {
-        for (int idx = tid; idx < NF * H; idx += NT) {
-            const int f = idx / H;
-            const int e2 = idx - f * H;
-            const double* ra = S + (size_t)(2 * f) * N + 2 * e2;
-            put_forward(sm + f * P::NPAD, e2, *reinterpret_cast<const double2*>(ra),
-                        *reinterpret_cast<const double2*>(ra + N), a.kind);
-        }
-    }
-
     // ---- passes ----
     template <int M, int R, bool INV>
     static CANS_HD void pass(cplx* sm, const cplx* twp, int tid) {
@@ -216,12 +205,6 @@ struct XPass {
     static CANS_HD void pass1_inv(cplx* sm, int tid) { pass<N, P::R1, true>(sm, tw_smem(sm), tid); }
     static CANS_HD void pass2_inv(cplx* sm, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw_smem(sm) + P::TW1, tid); }
     static CANS_HD void pass3_inv(cplx* sm, int tid) { pass<P::R3, P::R3, true>(sm, nullptr, tid); }
-    // the same passes with this direction's twiddle table given explicitly (fused kernels: one table shared
-    // by the warp groups of a CTA)
-    static CANS_HD void pass1_fwd(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, false>(sm, tw, tid); }
-    static CANS_HD void pass2_fwd(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, false>(sm, tw + P::TW1, tid); }
-    static CANS_HD void pass1_inv(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, true>(sm, tw, tid); }
-    static CANS_HD void pass2_inv(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw + P::TW1, tid); }
 
     // ---- forward store: separate the two lines and write slots ----
     static CANS_HD void store_forward(const XYArgs& a, const cplx* sm, long pair0, long npairs, int tid) {
@@ -293,16 +276,6 @@ struct XPass {
             pre_inverse(ia.x, ia.y, ib.x, ib.y, wq, a.kind, Zq, Zm);
             line[P::pad(P::loc_of_freq(s))] = Zq;
             line[P::pad(P::loc_of_freq(N - s))] = Zm;
-        }
-    }
-
-    static CANS_HD void unpack_inverse(const XYArgs& a, cplx* sm, const double* S, int tid) {
-        for (int idx = tid; idx < NF * H; idx += NT) {
-            const int f = idx / H;
-            const int s = idx - f * H;
-            const double* ra = S + (size_t)(2 * f) * N + 2 * s;
-            put_inverse(a, sm + f * P::NPAD, s, *reinterpret_cast<const double2*>(ra),
-                        *reinterpret_cast<const double2*>(ra + N));
         }
     }
 
@@ -378,15 +351,6 @@ struct YPass {
         sm[e * TXC + f] = z;
     }
 
-    // forward "load" from a staged dense copy of the tile in shared memory (row stride 2*TXC doubles)
-    static CANS_HD void unpack_forward(const XYArgs& a, cplx* sm, const double* S, int tid) {
-        for (int idx = tid; idx < N * TXC; idx += NT) {
-            const int j = idx / TXC;
-            const int f = idx - j * TXC;
-            put_forward(a, sm, j, f, *reinterpret_cast<const double2*>(S + 2 * (size_t)idx));
-        }
-    }
-
     template <int M, int R, bool INV>
     static CANS_HD void pass(cplx* sm, const cplx* twp, int tid) {
         constexpr int TASKS = N / R;
@@ -402,12 +366,6 @@ struct YPass {
     static CANS_HD void pass1_inv(cplx* sm, int tid) { pass<N, P::R1, true>(sm, tw_smem(sm), tid); }
     static CANS_HD void pass2_inv(cplx* sm, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw_smem(sm) + P::TW1, tid); }
     static CANS_HD void pass3_inv(cplx* sm, int tid) { pass<P::R3, P::R3, true>(sm, nullptr, tid); }
-    // the same passes with this direction's twiddle table given explicitly (fused kernels: one table shared
-    // by the warp groups of a CTA)
-    static CANS_HD void pass1_fwd(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, false>(sm, tw, tid); }
-    static CANS_HD void pass2_fwd(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, false>(sm, tw + P::TW1, tid); }
-    static CANS_HD void pass1_inv(cplx* sm, const cplx* tw, int tid) { pass<N, P::R1, true>(sm, tw, tid); }
-    static CANS_HD void pass2_inv(cplx* sm, const cplx* tw, int tid) { if (P::R2 > 1) pass<P::M2, P::R2, true>(sm, tw + P::TW1, tid); }
 
     static CANS_HD void store_forward(const XYArgs& a, const cplx* sm, int ctile, int k, int tid) {
         double* base = tile_base(a, ctile, k);
@@ -474,15 +432,6 @@ struct YPass {
             pre_inverse(r0.x, r1.x, r0.y, r1.y, wq, a.kind, Zq, Zm);
             sm[P::loc_of_freq(s) * TXC + f] = Zq;
             sm[P::loc_of_freq(N - s) * TXC + f] = Zm;
-        }
-    }
-
-    static CANS_HD void unpack_inverse(const XYArgs& a, cplx* sm, const double* S, int tid) {
-        for (int idx = tid; idx < H * TXC; idx += NT) {
-            const int s = idx / TXC;
-            const int f = idx - s * TXC;
-            put_inverse(a, sm, s, f, *reinterpret_cast<const double2*>(S + ((size_t)(2 * s) * TXC + f) * 2),
-                        *reinterpret_cast<const double2*>(S + ((size_t)(2 * s + 1) * TXC + f) * 2));
         }
     }
 

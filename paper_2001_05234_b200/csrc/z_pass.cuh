@@ -9,8 +9,8 @@
 // B200 mapping ("register-resident partitioned Thomas", fed by an asynchronous tile pipeline):
 //   * a CTA is persistent and draws tiles of TC consecutive columns (x fastest => TC*8 contiguous
 //     bytes per row) from a global ticket counter; the tile of the NEXT ticket is copied global ->
-//     shared with cp.async (LDGSTS, 16 B per thread, no register staging) while the current tile is
-//     being solved, so HBM reads stay in flight during the whole arithmetic phase;
+//     shared by the TMA unit (one cp.async.bulk.tensor.2d per box, completion on an mbarrier; z_solve.cu)
+//     while the current tile is being solved, so HBM reads stay in flight during the whole arithmetic phase;
 //   * a column is cut into P segments of MROWS rows; thread (c, s) owns segment s of column c with
 //     its MROWS right-hand sides in registers; the whole column never leaves the SM between the
 //     forward and backward sweeps (16 B/cell of HBM traffic, the structural minimum);
@@ -55,16 +55,6 @@ CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) {
     return 1.0 / ((bk + lam) - gk * rprev);
 }
 
-#if defined(__CUDACC__)
-CANS_D void cp_async16(void* smem_dst, const void* gmem_src) {
-    const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem_src) : "memory");
-}
-CANS_D void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-CANS_D void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
-#endif
-
 template <int MROWS>
 struct ZState {
     double d[MROWS];
@@ -91,37 +81,6 @@ struct ZPass {
             sm[3 * nzp + i] = a.gz[i];
         }
     }
-
-#if defined(__CUDACC__)
-    // asynchronous copy of tile `tile` (rows 0..nz-1, TC columns) into buf[k*TC + c].
-    // nthreads is a multiple of the CH = TC/2 chunks of a row, so a thread keeps its chunk column and
-    // walks down the rows with a constant stride: no per-copy index arithmetic.
-    static CANS_D void prefetch_tile(const ZArgs& a, double* buf, long tile, int tid, int nthreads) {
-        constexpr int CH = TC / 2;                      // 16-byte chunks per row
-        const long col0 = tile * TC;
-        const size_t plane = (size_t)a.ncols;
-        if (col0 + TC <= a.ncols) {
-            const int q = tid % CH;
-            const int kstep = nthreads / CH;
-            const double* src = a.p + (size_t)(tid / CH) * plane + col0 + 2 * q;
-            double* dst = buf + (size_t)(tid / CH) * TC + 2 * q;
-            const size_t sstep = (size_t)kstep * plane;
-            const int dstep = kstep * TC;
-#pragma unroll 4
-            for (int k = tid / CH; k < a.nz; k += kstep) {
-                cp_async16(dst, src);
-                src += sstep;
-                dst += dstep;
-            }
-        } else {                                        // ragged last tile: plain guarded loads
-            for (int id = tid; id < a.nz * TC; id += nthreads) {
-                const int k = id / TC;
-                const int c = id - k * TC;
-                buf[(size_t)k * TC + c] = (col0 + c < a.ncols) ? a.p[(size_t)k * plane + col0 + c] : 0.0;
-            }
-        }
-    }
-#endif
 
     // phase 1: take the segment from the tile buffer, pivots, local forward sweep from a zero start;
     // publish (end, factor)
