@@ -265,6 +265,8 @@ def run_ours(args):
     plan = binding.plan_for(w)
     if args.no_fuse:
         plan.set_fusion(False)
+    if args.fuse and not plan.set_fusion(True):
+        raise SystemExit("bench.py --fuse: this (nx, ny) has no fused kernels")
     u0, v0, w0 = (w.fields[c] for c in "uvw")
     u, v, ww = torch.empty_like(u0), torch.empty_like(u0), torch.empty_like(u0)
     p = torch.empty_like(u0)
@@ -412,7 +414,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
-    ap.add_argument("--no-fuse", action="store_true", help="time the unfused launch sequence (one kernel per step)")
+    ap.add_argument("--no-fuse", action="store_true", help="time the unfused launch sequence (one kernel per step; the default)")
+    ap.add_argument("--fuse", action="store_true", help="time the opt-in fused persistent sequence (3 launches per step)")
     ap.add_argument("--no-extra", action="store_true", help="skip the Poisson-only timings of C2..C5")
     args = ap.parse_args()
     if args.impl == "reference":
