@@ -242,6 +242,23 @@ def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
     return out
 
 
+def max_over_ranks(total_ms, world, device):
+    """Replicas only: every rank times its own independent replica; the job time is
+    the slowest rank's (all-reduce MAX; NCCL on GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return total_ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gcells_per_s(cells, steps, world, total_ms):
+    """Weak scaling: `world` replicas of `cells` cells each, `steps` steps in `total_ms` (max over ranks)."""
+    return world * cells * steps / (total_ms * 1e-3) / 1e9
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -305,12 +322,9 @@ def run_ours(args):
     plan.set_profiling(False)
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(step_ms)
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, world, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * cells * args.steps / (total_ms * 1e-3) / 1e9
+    value = whole_job_gcells_per_s(cells, args.steps, world, total_ms)
 
     if rank != 0:
         if world > 1:
