@@ -51,8 +51,20 @@ struct ZArgs {
 };
 
 // one pivot step; shared by the plan-time table kernel and the solve so the values are identical
+// The reciprocal is the hardware seed (rcp.approx, ~20 bits) refined by two Newton steps: full double precision
+// to about one unit in the last place for these well-scaled, strictly negative denominators, without the range
+// checks and the slow path of the IEEE division -- the pivot chain is the longest dependency chain of the solve.
 CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) {
-    return 1.0 / ((bk + lam) - gk * rprev);
+    const double den = (bk + lam) - gk * rprev;
+#if defined(__CUDA_ARCH__)
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
+    r = fma(fma(-den, r, 1.0), r, r);
+    r = fma(fma(-den, r, 1.0), r, r);
+    return r;
+#else
+    return 1.0 / den;
+#endif
 }
 
 template <int MROWS>

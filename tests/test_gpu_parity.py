@@ -237,3 +237,35 @@ def test_repeated_calls_are_bit_identical(B, nx, ny, nz):
             for a, b in zip(ref, (u, v, ww, p)):
                 assert torch.equal(a, b)
     plan.close()
+
+
+@pytest.mark.parametrize("nx,ny,nz", [(512, 512, 9), (768, 1024, 5), (1024, 768, 6)])
+def test_warp_level_transform_kernels_every_kind_pair(B, nx, ny, nz):
+    """Lengths 512 / 768 / 1024 run the warp-level 2-pass kernels (xw_pass.cuh, yw_pass.cuh): every (x, y)
+    boundary-pair combination against the oracle, on a stretched grid, Poisson and (where allowed) projection."""
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    seed = 4000
+    for px, py in itertools.product(XY, XY):
+        pz = "ND" if (px == "PP" and py == "PP") else "NN"
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        seed += 1
+        f = random_rhs(nx, ny, nz, bc, dzf, seed)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        torch.cuda.synchronize()
+        ref = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        check_field(np_of(p), ref, what=f"poisson {px}/{py}/{pz} {nx}x{ny}x{nz}")
+        if px != "DD" and py != "DD":
+            rng = np.random.default_rng(seed)
+            u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+            ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+            pd = torch.empty_like(ud)
+            plan.projection(ud, vd, wd, pd, 1e-3)
+            torch.cuda.synchronize()
+            un, vn, wn, phi, _ = orc.projection(u, v, w, 1e-3, lx, ly, lz, bc, dzc, dzf)
+            for got, refv, sc, nm in ((ud, un, 1.0, "u"), (vd, vn, 1.0, "v"), (wd, wn, 1.0, "w"), (pd, phi, 1e-3, "dt*Phi")):
+                check_field(np_of(got), refv, scale=sc, what=f"projection {nm} {px}/{py}/{pz} {nx}x{ny}x{nz}")
+        plan.close()
