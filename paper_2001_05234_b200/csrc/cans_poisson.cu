@@ -13,6 +13,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -26,6 +27,7 @@
 #include "fused_kernels.cuh"
 #include "xw_kernels.cuh"
 #include "yw_kernels.cuh"
+#include "yt_kernels.cuh"
 
 namespace cans {
 
@@ -132,6 +134,7 @@ struct cans_poisson_plan {
     int use_xw;               // 1: x transforms run the warp-per-line kernels
     cplx* tw2_y;              // the same for ny (yw_pass.cuh), or NULL
     int use_yw;
+    int use_yt;               // 1: y transforms run the persistent TMA-fed kernels (yt_pass.cuh)
     double inv_lz;
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
@@ -287,6 +290,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         up(make_two_pass_twiddles(ny), &pl->tw2_y);
         pl->use_yw = 1;
     }
+    pl->use_yt = (pl->use_yw && yt_supported(ny) && std::getenv("CANS_NO_YT") == nullptr) ? 1 : 0;
     if (e == cudaSuccess) {
         void* d = nullptr;
         e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
@@ -347,6 +351,11 @@ static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, 
     if (pl->use_xw && !pl->fused && (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV) &&
         xw_launch(n, op, a, pl->tw2_x, st, &err)) {
         if (err != cudaSuccess) return fail_cuda(err, "x transform launch");
+        return CANS_OK;
+    }
+    if (pl->use_yt && !pl->fused && (op == OP_Y_FWD || op == OP_Y_INV) &&
+        yt_launch(n, op, a, pl->tw2_y, pl->num_sms, st, &err)) {
+        if (err != cudaSuccess) return fail_cuda(err, "y transform launch");
         return CANS_OK;
     }
     if (pl->use_yw && !pl->fused && (op == OP_Y_FWD || op == OP_Y_INV) && yw_launch(n, op, a, pl->tw2_y, st, &err)) {

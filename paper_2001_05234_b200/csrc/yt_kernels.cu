@@ -1,0 +1,100 @@
+// yt_kernels.cu -- persistent TMA-fed y transform kernels (yt_pass.cuh) and their launcher.
+#include "yt_kernels.cuh"
+
+namespace cans {
+
+extern __shared__ __align__(1024) unsigned char cans_dyn_smem_1k[];
+
+template <int N, int R1, bool INV>
+__global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx* __restrict__ tw,
+                                                      const __grid_constant__ CUtensorMap tmap, int ntx, long ntiles) {
+    typedef YTPass<N, R1> W;
+    cplx* bufs = reinterpret_cast<cplx*>(cans_dyn_smem_1k);
+    __shared__ __align__(8) unsigned long long s_bar[2];
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5, lane = tid & 31;
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    // tile t = (plane k, column tile c): boxes of 16 doubles x 256 rows at (16 c, k N + 256 box)
+    auto issue_load = [&](long t, int bsel) {
+        const int k = (int)(t / ntx);
+        const int c = (int)(t - (long)k * ntx);
+        mbar_expect_tx(&s_bar[bsel], W::TILE_BYTES);
+        for (int box = 0; box < W::NBOX; ++box)
+            tma_load_2d(bufs + (size_t)bsel * W::TILE + (size_t)box * YT_BOX_ROWS * YT_COLS, &tmap, 2 * YT_COLS * c,
+                        k * N + box * YT_BOX_ROWS, &s_bar[bsel]);
+    };
+    long t = blockIdx.x;
+    if (t >= ntiles) return;
+    if (tid == 0) issue_load(t, 0);
+    unsigned phases = 0u;
+    int b = 0;
+    for (; t < ntiles; t += gridDim.x) {
+        const long tn = t + gridDim.x;
+        if (tid == 0 && tn < ntiles) {
+            tma_store_wait_read();              // the write-back issued from buffer b^1 has finished reading it
+            issue_load(tn, b ^ 1);
+        }
+        mbar_wait(&s_bar[b], (phases >> b) & 1u);
+        phases ^= 1u << b;
+        cplx* T = bufs + (size_t)b * W::TILE;
+        if (INV) {
+            W::slots_in(a, T, warp, lane);
+            W::column_inverse(T, warp, tw, lane);
+            W::permute_out(T, warp, a.kind, lane);
+        } else {
+            W::permute_in(T, warp, a.kind, lane);
+            W::column_forward(T, warp, tw, lane);
+            W::slots_out(a, T, warp, lane);
+        }
+        fence_proxy_async_smem();               // this thread's shared-memory writes -> visible to the TMA unit
+        __syncthreads();
+        if (tid == 0) {
+            const int k = (int)(t / ntx);
+            const int c = (int)(t - (long)k * ntx);
+            for (int box = 0; box < W::NBOX; ++box)
+                tma_store_2d(&tmap, 2 * YT_COLS * c, k * N + box * YT_BOX_ROWS, T + (size_t)box * YT_BOX_ROWS * YT_COLS);
+            tma_store_commit();
+        }
+        b ^= 1;
+    }
+    if (tid == 0) tma_store_wait_all();
+}
+
+template <int N, int R1>
+static cudaError_t yt_launch_n(int op, const XYArgs& a, const cplx* tw, int num_sms, cudaStream_t st) {
+    const size_t smem = 2 * sizeof(cplx) * (size_t)YTPass<N, R1>::TILE;
+    static bool once = false;
+    if (!once) {
+        cudaError_t e = cudaFuncSetAttribute(yt_kernel<N, R1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(yt_kernel<N, R1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        once = true;
+    }
+    // the field as a 2-D tensor: nx doubles per row, ny*nz rows
+    CUtensorMap tmap;
+    cudaError_t e = make_tensor_map_2d(&tmap, a.p, (unsigned long long)a.nx, (unsigned long long)a.ny * a.nz,
+                                       (unsigned long long)a.nx * sizeof(double), 2 * YT_COLS, YT_BOX_ROWS,
+                                       CU_TENSOR_MAP_SWIZZLE_128B);
+    if (e != cudaSuccess) return e;
+    const int ntx = a.nx / 2 / YT_COLS;
+    const long ntiles = (long)ntx * a.nz;
+    const unsigned grid = (unsigned)(ntiles < num_sms ? ntiles : num_sms);
+    if (op == OP_Y_FWD) yt_kernel<N, R1, false><<<grid, YT_NT, smem, st>>>(a, tw, tmap, ntx, ntiles);
+    else yt_kernel<N, R1, true><<<grid, YT_NT, smem, st>>>(a, tw, tmap, ntx, ntiles);
+    return cudaGetLastError();
+}
+
+bool yt_launch(int n, int op, const XYArgs& a, const cplx* tw, int num_sms, cudaStream_t st, cudaError_t* err) {
+    switch (n) {
+        case 512: *err = yt_launch_n<512, 16>(op, a, tw, num_sms, st); return true;
+        case 768: *err = yt_launch_n<768, 24>(op, a, tw, num_sms, st); return true;
+        default: return false;
+    }
+}
+
+}  // namespace cans

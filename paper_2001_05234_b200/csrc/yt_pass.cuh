@@ -1,0 +1,193 @@
+// yt_pass.cuh -- TMA-fed y transforms (N = R1 * 32 with two tiles fitting shared memory: 512, 768): F^y of eq. 6
+// and its inverse.  Mathematics and slot layout as YPass / YWPass.
+//
+// A persistent CTA of 8 warps (one per SM) walks over tiles of 8 complex columns x N rows:
+//   * the TMA unit copies the tile global -> shared (cp.async.bulk.tensor.2d, boxes of 16 doubles x 256 rows,
+//     SWIZZLE_128B, completion on an mbarrier) and, after the transform, shared -> global -- no thread issues a
+//     global load or store, and the copy of tile n+1 / the write-back of tile n-1 overlap the transform of tile n
+//     (two buffers);
+//   * warp f owns column f of the tile from the first to the last shared-memory access: input permutation,
+//     2-pass register FFT (as yw_pass.cuh) and real/imaginary separation all happen in place with __syncwarp
+//     only; one CTA barrier per tile hands the finished tile to the TMA store.
+// With the 128-byte swizzle, element (row e, column f) sits at complex index e*8 + (f ^ (e & 7)): the eight lanes of a
+// quarter warp reading one column at eight consecutive (or XOR-permuted) rows hit eight different 16-byte bank
+// groups, so every column access of the FFT is conflict free without padding.
+#pragma once
+#include "xw_pass.cuh"
+#include "tma_util.cuh"
+
+namespace cans {
+
+constexpr int YT_COLS = 8;                       // complex columns per tile = warps per CTA
+constexpr int YT_NT = YT_COLS * 32;
+constexpr int YT_BOX_ROWS = 256;
+inline bool yt_supported(int n) { return n == 512 || n == 768; }
+
+template <int N_, int R1_>
+struct YTPass {
+    static constexpr int N = N_, R1 = R1_, H = N_ / 2;
+    static_assert(R1_ * 32 == N_ && N_ % YT_BOX_ROWS == 0, "N = R1 * 32, whole TMA boxes");
+    static constexpr int TILE = N * YT_COLS;                         // cplx per buffer
+    static constexpr int NBOX = N / YT_BOX_ROWS;
+    static constexpr unsigned TILE_BYTES = (unsigned)(TILE * sizeof(cplx));
+
+#if defined(__CUDACC__)
+    static CANS_D int at(int e, int f) { return e * YT_COLS + (f ^ (e & 7)); }
+
+    template <bool INV>
+    static CANS_D void apply_twiddles(cplx (&v)[R1], const cplx* __restrict__ tw, int lane) {
+        cplx anchor[R1 / 8];
+#pragma unroll
+        for (int g = 0; g < R1 / 8; ++g) anchor[g] = __ldg(tw + (g == 0 ? 1 : 8 * g) * 32 + lane);
+        const cplx w1 = anchor[0];
+        cplx wk = w1;
+#pragma unroll
+        for (int k1 = 1; k1 < R1; ++k1) {
+            if ((k1 & 7) == 0) wk = anchor[k1 / 8];
+            else if (k1 > 1) wk = cmul(wk, w1);
+            v[k1] = INV ? cmulc(v[k1], wk) : cmul(v[k1], wk);
+        }
+    }
+
+    // natural-order input -> natural-order spectrum, in place in column f (unnormalised)
+    static CANS_D void column_forward(cplx* t, int f, const cplx* __restrict__ tw, int lane) {
+        cplx v[R1];
+#pragma unroll
+        for (int m = 0; m < R1; ++m) v[m] = t[at(lane + 32 * m, f)];
+        Dft<R1, false>::run(v);
+        apply_twiddles<false>(v, tw, lane);
+        __syncwarp();
+#pragma unroll
+        for (int k1 = 0; k1 < R1; ++k1) t[at(k1 * 32 + (lane ^ k1), f)] = v[k1];
+        __syncwarp();
+        cplx w[32];
+        if (lane < R1) {
+#pragma unroll
+            for (int p = 0; p < 32; ++p) w[p] = t[at(lane * 32 + (p ^ lane), f)];
+            Dft<32, false>::run(w);
+        }
+        __syncwarp();
+        if (lane < R1) {
+#pragma unroll
+            for (int k2 = 0; k2 < 32; ++k2) t[at(lane + R1 * k2, f)] = w[k2];
+        }
+        __syncwarp();
+    }
+    static CANS_D void column_inverse(cplx* t, int f, const cplx* __restrict__ tw, int lane) {
+        cplx w[32];
+        if (lane < R1) {
+#pragma unroll
+            for (int k2 = 0; k2 < 32; ++k2) w[k2] = t[at(lane + R1 * k2, f)];
+            Dft<32, true>::run(w);
+        }
+        __syncwarp();
+        if (lane < R1) {
+#pragma unroll
+            for (int p = 0; p < 32; ++p) t[at(lane * 32 + (p ^ lane), f)] = w[p];
+        }
+        __syncwarp();
+        cplx v[R1];
+#pragma unroll
+        for (int k1 = 0; k1 < R1; ++k1) v[k1] = t[at(k1 * 32 + (lane ^ k1), f)];
+        apply_twiddles<true>(v, tw, lane);
+        Dft<R1, true>::run(v);
+        __syncwarp();
+#pragma unroll
+        for (int m = 0; m < R1; ++m) t[at(lane + 32 * m, f)] = v[m];
+        __syncwarp();
+    }
+
+    // rows j (as loaded) -> FFT input elements e, in place through registers (NN / DD only; PP is the identity)
+    static CANS_D void permute_in(cplx* t, int f, int kind, int lane) {
+        if (kind == KIND_PP) return;
+        cplx v[R1];
+#pragma unroll
+        for (int m = 0; m < R1; ++m) v[m] = t[at(lane + 32 * m, f)];
+        __syncwarp();
+#pragma unroll
+        for (int m = 0; m < R1; ++m) {
+            const int j = lane + 32 * m;
+            t[at(elem_of_index<N>(j, kind), f)] = (kind == KIND_DD && (j & 1)) ? cneg(v[m]) : v[m];
+        }
+        __syncwarp();
+    }
+    // FFT output elements e -> rows j (inverse of permute_in)
+    static CANS_D void permute_out(cplx* t, int f, int kind, int lane) {
+        if (kind == KIND_PP) return;
+        cplx v[R1];
+#pragma unroll
+        for (int m = 0; m < R1; ++m) {
+            const int j = lane + 32 * m;
+            const cplx z = t[at(elem_of_index<N>(j, kind), f)];
+            v[m] = (kind == KIND_DD && (j & 1)) ? cneg(z) : z;
+        }
+        __syncwarp();
+#pragma unroll
+        for (int m = 0; m < R1; ++m) t[at(lane + 32 * m, f)] = v[m];
+        __syncwarp();
+    }
+    // natural-order spectrum -> slot rows (2s, 2s+1), in place through registers (YPass::store_forward)
+    static CANS_D void slots_out(const XYArgs& a, cplx* t, int f, int lane) {
+        constexpr int NS = H / 32;
+        cplx zq[NS], zm[NS];
+#pragma unroll
+        for (int m = 0; m < NS; ++m) {
+            const int s = lane + 32 * m;
+            zq[m] = t[at(s, f)];
+            zm[m] = t[at(s == 0 ? H : N - s, f)];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int m = 0; m < NS; ++m) {
+            const int s = lane + 32 * m;
+            cplx r0, r1;
+            if (s == 0) {
+                const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
+                r0 = make_double2(zq[m].x, zq[m].y);
+                r1 = make_double2(c * zm[m].x, c * zm[m].y);
+            } else {
+                cplx wq = make_double2(1.0, 0.0);
+                if (a.kind != KIND_PP) wq = __ldg(a.wpost + s);
+                double A0, A1, B0, B1;
+                post_forward(zq[m], zm[m], wq, a.kind, A0, A1, B0, B1);
+                r0 = make_double2(A0, B0);
+                r1 = make_double2(A1, B1);
+            }
+            t[at(2 * s, f)] = r0;
+            t[at(2 * s + 1, f)] = r1;
+        }
+        __syncwarp();
+    }
+    // slot rows -> natural-order spectrum, in place through registers (YPass::load_inverse)
+    static CANS_D void slots_in(const XYArgs& a, cplx* t, int f, int lane) {
+        constexpr int NS = H / 32;
+        cplx r0[NS], r1[NS];
+#pragma unroll
+        for (int m = 0; m < NS; ++m) {
+            const int s = lane + 32 * m;
+            r0[m] = t[at(2 * s, f)];
+            r1[m] = t[at(2 * s + 1, f)];
+        }
+        __syncwarp();
+#pragma unroll
+        for (int m = 0; m < NS; ++m) {
+            const int s = lane + 32 * m;
+            if (s == 0) {
+                const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
+                t[at(0, f)] = make_double2(r0[m].x, r0[m].y);
+                t[at(H, f)] = make_double2(c * r1[m].x, c * r1[m].y);
+            } else {
+                cplx wq = make_double2(1.0, 0.0);
+                if (a.kind != KIND_PP) wq = __ldg(a.wpost + s);
+                cplx Zq, Zm;
+                pre_inverse(r0[m].x, r1[m].x, r0[m].y, r1[m].y, wq, a.kind, Zq, Zm);
+                t[at(s, f)] = Zq;
+                t[at(N - s, f)] = Zm;
+            }
+        }
+        __syncwarp();
+    }
+#endif
+};
+
+}  // namespace cans

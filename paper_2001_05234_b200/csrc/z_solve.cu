@@ -1,35 +1,8 @@
 // z_solve.cu -- pass B: persistent, cp.async double-buffered partitioned Thomas solve (z_pass.cuh).
-#include <cuda.h>
-
 #include "z_kernels.cuh"
+#include "tma_util.cuh"
 
 namespace cans {
-
-// ---- TMA / mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS) ----
-CANS_D unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-CANS_D void mbar_init(unsigned long long* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-CANS_D void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-CANS_D void mbar_wait(unsigned long long* bar, unsigned parity) {
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// 2-D tiled load: box (TC columns x box_rows rows) at (col0, row0) of the (nz, ncols) view of the field
-CANS_D void tma_load_2d(void* dst, const CUtensorMap* tmap, int col0, int row0, unsigned long long* bar) {
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];\n"
-        ::"r"(smem_u32(dst)), "l"(tmap), "r"(col0), "r"(row0), "r"(smem_u32(bar)) : "memory");
-}
 
 template <int MROWS, int TC>
 __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __grid_constant__ CUtensorMap tmap) {
@@ -53,7 +26,7 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
     if (tid == 0) {
         mbar_init(&s_bar[0], 1);
         mbar_init(&s_bar[1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        mbar_fence_init();
         s_next = (long)atomicAdd(a.ticket, 1u);
     }
     __syncthreads();
@@ -71,7 +44,7 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
     };
     if (tid == 0) {
         // the generic-proxy reads / writes of the staging area above are ordered before the async-proxy writes
-        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+        fence_proxy_async_smem();
         issue_tile(cur, 0);
         s_next = (long)atomicAdd(a.ticket, 1u);
     }
@@ -149,31 +122,6 @@ cudaError_t z_solve_configure(int nseg, int nz, int num_sms, int* grid_out, size
     }
 }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-static cudaError_t z_make_tensor_map(const ZArgs& a, int tc, CUtensorMap* tmap) {
-    static EncodeTiledFn encode = nullptr;
-    if (!encode) {
-        void* fn = nullptr;
-        cudaDriverEntryPointQueryResult qres;
-        cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
-        if (e != cudaSuccess) return e;
-        if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
-        encode = (EncodeTiledFn)fn;
-    }
-    const cuuint64_t dims[2] = {(cuuint64_t)a.ncols, (cuuint64_t)a.nz};
-    const cuuint64_t strides[1] = {(cuuint64_t)a.ncols * sizeof(double)};
-    const cuuint32_t box[2] = {(cuuint32_t)tc, (cuuint32_t)a.box_rows};
-    const cuuint32_t estr[2] = {1, 1};
-    CUresult r = encode(tmap, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 2, (void*)a.p, dims, strides, box, estr,
-                        CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                        CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
-}
-
 cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, cudaStream_t st) {
     ZArgs a = a_in;
     long g = grid;
@@ -187,7 +135,9 @@ cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, cudaStream_
     a.nbox = a.nseg / d;
     const int tc = z_tc_for(a.nseg);
     CUtensorMap tmap;
-    cudaError_t e = z_make_tensor_map(a, tc, &tmap);
+    cudaError_t e = make_tensor_map_2d(&tmap, a.p, (unsigned long long)a.ncols, (unsigned long long)a.nz,
+                                       (unsigned long long)a.ncols * sizeof(double), (unsigned)tc, (unsigned)a.box_rows,
+                                       CU_TENSOR_MAP_SWIZZLE_NONE);
     if (e != cudaSuccess) return e;
     switch (tc) {
         case 32: z_solve_kernel<Z_MROWS, 32><<<(unsigned)g, 32 * a.nseg, smem, st>>>(a, tmap); break;
