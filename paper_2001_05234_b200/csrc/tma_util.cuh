@@ -41,6 +41,9 @@ CANS_D void tma_store_2d(const CUtensorMap* tmap, int c0, int c1, const void* sr
 CANS_D void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
 // wait until the bulk stores of this thread have finished READING shared memory (the buffer may be reused)
 CANS_D void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
+// the same, allowing the PENDING most recent groups to be still reading
+template <int PENDING>
+CANS_D void tma_store_wait_read_pending() { asm volatile("cp.async.bulk.wait_group.read %0;\n" ::"n"(PENDING) : "memory"); }
 CANS_D void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory"); }
 // generic-proxy writes to shared memory become visible to the async proxy (TMA) after this fence
 CANS_D void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }

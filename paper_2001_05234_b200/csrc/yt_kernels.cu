@@ -20,24 +20,32 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     }
     __syncthreads();
     // tile t = (plane k, column tile c): boxes of 16 doubles x 256 rows at (16 c, k N + 256 box)
-    auto issue_load = [&](long t, int bsel) {
+    // FIRST: all boxes at once.  Otherwise box by box, each as soon as the write-back of the same box of the tile
+    // that occupied this buffer (one bulk group per box, oldest first) has finished reading shared memory.
+    auto issue_load = [&](long t, int bsel, bool first) {
         const int k = (int)(t / ntx);
         const int c = (int)(t - (long)k * ntx);
         mbar_expect_tx(&s_bar[bsel], W::TILE_BYTES);
-        for (int box = 0; box < W::NBOX; ++box)
+#pragma unroll
+        for (int box = 0; box < W::NBOX; ++box) {
+            if (!first) {
+                if (box == 0) tma_store_wait_read_pending<W::NBOX - 1>();
+                else if (box == 1) tma_store_wait_read_pending<(W::NBOX > 2 ? W::NBOX - 2 : 0)>();
+                else tma_store_wait_read_pending<0>();
+            }
             tma_load_2d(bufs + (size_t)bsel * W::TILE + (size_t)box * YT_BOX_ROWS * YT_COLS, &tmap, 2 * YT_COLS * c,
                         k * N + box * YT_BOX_ROWS, &s_bar[bsel]);
+        }
     };
     long t = blockIdx.x;
     if (t >= ntiles) return;
-    if (tid == 0) issue_load(t, 0);
+    if (tid == 0) issue_load(t, 0, true);
     unsigned phases = 0u;
     int b = 0;
     for (; t < ntiles; t += gridDim.x) {
         const long tn = t + gridDim.x;
         if (tid == 0 && tn < ntiles) {
-            tma_store_wait_read();              // the write-back issued from buffer b^1 has finished reading it
-            issue_load(tn, b ^ 1);
+            issue_load(tn, b ^ 1, false);
         }
         mbar_wait(&s_bar[b], (phases >> b) & 1u);
         phases ^= 1u << b;
@@ -57,8 +65,10 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
             const int k = (int)(t / ntx);
             const int c = (int)(t - (long)k * ntx);
             for (int box = 0; box < W::NBOX; ++box)
+            {
                 tma_store_2d(&tmap, 2 * YT_COLS * c, k * N + box * YT_BOX_ROWS, T + (size_t)box * YT_BOX_ROWS * YT_COLS);
-            tma_store_commit();
+                tma_store_commit();             // one bulk group per box
+            }
         }
         b ^= 1;
     }
