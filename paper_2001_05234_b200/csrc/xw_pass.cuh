@@ -101,7 +101,7 @@ struct XWPass {
         // global memory as coalesced 16-byte loads, UB column pairs per lane in flight at a time
         const size_t plane = (size_t)a.nx * a.ny;
         constexpr int NQ = H / 32;                       // column pairs per lane
-        constexpr int UB = DIV ? 2 : (NQ < 16 ? NQ : 16);
+        constexpr int UB = DIV ? 4 : (NQ < 16 ? NQ : 16);
         cplx v[R1];
         const bool direct = !DIV && a.kind == KIND_PP;   // periodic rows of a stored field: no staging needed
         if (direct) {
