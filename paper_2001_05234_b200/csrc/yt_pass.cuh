@@ -153,8 +153,11 @@ struct YTPass {
                 r0 = make_double2(A0, B0);
                 r1 = make_double2(A1, B1);
             }
-            t[at(2 * s, f)] = r0;
-            t[at(2 * s + 1, f)] = r1;
+            // rows 2s and 2s+1: lanes 0-3 of every group of eight write the even row first and lanes 4-7 the odd
+            // one, so that the eight rows of one store instruction differ modulo 8 (conflict free under the swizzle)
+            const bool odd_first = (lane & 4) != 0;
+            t[at(2 * s + (odd_first ? 1 : 0), f)] = odd_first ? r1 : r0;
+            t[at(2 * s + (odd_first ? 0 : 1), f)] = odd_first ? r0 : r1;
         }
         __syncwarp();
     }
@@ -165,8 +168,11 @@ struct YTPass {
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
-            r0[m] = t[at(2 * s, f)];
-            r1[m] = t[at(2 * s + 1, f)];
+            const bool odd_first = (lane & 4) != 0;        // as in slots_out: eight different rows modulo 8 per load
+            const cplx x0 = t[at(2 * s + (odd_first ? 1 : 0), f)];
+            const cplx x1 = t[at(2 * s + (odd_first ? 0 : 1), f)];
+            r0[m] = odd_first ? x1 : x0;
+            r1[m] = odd_first ? x0 : x1;
         }
         __syncwarp();
 #pragma unroll
