@@ -269,3 +269,27 @@ def test_warp_level_transform_kernels_every_kind_pair(B, nx, ny, nz):
             for got, refv, sc, nm in ((ud, un, 1.0, "u"), (vd, vn, 1.0, "v"), (wd, wn, 1.0, "w"), (pd, phi, 1e-3, "dt*Phi")):
                 check_field(np_of(got), refv, scale=sc, what=f"projection {nm} {px}/{py}/{pz} {nx}x{ny}x{nz}")
         plan.close()
+
+
+@pytest.mark.parametrize("nx,ny,nz", [(1024, 768, 3), (768, 1024, 3), (512, 512, 17), (256, 128, 18), (48, 96, 33)])
+def test_no_write_outside_the_fields(B, nx, ny, nz):
+    """Every field lives inside a larger allocation whose guard zones (before and after, 1 MiB each) hold a
+    sentinel: no kernel family (warp-level, TMA-fed, 3-pass, z tiles, gradient) may touch them."""
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    bc = (("P", "P"), ("N", "N"), ("N", "N"))
+    n = nx * ny * nz
+    guard = 131072                                     # doubles (1 MiB), keeps the fields 16-byte aligned
+    sentinel = -7.25e300
+    big = [torch.full((n + 2 * guard,), sentinel, dtype=torch.float64, device="cuda") for _ in range(4)]
+    views = [b[guard:guard + n].view(nz, ny, nx) for b in big]
+    g = torch.Generator(device="cuda").manual_seed(5)
+    for v in views[:3]:
+        v.copy_(torch.rand((nz, ny, nx), dtype=torch.float64, device="cuda", generator=g))
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc)
+    plan.projection(views[0], views[1], views[2], views[3], 1e-3)
+    plan.poisson_solve(views[3])
+    torch.cuda.synchronize()
+    plan.close()
+    for b in big:
+        assert bool((b[:guard] == sentinel).all()) and bool((b[guard + n:] == sentinel).all())
+        assert bool(torch.isfinite(b[guard:guard + n]).all())
