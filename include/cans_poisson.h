@@ -89,7 +89,8 @@ int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream);
  *   p        DEVICE, overwritten with Phi (entry contents ignored; eq. 2d is the caller's).
  *   dt       the whole factor gamma_k*Delta_t of eqs. 2b-2c (> 0).
  * The boundary-normal velocity on a lower 'P' face is the wrapped value, on a lower 'N' face 0
- * (or the plane registered with cans_projection_set_lower_face); the value on an upper 'N' face
+ * (or the plane registered with cans_projection_set_lower_face), on a lower 'D' face the registered plane
+ * (required); the value on an upper 'N' face
  * (array index n-1) is read and left bit-identical.
  */
 int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, double* p,
@@ -97,10 +98,14 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
 
 /*
  * cans_projection_set_lower_face -- register the boundary-normal velocity on the LOWER face of
- * direction dir (0,1,2): DEVICE plane of (product of the other two extents) doubles, x fastest,
- * or NULL to unregister.  On a 'D' side the plane is read by the divergence and corrected
- * (-= dt*2*Phi_0/h); on an 'N' side it is a prescribed inflow and is not modified.
- * (Not implemented yet: returns CANS_ERR_UNSUPPORTED_BC for a non-NULL plane.)
+ * direction dir (0,1,2): DEVICE plane of (product of the other two extents) doubles, x fastest among the
+ * remaining indices (dir 0: j + ny*k; dir 1: i + nx*k; dir 2: i + nx*j), 16-byte aligned, or NULL to
+ * unregister.  The library keeps the pointer (caller-owned memory, must outlive its registration).
+ * On a 'D' side the plane is read by the divergence (eq. 2b) and corrected in place by eq. 2c with the
+ * anti-mirrored ghost (-= dt*2*Phi_0/h, h = dx, dy or dzc[0]); without it cans_projection returns
+ * CANS_ERR_NEEDS_FACE, because the projected field would not be divergence free.  On an 'N' side it is a
+ * prescribed inflow, read by the divergence and not modified.  A periodic direction has no lower face:
+ * CANS_ERR_INVALID_ARG.  cans_poisson_solve ignores the planes.
  */
 int cans_projection_set_lower_face(cans_poisson_plan* plan, int dir, double* face_plane);
 

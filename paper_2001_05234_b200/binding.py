@@ -166,7 +166,18 @@ class PoissonPlan:
                                     _stream_ptr(stream)))
 
     def set_lower_face(self, direction: int, plane: Optional[torch.Tensor]):
-        ptr = None if plane is None else plane.data_ptr()
+        """cans_projection_set_lower_face: register (or, with None, unregister) the boundary-normal velocity on the
+        lower face of `direction`: a contiguous float64 CUDA tensor with the field's shape and extent 1 along that
+        direction.  The library keeps the pointer, not the tensor: keep it alive while it is registered."""
+        ptr = None
+        if plane is not None:
+            nz, ny, nx = self.shape
+            want = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}.get(int(direction))
+            if want is None:
+                raise ValueError("direction must be 0, 1 or 2")
+            if plane.dtype != torch.float64 or not plane.is_cuda or not plane.is_contiguous() or tuple(plane.shape) != want:
+                raise ValueError(f"lower-face plane must be a contiguous float64 CUDA tensor of shape {want}")
+            ptr = plane.data_ptr()
         _check(_lib.cans_projection_set_lower_face(self._h, int(direction), ptr))
 
     # --- host-buffer entry points (end-to-end timing) ---------------------------------------------

@@ -90,6 +90,27 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
     }
 }
 
+// Lower boundary face of a direction with a pressure-Dirichlet lower side: the face velocity is an unknown of the
+// projection and takes the correction of eq. 2c with the anti-mirrored ghost, face -= dt (Phi_0 - (-Phi_0)) / h.
+// Generic over the direction: the plane has n0 x n1 entries (n0 fastest), Phi_0 of entry (a0, a1) sits at
+// phi[a0 * s0 + a1 * s1].
+struct FaceArgs {
+    double* face;
+    const double* phi;
+    int n0, n1;
+    size_t s0, s1;
+    double dt, h;
+};
+
+__global__ void __launch_bounds__(256) face_correct_kernel(const FaceArgs a) {
+    const size_t n = (size_t)a.n0 * a.n1;
+    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        const size_t a1 = t / a.n0, a0 = t - a1 * a.n0;
+        const double first = a.phi[a0 * a.s0 + a1 * a.s1];
+        a.face[t] -= a.dt * (first + first) / a.h;
+    }
+}
+
 bool fused_dispatch(int nx, int ny, int what, const FusedArgs* a, int num_sms, int* grid, size_t* smem,
                     cudaStream_t st, cudaError_t* err) {
     switch (nx) {
@@ -136,13 +157,15 @@ struct cans_poisson_plan {
     int use_yw;
     int use_yt;               // 1: y transforms run the persistent TMA-fed kernels (yt_pass.cuh)
     double inv_lz;
+    double* face[3];          // registered lower-face planes (caller-owned device memory) or NULL
+    double dzc0;              // dzc[0]: distance from the lower z face's ghost centre to the first centre
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
     // optional per-kernel timing (cans_plan_set_profiling): event pair around every launch
     int prof;
     int nrec;
-    cudaEvent_t ev[2 * 8];
-    const char* kname[8];
+    cudaEvent_t ev[2 * 12];
+    const char* kname[12];
 };
 
 // bracket one kernel launch with events when profiling is on
@@ -150,10 +173,10 @@ struct LaunchScope {
     cans_poisson_plan* pl;
     cudaStream_t st;
     LaunchScope(cans_poisson_plan* p, cudaStream_t s, const char* name) : pl(p), st(s) {
-        if (pl->prof && pl->nrec < 8) { pl->kname[pl->nrec] = name; cudaEventRecord(pl->ev[2 * pl->nrec], st); }
+        if (pl->prof && pl->nrec < 12) { pl->kname[pl->nrec] = name; cudaEventRecord(pl->ev[2 * pl->nrec], st); }
     }
     ~LaunchScope() {
-        if (pl->prof && pl->nrec < 8) { cudaEventRecord(pl->ev[2 * pl->nrec + 1], st); pl->nrec++; }
+        if (pl->prof && pl->nrec < 12) { cudaEventRecord(pl->ev[2 * pl->nrec + 1], st); pl->nrec++; }
     }
 };
 
@@ -208,7 +231,7 @@ void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
     if (!plan) return;
     for (void* d : plan->dev_allocs) cudaFree(d);
     for (int i = 0; i < 4; ++i) if (plan->hostbuf[i]) cudaFree(plan->hostbuf[i]);
-    if (plan->prof) for (int i = 0; i < 16; ++i) cudaEventDestroy(plan->ev[i]);
+    if (plan->prof) for (int i = 0; i < 24; ++i) cudaEventDestroy(plan->ev[i]);
     delete plan;
 }
 
@@ -253,6 +276,8 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->kind_x = kx; pl->kind_y = ky;
     pl->nseg = nseg; pl->nzp = nseg * Z_MROWS;
     for (int i = 0; i < 4; ++i) pl->hostbuf[i] = nullptr;
+    for (int i = 0; i < 3; ++i) pl->face[i] = nullptr;
+    pl->dzc0 = hdzc[0];
     pl->prof = 0; pl->nrec = 0;
     pl->fused = 0;
     pl->fused_ok = 0;
@@ -461,7 +486,12 @@ int cans_plan_set_fusion(cans_poisson_plan* plan, int enable) {
 }
 
 int cans_plan_launches_per_solve(const cans_poisson_plan* plan) { return (plan && plan->fused) ? 3 : 5; }
-int cans_plan_launches_per_projection(const cans_poisson_plan* plan) { return (plan && plan->fused) ? 3 : 6; }
+int cans_plan_launches_per_projection(const cans_poisson_plan* plan) {
+    if (!plan) return 6;
+    int n = plan->fused ? 3 : 6;
+    for (int d = 0; d < 3; ++d) n += (plan->bc[d][0] == 'D' && plan->face[d]) ? 1 : 0;   // lower-face corrections
+    return n;
+}
 
 int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream) {
     g_status = CANS_OK;
@@ -478,8 +508,8 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
           reinterpret_cast<size_t>(w)) & 15) != 0)
         return fail(CANS_ERR_INVALID_ARG, "fields must be 16-byte aligned");
     for (int d = 0; d < 3; ++d)
-        if (plan->bc[d][0] == 'D')
-            return fail(CANS_ERR_NEEDS_FACE, "a lower 'D' side needs a registered lower-face plane (not implemented)");
+        if (plan->bc[d][0] == 'D' && !plan->face[d])
+            return fail(CANS_ERR_NEEDS_FACE, "a lower 'D' side needs a lower-face plane (cans_projection_set_lower_face)");
     cudaStream_t st = (cudaStream_t)stream;
     XYArgs a = make_xyargs(plan, p, true);
     a.u = u; a.v = v; a.w = w;
@@ -490,6 +520,7 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     a.wrap_x = plan->bc[0][0] == 'P';
     a.wrap_y = plan->bc[1][0] == 'P';
     a.wrap_z = plan->bc[2][0] == 'P';
+    a.fx = plan->face[0]; a.fy = plan->face[1]; a.fz = plan->face[2];
     GradArgs g;
     g.nx = plan->nx; g.ny = plan->ny; g.nz = plan->nz;
     g.u = u; g.v = v; g.w = w; g.phi = p;
@@ -505,20 +536,39 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     ghost(plan->bc[0][1], plan->nx, &g.gx_idx, &g.gx_sgn);
     ghost(plan->bc[1][1], plan->ny, &g.gy_idx, &g.gy_sgn);
     ghost(plan->bc[2][1], plan->nz, &g.gz_idx, &g.gz_sgn);
-    return run_core(plan, p, &a, &g, st);
+    int rc = run_core(plan, p, &a, &g, st);
+    if (rc) return rc;
+    // a7 on the registered lower faces of pressure-Dirichlet sides (planes on 'N' sides are prescribed inflow)
+    const int nx = plan->nx, ny = plan->ny, nz = plan->nz;
+    for (int d = 0; d < 3; ++d) {
+        if (plan->bc[d][0] != 'D') continue;
+        FaceArgs fa;
+        fa.face = plan->face[d];
+        fa.phi = p;
+        fa.dt = dt;
+        if (d == 0) { fa.n0 = ny; fa.n1 = nz; fa.s0 = (size_t)nx; fa.s1 = (size_t)nx * ny; fa.h = plan->lx / nx; }
+        else if (d == 1) { fa.n0 = nx; fa.n1 = nz; fa.s0 = 1; fa.s1 = (size_t)nx * ny; fa.h = plan->ly / ny; }
+        else { fa.n0 = nx; fa.n1 = ny; fa.s0 = 1; fa.s1 = (size_t)nx; fa.h = plan->dzc0; }
+        const size_t n = (size_t)fa.n0 * fa.n1;
+        LaunchScope scope(plan, st, "face_correct");
+        face_correct_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(fa);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return fail_cuda(e, "lower-face correction launch");
+    }
+    return CANS_OK;
 }
 
 int cans_plan_set_profiling(cans_poisson_plan* plan, int enable) {
     g_status = CANS_OK;
     if (!plan) return fail(CANS_ERR_INVALID_ARG, "plan is NULL");
     if (enable && !plan->prof) {
-        for (int i = 0; i < 16; ++i) {
+        for (int i = 0; i < 24; ++i) {
             cudaError_t e = cudaEventCreate(&plan->ev[i]);
             if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
         }
         plan->prof = 1;
     } else if (!enable && plan->prof) {
-        for (int i = 0; i < 16; ++i) cudaEventDestroy(plan->ev[i]);
+        for (int i = 0; i < 24; ++i) cudaEventDestroy(plan->ev[i]);
         plan->prof = 0;
     }
     plan->nrec = 0;
@@ -546,7 +596,13 @@ const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx) {
 int cans_projection_set_lower_face(cans_poisson_plan* plan, int dir, double* face_plane) {
     g_status = CANS_OK;
     if (!plan || dir < 0 || dir > 2) return fail(CANS_ERR_INVALID_ARG, "bad plan or direction");
-    if (face_plane) return fail(CANS_ERR_UNSUPPORTED_BC, "lower-face planes are not implemented yet");
+    if (face_plane) {
+        if (plan->bc[dir][0] == 'P')
+            return fail(CANS_ERR_INVALID_ARG, "a periodic direction has no lower boundary face (it is the wrapped value)");
+        if ((reinterpret_cast<size_t>(face_plane) & 15) != 0)
+            return fail(CANS_ERR_INVALID_ARG, "the face plane must be 16-byte aligned");
+    }
+    plan->face[dir] = face_plane;
     return CANS_OK;
 }
 

@@ -135,11 +135,13 @@ struct XWPass {
                     if (lane == 0) {
                         if (i0 > 0) { ula0[u] = a.u[ro + i0 - 1]; ulb0[u] = a.u[ro + a.nx + i0 - 1]; }
                         else if (a.wrap_x) { ula0[u] = a.u[ro + a.nx - 1]; ulb0[u] = a.u[ro + 2 * (size_t)a.nx - 1]; }
+                        else if (a.fx) { ula0[u] = a.fx[(size_t)k * a.ny + j]; ulb0[u] = a.fx[(size_t)k * a.ny + j + 1]; }
                     }
                     v1[u] = *reinterpret_cast<const double2*>(a.v + ro + i0);
                     v2[u] = *reinterpret_cast<const double2*>(a.v + ro + a.nx + i0);
                     if (j > 0) v0[u] = *reinterpret_cast<const double2*>(a.v + ro - a.nx + i0);
                     else if (a.wrap_y) v0[u] = *reinterpret_cast<const double2*>(a.v + ro + (size_t)(a.ny - 1) * a.nx + i0);
+                    else if (a.fy) v0[u] = *reinterpret_cast<const double2*>(a.fy + (size_t)k * a.nx + i0);
                     else v0[u] = zero2;
                     wa[u] = *reinterpret_cast<const double2*>(a.w + ro + i0);
                     wb[u] = *reinterpret_cast<const double2*>(a.w + ro + a.nx + i0);
@@ -149,6 +151,9 @@ struct XWPass {
                     } else if (a.wrap_z) {
                         wla[u] = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + i0);
                         wlb[u] = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + a.nx + i0);
+                    } else if (a.fz) {
+                        wla[u] = *reinterpret_cast<const double2*>(a.fz + (size_t)j * a.nx + i0);
+                        wlb[u] = *reinterpret_cast<const double2*>(a.fz + (size_t)(j + 1) * a.nx + i0);
                     } else { wla[u] = zero2; wlb[u] = zero2; }
                 }
                 const double rz = a.rdzf[k];

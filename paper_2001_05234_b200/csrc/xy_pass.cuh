@@ -34,7 +34,12 @@ struct XYArgs {
     const double* w;
     const double* rdzf;     // 1/dzf[k]
     double rdx, rdy, rdt;
-    int wrap_x, wrap_y, wrap_z;   // 1 if that direction is periodic (lower face = wrapped value), else 0 (=> 0)
+    int wrap_x, wrap_y, wrap_z;   // 1 if that direction is periodic (lower face = wrapped value), else 0
+    // boundary-normal velocity on the lower face of a non-periodic direction (cans_projection_set_lower_face), or
+    // NULL (=> 0, no penetration): fx[j + ny*k], fy[i + nx*k], fz[i + nx*j]
+    const double* fx;
+    const double* fy;
+    const double* fz;
 };
 
 // natural index i of a line  ->  FFT input element (and whether the sample is negated)
@@ -123,6 +128,7 @@ struct XPass {
             double ula, ulb;
             if (i0 > 0) { ula = a.u[ro + i0 - 1]; ulb = a.u[ro + a.nx + i0 - 1]; }
             else if (a.wrap_x) { ula = a.u[ro + a.nx - 1]; ulb = a.u[ro + 2 * (size_t)a.nx - 1]; }
+            else if (a.fx) { ula = a.fx[(size_t)k * a.ny + j]; ulb = a.fx[(size_t)k * a.ny + j + 1]; }
             else { ula = 0.0; ulb = 0.0; }
             // v: rows j-1, j, j+1
             const double2 v1 = *reinterpret_cast<const double2*>(a.v + ro + i0);
@@ -130,6 +136,7 @@ struct XPass {
             double2 v0;
             if (j > 0) v0 = *reinterpret_cast<const double2*>(a.v + ro - a.nx + i0);
             else if (a.wrap_y) v0 = *reinterpret_cast<const double2*>(a.v + ro + (size_t)(a.ny - 1) * a.nx + i0);
+            else if (a.fy) v0 = *reinterpret_cast<const double2*>(a.fy + (size_t)k * a.nx + i0);
             else v0 = make_double2(0.0, 0.0);
             // w: planes k-1, k
             const double2 wa = *reinterpret_cast<const double2*>(a.w + ro + i0);
@@ -141,6 +148,9 @@ struct XPass {
             } else if (a.wrap_z) {
                 wla = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + i0);
                 wlb = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + a.nx + i0);
+            } else if (a.fz) {
+                wla = *reinterpret_cast<const double2*>(a.fz + (size_t)j * a.nx + i0);
+                wlb = *reinterpret_cast<const double2*>(a.fz + (size_t)(j + 1) * a.nx + i0);
             } else { wla = make_double2(0.0, 0.0); wlb = wla; }
             const double rz = a.rdzf[k];
             va.x = div_value(ua.x - ula, v1.x - v0.x, wa.x - wla.x, a.rdx, a.rdy, rz, a.rdt);

@@ -293,3 +293,63 @@ def test_no_write_outside_the_fields(B, nx, ny, nz):
     for b in big:
         assert bool((b[:guard] == sentinel).all()) and bool((b[guard + n:] == sentinel).all())
         assert bool(torch.isfinite(b[guard:guard + n]).all())
+
+
+@pytest.mark.parametrize("nx,ny,nz", [(96, 64, 20), (512, 512, 5), (1024, 768, 3)])
+@pytest.mark.parametrize("px,py,pz,inflow", [("DD", "PP", "NN", None), ("PP", "DD", "NN", None), ("NN", "NN", "DN", None),
+                                              ("DD", "DD", "DD", None), ("NN", "PP", "ND", 0), ("PP", "NN", "ND", 1)])
+def test_projection_with_lower_face_planes(B, nx, ny, nz, px, py, pz, inflow):
+    """Lower 'D' sides carry a registered face plane that the divergence reads and eq. 2c corrects; a plane on a lower
+    'N' side is a prescribed inflow.  Fields and planes against the oracle; the result is divergence free."""
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+    rng = np.random.default_rng(nx + 7 * nz)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+    faces = {d: rng.standard_normal(shapes[d]) for d, pr in enumerate((px, py, pz)) if pr[0] == "D"}
+    if inflow is not None:
+        faces[inflow] = rng.standard_normal(shapes[inflow])
+    dt = 1e-3
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+    pd = torch.empty_like(ud)
+    fd = {d: torch.from_numpy(f).cuda() for d, f in faces.items()}
+    for d, t in fd.items():
+        plan.set_lower_face(d, t)
+    assert plan.launches_per_projection == 6 + sum(1 for d in fd if bc[d][0] == "D")
+    plan.projection(ud, vd, wd, pd, dt)
+    torch.cuda.synchronize()
+    un, vn, wn, phi, fn = orc.projection(u, v, w, dt, lx, ly, lz, bc, dzc, dzf, faces)
+    check_field(np_of(ud), un, what="u")
+    check_field(np_of(vd), vn, what="v")
+    check_field(np_of(wd), wn, what="w")
+    check_field(np_of(pd), phi, scale=dt, what="dt*Phi")
+    got_faces = {d: np_of(t) for d, t in fd.items()}
+    for d in fd:
+        check_field(got_faces[d], fn[d], what=f"face {d}")
+        if bc[d][0] == "N":
+            assert np.array_equal(got_faces[d], faces[d])        # prescribed inflow: untouched
+    div = orc.divergence(np_of(ud), np_of(vd), np_of(wd), lx, ly, lz, bc, dzc, dzf, got_faces)
+    assert np.max(np.abs(div)) < 1e-10 * max(np.max(np.abs(u)), 1.0) / min(lx / nx, ly / ny, dzf.min())
+    # unregistering brings CANS_ERR_NEEDS_FACE back for 'D' sides
+    d_sides = [d for d in fd if bc[d][0] == "D"]
+    if d_sides:
+        plan.set_lower_face(d_sides[0], None)
+        with pytest.raises(B.CansError) as ei:
+            plan.projection(ud, vd, wd, pd, dt)
+        assert ei.value.status == B.CANS_ERR_NEEDS_FACE
+    plan.close()
+
+
+def test_lower_face_argument_checks(B):
+    plan = B.PoissonPlan(32, 32, 16, 1.0, 1.0, 1.0, (("P", "P"), ("N", "N"), ("D", "N")))
+    with pytest.raises(B.CansError) as ei:
+        plan.set_lower_face(0, torch.zeros((16, 32, 1), dtype=torch.float64, device="cuda"))    # periodic direction
+    assert ei.value.status == B.CANS_ERR_INVALID_ARG
+    with pytest.raises(ValueError):
+        plan.set_lower_face(2, torch.zeros((1, 32, 31), dtype=torch.float64, device="cuda"))    # wrong shape
+    plan.set_lower_face(2, torch.zeros((1, 32, 32), dtype=torch.float64, device="cuda"))
+    plan.set_lower_face(2, None)
+    plan.close()
