@@ -203,8 +203,8 @@ def time_poisson_config(binding, workloads, torch, name, steps=10, warmup=3):
 
 def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
     """Every supported boundary-condition combination on the C5 grid (BASELINE.json: "for every supported
-    boundary-condition combination"): Poisson solve for {PP,NN,DD}^2 x {NN,DN,ND,DD}; projection step for the
-    combinations without a lower 'D' side ({PP,NN}^2 x {NN,ND}).  Median ms per call, CUDA events."""
+    boundary-condition combination"): Poisson solve and projection step for {PP,NN,DD}^2 x {NN,DN,ND,DD}
+    (lower 'D' sides with a registered face plane).  Median ms per call, CUDA events."""
     w = workloads.make_workload("C5", device="cuda", with_fields=False)
     nx, ny, nz = w.n
     lx, ly, lz = w.lengths
@@ -229,12 +229,18 @@ def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
                 plan = binding.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, w.dzc, w.dzf)
                 key = f"{px}/{py}/{pz}"
                 out["poisson_ms"][key] = med(lambda: plan.poisson_solve(bufs[3]), lambda: bufs[3].copy_(f))
-                if px != "DD" and py != "DD" and pz[0] == "N":
-                    def reset():
-                        for b in bufs[:3]:
-                            b.copy_(f)
-                    out["projection_ms"][key] = med(
-                        lambda: plan.projection(bufs[0], bufs[1], bufs[2], bufs[3], 1e-4), reset)
+                # lower 'D' sides carry a registered face plane (kept alive in `planes` while registered)
+                shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+                planes = {d: torch.zeros(shapes[d], dtype=torch.float64, device="cuda")
+                          for d, pr in enumerate((px, py, pz)) if pr[0] == "D"}
+                for d, t in planes.items():
+                    plan.set_lower_face(d, t)
+
+                def reset():
+                    for b in bufs[:3]:
+                        b.copy_(f)
+                out["projection_ms"][key] = med(
+                    lambda: plan.projection(bufs[0], bufs[1], bufs[2], bufs[3], 1e-4), reset)
                 plan.close()
     pv, jv = list(out["poisson_ms"].values()), list(out["projection_ms"].values())
     out["poisson_ms_min_max"] = [min(pv), max(pv)]
