@@ -76,11 +76,12 @@ struct ZState {
     bool active;
 };
 
-// shared memory (doubles): tables az,bz,cz,gz [4][nzp]; scan arrays end[TC*P], fac[TC*P];
+// shared memory (doubles): tables az,bz,cz,gz [4][nzp]; scan arrays end[TC*P], fac[TC*P] of the forward sweep and a
+// second pair for the backward sweep (so that no barrier is needed between reading one and writing the other);
 // two tile buffers [nzp][TC]
 template <int MROWS, int TC>
 struct ZPass {
-    static CANS_HD size_t table_doubles(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)2 * TC * nseg; }
+    static CANS_HD size_t table_doubles(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)4 * TC * nseg; }
     static CANS_HD size_t tile_doubles(int nseg) { return (size_t)nseg * MROWS * TC; }
     static CANS_HD size_t smem_doubles(int nseg) { return table_doubles(nseg) + 2 * tile_doubles(nseg); }
 
@@ -147,12 +148,12 @@ struct ZPass {
         for (int q = 0; q < s; ++q) D = s_end[q * TC + c] + s_fac[q * TC + c] * D;
         st.start = D;
     }
-    // (a barrier separates 2a and 2b because 2b overwrites the scan arrays)
+    // (2b publishes into the backward pair of scan arrays, so 2a and 2b need no barrier between them)
     static CANS_HD void phase2b(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
         const double* scz = sm + 2 * nzp;
-        double* s_end = sm + 4 * nzp;
+        double* s_end = sm + 4 * nzp + 2 * TC * a.nseg;      // backward pair
         double* s_fac = s_end + TC * a.nseg;
         const int c = tid % TC;
         const int s = tid / TC;
@@ -185,7 +186,7 @@ struct ZPass {
     static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
         const int nzp = a.nseg * MROWS;
         const double* scz = sm + 2 * nzp;
-        const double* s_end = sm + 4 * nzp;
+        const double* s_end = sm + 4 * nzp + 2 * TC * a.nseg;   // backward pair
         const double* s_fac = s_end + TC * a.nseg;
         const int c = tid % TC;
         const int s = tid / TC;

@@ -81,7 +81,6 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
         // every thread has read s_next (before the barrier above): thread 0 may now draw the ticket after next
         if (tid == 0 && nxt < a.ntiles) s_next = (long)atomicAdd(a.ticket, 1u);
         Z::phase2a(a, zsm, st, tid);
-        __syncthreads();
         Z::phase2b(a, zsm, st, tid);
         __syncthreads();
         Z::phase3(a, zsm, st, tid);
