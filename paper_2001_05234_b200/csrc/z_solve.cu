@@ -67,8 +67,10 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
     };
     double rs, l1, l2;
     tile_scalars(cur, rs, l1, l2);
+    __syncthreads();                           // the first s_next is visible
     while (true) {
-        __syncthreads();                       // s_next visible; buffer b^1 no longer read by anyone
+        // No barrier here: s_next was rewritten behind the phase-1 barrier of the previous tile and published by
+        // its phase-2 barrier; buffer b^1 was last read in that tile's phase 1, also behind that barrier.
         const long nxt = s_next;
         if (tid == 0 && nxt < a.ntiles) issue_tile(nxt, b ^ 1);
         double rs_n, l1_n, l2_n;
