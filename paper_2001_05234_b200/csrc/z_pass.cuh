@@ -103,8 +103,7 @@ struct ZPass {
         const double* saz = sm;
         const double* sbz = sm + nzp;
         const double* sgz = sm + 3 * nzp;
-        double* s_end = sm + 4 * nzp;
-        double* s_fac = s_end + TC * a.nseg;
+        double2* s_scan = reinterpret_cast<double2*>(sm + 4 * nzp);      // forward (end, factor) pairs
         const int c = tid % TC;
         const int s = tid / TC;
         const long col = tile * TC + c;
@@ -129,23 +128,24 @@ struct ZPass {
                 st.d[r] = dp;
                 fac *= -e;
             }
-            s_end[s * TC + c] = dp;
-            s_fac[s * TC + c] = fac;
+            s_scan[s * TC + c] = make_double2(dp, fac);
         } else {
-            s_end[s * TC + c] = 0.0;
-            s_fac[s * TC + c] = 0.0;
+            s_scan[s * TC + c] = make_double2(0.0, 0.0);
         }
     }
 
     // phase 2: scan the segment ends -> true start; propagate; local backward sweep from a zero start; publish
     static CANS_HD void phase2a(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
         const int nzp = a.nseg * MROWS;
-        const double* s_end = sm + 4 * nzp;
-        const double* s_fac = s_end + TC * a.nseg;
+        const double2* s_scan = reinterpret_cast<const double2*>(sm + 4 * nzp);
         const int c = tid % TC;
         const int s = tid / TC;
         double D = 0.0;                     // true d' at the end of segment s'-1
-        for (int q = 0; q < s; ++q) D = s_end[q * TC + c] + s_fac[q * TC + c] * D;
+#pragma unroll 4
+        for (int q = 0; q < s; ++q) {
+            const double2 ef = s_scan[q * TC + c];      // one 16-byte load per segment
+            D = ef.x + ef.y * D;
+        }
         st.start = D;
     }
     // (2b publishes into the backward pair of scan arrays, so 2a and 2b need no barrier between them)
@@ -153,8 +153,7 @@ struct ZPass {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
         const double* scz = sm + 2 * nzp;
-        double* s_end = sm + 4 * nzp + 2 * TC * a.nseg;      // backward pair
-        double* s_fac = s_end + TC * a.nseg;
+        double2* s_scan = reinterpret_cast<double2*>(sm + 4 * nzp + 2 * TC * a.nseg);   // backward pairs
         const int c = tid % TC;
         const int s = tid / TC;
         const int k0 = s * MROWS;
@@ -174,11 +173,9 @@ struct ZPass {
                 st.d[r] = xs;
                 g *= -cp;
             }
-            s_end[s * TC + c] = xs;     // x^0 at the top row of the segment
-            s_fac[s * TC + c] = g;
+            s_scan[s * TC + c] = make_double2(xs, g);     // x^0 at the top row of the segment, its factor
         } else {
-            s_end[s * TC + c] = 0.0;
-            s_fac[s * TC + c] = 0.0;
+            s_scan[s * TC + c] = make_double2(0.0, 0.0);
         }
     }
 
@@ -186,13 +183,16 @@ struct ZPass {
     static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
         const int nzp = a.nseg * MROWS;
         const double* scz = sm + 2 * nzp;
-        const double* s_end = sm + 4 * nzp + 2 * TC * a.nseg;   // backward pair
-        const double* s_fac = s_end + TC * a.nseg;
+        const double2* s_scan = reinterpret_cast<const double2*>(sm + 4 * nzp + 2 * TC * a.nseg);   // backward pairs
         const int c = tid % TC;
         const int s = tid / TC;
         const int k0 = s * MROWS;
         double X = 0.0;                     // true x at the top row of segment s'+1
-        for (int q = a.nseg - 1; q > s; --q) X = s_end[q * TC + c] + s_fac[q * TC + c] * X;
+#pragma unroll 4
+        for (int q = a.nseg - 1; q > s; --q) {
+            const double2 ef = s_scan[q * TC + c];
+            X = ef.x + ef.y * X;
+        }
         if (st.active) {
             const size_t plane = (size_t)a.ncols;
             double g = 1.0;
