@@ -73,9 +73,4 @@ CANS_HD void grad_apply(const GradArgs& a, const GradIn& in) {
     *reinterpret_cast<double2*>(a.w + in.o) = ww;
 }
 
-CANS_HD void grad_correct_pair(const GradArgs& a, size_t t) {
-    const GradIn in = grad_load(a, t);
-    grad_apply(a, in);
-}
-
 }  // namespace cans

@@ -39,9 +39,8 @@ CANS_D void tma_store_2d(const CUtensorMap* tmap, int c0, int c1, const void* sr
                  ::"l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(src)) : "memory");
 }
 CANS_D void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;\n" ::: "memory"); }
-// wait until the bulk stores of this thread have finished READING shared memory (the buffer may be reused)
-CANS_D void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;\n" ::: "memory"); }
-// the same, allowing the PENDING most recent groups to be still reading
+// wait until the bulk stores of this thread have finished READING shared memory (the buffer may be reused),
+// allowing the PENDING most recent groups to be still reading
 template <int PENDING>
 CANS_D void tma_store_wait_read_pending() { asm volatile("cp.async.bulk.wait_group.read %0;\n" ::"n"(PENDING) : "memory"); }
 CANS_D void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;\n" ::: "memory"); }
