@@ -353,3 +353,24 @@ def test_lower_face_argument_checks(B):
     plan.set_lower_face(2, torch.zeros((1, 32, 32), dtype=torch.float64, device="cuda"))
     plan.set_lower_face(2, None)
     plan.close()
+
+
+@pytest.mark.parametrize("nz", [1024, 1000, 513])
+def test_tallest_columns(B, nz):
+    """nz up to the documented maximum (64 z segments, tiles of 8 columns, four TMA boxes per tile) and ragged heights."""
+    nx, ny = 48, 32
+    lx, ly, lz = 1.0, 1.0, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.8)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    for bc in ((("P", "P"), ("P", "P"), ("N", "N")), (("N", "N"), ("D", "D"), ("D", "N"))):
+        f = random_rhs(nx, ny, nz, bc, dzf, nz)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        torch.cuda.synchronize()
+        plan.close()
+        ref = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        check_field(np_of(p), ref, what=f"nz={nz} {bc}")
+    with pytest.raises(B.CansError) as ei:
+        B.PoissonPlan(nx, ny, 1025, lx, ly, lz, bc)
+    assert ei.value.status == B.CANS_ERR_UNSUPPORTED_SIZE
