@@ -21,6 +21,7 @@ CANS_ERR_UNSUPPORTED_SIZE = 3
 CANS_ERR_ALLOC = 4
 CANS_ERR_CUDA = 5
 CANS_ERR_NEEDS_FACE = 6
+MAX_KERNEL_RECORDS = 16      # CANS_MAX_KERNEL_RECORDS of the header
 
 EXPORTED_SYMBOLS = (
     "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
@@ -28,7 +29,7 @@ EXPORTED_SYMBOLS = (
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
     "cans_plan_set_profiling", "cans_plan_kernel_times", "cans_plan_kernel_name",
-    "cans_plan_set_fusion",
+    "cans_plan_set_batch",
 )
 
 
@@ -69,8 +70,8 @@ def _load() -> ctypes.CDLL:
     lib.cans_plan_launches_per_projection.argtypes = [vp]
     lib.cans_plan_set_profiling.restype = i32
     lib.cans_plan_set_profiling.argtypes = [vp, i32]
-    lib.cans_plan_set_fusion.restype = i32
-    lib.cans_plan_set_fusion.argtypes = [vp, i32]
+    lib.cans_plan_set_batch.restype = i32
+    lib.cans_plan_set_batch.argtypes = [vp, i32]
     lib.cans_plan_kernel_times.restype = i32
     lib.cans_plan_kernel_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32]
     lib.cans_plan_kernel_name.restype = ctypes.c_char_p
@@ -192,14 +193,14 @@ class PoissonPlan:
     def set_profiling(self, enable: bool):
         _check(_lib.cans_plan_set_profiling(self._h, 1 if enable else 0))
 
-    def set_fusion(self, enable: bool) -> bool:
-        """Select the fused (3 launches) or unfused launch sequence; returns the resulting state."""
-        return bool(_lib.cans_plan_set_fusion(self._h, 1 if enable else 0))
+    def set_batch(self, planes: int) -> int:
+        """cans_plan_set_batch: planes per launch of the x / y / correction kernels (0: all planes in one launch)."""
+        return int(_lib.cans_plan_set_batch(self._h, int(planes)))
 
     def kernel_times(self):
         """[(kernel name, ms)] of the last call, in launch order (profiling must be enabled)."""
-        buf = (ctypes.c_float * 8)()
-        n = _lib.cans_plan_kernel_times(self._h, buf, 8)
+        buf = (ctypes.c_float * MAX_KERNEL_RECORDS)()
+        n = _lib.cans_plan_kernel_times(self._h, buf, MAX_KERNEL_RECORDS)
         if n < 0:
             raise CansError(_lib.cans_last_status(), last_error())
         return [(_lib.cans_plan_kernel_name(self._h, i).decode(), float(buf[i])) for i in range(n)]

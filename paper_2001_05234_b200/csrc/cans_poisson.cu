@@ -9,7 +9,9 @@
 //   a6     xw_kernel<inv>      / x_pass_kernel
 //   a7     grad_correct_kernel                   u -= dt G Phi
 // (xw / yw: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
-//  FFTs for the other lengths.)  Opt-in: the fused persistent passes of fused_pass.cuh.
+//  FFTs for the other lengths.)
+// Plane-batched sequence (cans_plan_set_batch): the same kernels launched per batch of consecutive k-planes, x then y
+// (pass A) and y, x, gradient (pass C), so that the intermediate planes stay in L2 between the launches.
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -24,7 +26,6 @@
 #include "xy_kernels.cuh"
 #include "z_kernels.cuh"
 #include "grad_pass.cuh"
-#include "fused_kernels.cuh"
 #include "xw_kernels.cuh"
 #include "yw_kernels.cuh"
 #include "yt_kernels.cuh"
@@ -57,8 +58,8 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
     const size_t cols = (size_t)hx * a.ny;
     const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= cols) return;
-    const int k0 = (int)blockIdx.y * GRAD_KC;
-    const int k1 = (k0 + GRAD_KC < a.nz) ? k0 + GRAD_KC : a.nz;
+    const int k0 = a.k0 + (int)blockIdx.y * GRAD_KC;
+    const int k1 = (k0 + GRAD_KC < a.k1) ? k0 + GRAD_KC : a.k1;
     const int i = 2 * (int)(c % hx);
     const int j = (int)(c / hx);
     const size_t plane = (size_t)a.nx * a.ny;
@@ -111,18 +112,6 @@ __global__ void __launch_bounds__(256) face_correct_kernel(const FaceArgs a) {
     }
 }
 
-bool fused_dispatch(int nx, int ny, int what, const FusedArgs* a, int num_sms, int* grid, size_t* smem,
-                    cudaStream_t st, cudaError_t* err) {
-    switch (nx) {
-        case 256: return fused_dispatch_256(ny, what, a, num_sms, grid, smem, st, err);
-        case 384: return fused_dispatch_384(ny, what, a, num_sms, grid, smem, st, err);
-        case 512: return fused_dispatch_512(ny, what, a, num_sms, grid, smem, st, err);
-        case 768: return fused_dispatch_768(ny, what, a, num_sms, grid, smem, st, err);
-        case 1024: return fused_dispatch_1024(ny, what, a, num_sms, grid, smem, st, err);
-        default: return false;
-    }
-}
-
 }  // namespace cans
 
 using namespace cans;
@@ -130,6 +119,8 @@ using namespace cans;
 // ------------------------------------------------------------------------------------------------
 // the plan
 // ------------------------------------------------------------------------------------------------
+constexpr int MAX_REC = CANS_MAX_KERNEL_RECORDS;
+
 struct cans_poisson_plan {
     int nx, ny, nz;
     double lx, ly, lz;
@@ -137,15 +128,12 @@ struct cans_poisson_plan {
     int kind_x, kind_y;
     int singular;
     int nseg, nzp;
+    int device;               // the device the plan was created on (tables, kernel attributes)
     int num_sms;
     int z_grid;               // persistent grid of the z solve
     size_t z_smem;
-    // fused passes A / C (fused_pass.cuh): persistent grid, ticket tables
-    int fused;                // 1: (nx, ny) has fused kernels and fusion is enabled
-    int fused_ok;             // 1: (nx, ny) has fused kernels
-    int fused_grid;
-    size_t fused_smem;
-    unsigned int* sched;      // scheduler state (tickets, per-plane counters), zeroed at the start of every call
+    int batch;                // planes per launch of the x / y / gradient kernels; 0: one launch per step over all planes
+    unsigned int* sched;      // scheduler state (z tile ticket), zeroed at the start of every call
     size_t sched_bytes;
     std::vector<void*> dev_allocs;
     // device tables
@@ -156,27 +144,33 @@ struct cans_poisson_plan {
     cplx* tw2_y;              // the same for ny (yw_pass.cuh), or NULL
     int use_yw;
     int use_yt;               // 1: y transforms run the persistent TMA-fed kernels (yt_pass.cuh)
+    // TMA descriptors of the field the last call worked on: encoded on the host only when the pointer changes
+    const double* tmap_field;
+    CUtensorMap tmap_y, tmap_z;
     double inv_lz;
     double* face[3];          // registered lower-face planes (caller-owned device memory) or NULL
     double dzc0;              // dzc[0]: distance from the lower z face's ghost centre to the first centre
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
-    // optional per-kernel timing (cans_plan_set_profiling): event pair around every launch
+    // optional timing (cans_plan_set_profiling): an event pair around every kernel launch (one launch per step) or around
+    // every pass (plane-batched sequence)
     int prof;
     int nrec;
-    cudaEvent_t ev[2 * 12];
-    const char* kname[12];
+    cudaEvent_t ev[2 * MAX_REC];
+    const char* kname[MAX_REC];
 };
 
-// bracket one kernel launch with events when profiling is on
+// bracket one kernel launch (or one pass of batched launches) with events when profiling is on
 struct LaunchScope {
     cans_poisson_plan* pl;
     cudaStream_t st;
-    LaunchScope(cans_poisson_plan* p, cudaStream_t s, const char* name) : pl(p), st(s) {
-        if (pl->prof && pl->nrec < 12) { pl->kname[pl->nrec] = name; cudaEventRecord(pl->ev[2 * pl->nrec], st); }
+    bool on;
+    LaunchScope(cans_poisson_plan* p, cudaStream_t s, const char* name, bool enable = true)
+        : pl(p), st(s), on(enable && p->prof && p->nrec < MAX_REC) {
+        if (on) { pl->kname[pl->nrec] = name; cudaEventRecord(pl->ev[2 * pl->nrec], st); }
     }
     ~LaunchScope() {
-        if (pl->prof && pl->nrec < 12) { cudaEventRecord(pl->ev[2 * pl->nrec + 1], st); pl->nrec++; }
+        if (on) { cudaEventRecord(pl->ev[2 * pl->nrec + 1], st); pl->nrec++; }
     }
 };
 
@@ -199,7 +193,7 @@ static cudaError_t upload(cans_poisson_plan* pl, const std::vector<double>& h, T
 }
 
 // layout of the scheduler state (unsigned ints)
-enum { SCHED_Z_TICKET = 0, SCHED_A_TICKET = 1, SCHED_C_TICKET = 2, SCHED_ERR = 3, SCHED_PLANES = 8 };
+enum { SCHED_Z_TICKET = 0, SCHED_WORDS = 8 };
 
 static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
     ZArgs z;
@@ -221,17 +215,65 @@ static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
     return z;
 }
 
+static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
+    XYArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.nx = pl->nx; a.ny = pl->ny; a.nz = pl->nz;
+    a.k0 = 0; a.nk = pl->nz;
+    a.kind = xdir ? pl->kind_x : pl->kind_y;
+    a.tw = xdir ? pl->tw_x : pl->tw_y;
+    a.wpost = xdir ? pl->wpost_x : pl->wpost_y;
+    a.p = p;
+    return a;
+}
+
+static const char* const XY_NAMES[5] = {"x_fwd", "x_fwd_div", "x_inv", "y_fwd", "y_inv"};
+
+// one x / y transform launch over the planes [a.k0, a.k0 + a.nk)
+static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, cudaStream_t st, bool record) {
+    cudaError_t err = cudaSuccess;
+    const bool xdir = (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV);
+    LaunchScope scope(pl, st, XY_NAMES[op], record);
+    bool done = false;
+    if (xdir && pl->use_xw) done = xw_launch(n, op, a, pl->tw2_x, st, &err);
+    else if (!xdir && pl->use_yt) done = yt_launch(n, op, a, pl->tw2_y, &pl->tmap_y, pl->num_sms, st, &err);
+    else if (!xdir && pl->use_yw) done = yw_launch(n, op, a, pl->tw2_y, st, &err);
+    if (!done)
+        done = launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||
+               launch_xy_group_c(n, op, a, st, &err) || launch_xy_group_d(n, op, a, st, &err);
+    if (!done) return fail(CANS_ERR_UNSUPPORTED_SIZE, "transform length not instantiated");
+    if (err != cudaSuccess) return fail_cuda(err, xdir ? "x transform launch" : "y transform launch");
+    return CANS_OK;
+}
+
+// plan time: dynamic shared memory opt-in of every transform kernel this plan can run, on the plan's device
+static cudaError_t configure_kernels(cans_poisson_plan* pl) {
+    const XYArgs dummy = make_xyargs(pl, nullptr, true);
+    cudaError_t e = cudaSuccess;
+    const int lens[2] = {pl->nx, pl->ny};
+    for (int n : lens) {
+        const bool found = launch_xy_group_a(n, OP_CONFIGURE, dummy, 0, &e) || launch_xy_group_b(n, OP_CONFIGURE, dummy, 0, &e) ||
+                           launch_xy_group_c(n, OP_CONFIGURE, dummy, 0, &e) || launch_xy_group_d(n, OP_CONFIGURE, dummy, 0, &e);
+        if (!found) return cudaErrorInvalidValue;
+        if (e != cudaSuccess) return e;
+    }
+    if (pl->use_xw) { xw_launch(pl->nx, OP_CONFIGURE, dummy, pl->tw2_x, 0, &e); if (e != cudaSuccess) return e; }
+    if (pl->use_yw) { yw_launch(pl->ny, OP_CONFIGURE, dummy, pl->tw2_y, 0, &e); if (e != cudaSuccess) return e; }
+    if (pl->use_yt) { yt_launch(pl->ny, OP_CONFIGURE, dummy, pl->tw2_y, nullptr, pl->num_sms, 0, &e); if (e != cudaSuccess) return e; }
+    return e;
+}
+
 extern "C" {
 
 const char* cans_last_error(void) { return g_err.c_str(); }
 int cans_last_status(void) { return g_status; }
-const char* cans_version(void) { return "0.1"; }
+const char* cans_version(void) { return "0.2"; }
 
 void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
     if (!plan) return;
     for (void* d : plan->dev_allocs) cudaFree(d);
     for (int i = 0; i < 4; ++i) if (plan->hostbuf[i]) cudaFree(plan->hostbuf[i]);
-    if (plan->prof) for (int i = 0; i < 24; ++i) cudaEventDestroy(plan->ev[i]);
+    if (plan->prof) for (int i = 0; i < 2 * MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
     delete plan;
 }
 
@@ -279,13 +321,13 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     for (int i = 0; i < 3; ++i) pl->face[i] = nullptr;
     pl->dzc0 = hdzc[0];
     pl->prof = 0; pl->nrec = 0;
-    pl->fused = 0;
-    pl->fused_ok = 0;
+    pl->batch = 0;
+    pl->tmap_field = nullptr;
     pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
-    int dev = 0;
-    cudaGetDevice(&dev);
+    pl->device = 0;
+    cudaGetDevice(&pl->device);
     pl->num_sms = 148;
-    cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, pl->device);
 
     const double dx = lx / nx, dy = ly / ny;
     ZRows zr = make_z_rows(nz, pl->nzp, hdzc.data(), hdzf.data(), bc[2][0], bc[2][1]);
@@ -315,7 +357,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         up(make_two_pass_twiddles(ny), &pl->tw2_y);
         pl->use_yw = 1;
     }
-    pl->use_yt = (pl->use_yw && yt_supported(ny) && std::getenv("CANS_NO_YT") == nullptr) ? 1 : 0;
+    pl->use_yt = (pl->use_yw && yt_supported(ny)) ? 1 : 0;
     if (e == cudaSuccess) {
         void* d = nullptr;
         e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
@@ -327,7 +369,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->r00 = (double*)d; }
     }
     if (e == cudaSuccess) {
-        pl->sched_bytes = sizeof(unsigned int) * (size_t)(SCHED_PLANES + 6 * (nz + 4));
+        pl->sched_bytes = sizeof(unsigned int) * SCHED_WORDS;
         void* d = nullptr;
         e = cudaMalloc(&d, pl->sched_bytes);
         if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->sched = (unsigned int*)d; e = cudaMemset(d, 0, pl->sched_bytes); }
@@ -337,121 +379,48 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         e = z_setup_launch(z, pl->rstart, pl->r00);
     }
     if (e == cudaSuccess) e = z_solve_configure(nseg, nz, pl->num_sms, &pl->z_grid, &pl->z_smem);
-    pl->fused = 0;
-    if (e == cudaSuccess && fused_supported(nx, ny)) {
-        cudaError_t fe = cudaSuccess;
-        if (fused_dispatch(nx, ny, 0, nullptr, pl->num_sms, &pl->fused_grid, &pl->fused_smem, 0, &fe)) e = fe;
-        if (e == cudaSuccess) {
-            pl->fused = 0;        // opt-in (cans_plan_set_fusion): the unfused sequence is currently faster
-            pl->fused_ok = 1;
-        }
-    }
-    if (e != cudaSuccess) {
+    if (e == cudaSuccess) e = configure_kernels(pl);
+    const int rc = CANS_OK;
+    if (e != cudaSuccess || rc != CANS_OK) {
         const bool oom = (e == cudaErrorMemoryAllocation);
-        std::string msg = std::string("plan creation: ") + cudaGetErrorString(e);
+        std::string msg = (rc != CANS_OK) ? g_err : std::string("plan creation: ") + cudaGetErrorString(e);
+        const int code = (rc != CANS_OK) ? rc : (oom ? CANS_ERR_ALLOC : CANS_ERR_CUDA);
         cans_poisson_plan_destroy(pl);
         cudaGetLastError();
-        fail(oom ? CANS_ERR_ALLOC : CANS_ERR_CUDA, msg);
+        fail(code, msg);
         return nullptr;
     }
     return pl;
 }
 
-static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
-    XYArgs a;
-    std::memset(&a, 0, sizeof(a));
-    a.nx = pl->nx; a.ny = pl->ny; a.nz = pl->nz;
-    a.kind = xdir ? pl->kind_x : pl->kind_y;
-    a.tw = xdir ? pl->tw_x : pl->tw_y;
-    a.wpost = xdir ? pl->wpost_x : pl->wpost_y;
-    a.p = p;
-    return a;
-}
-
-static const char* const XY_NAMES[5] = {"x_fwd", "x_fwd_div", "x_inv", "y_fwd", "y_inv"};
-
-static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, cudaStream_t st) {
-    cudaError_t err = cudaSuccess;
-    LaunchScope scope(pl, st, XY_NAMES[op]);
-    if (pl->use_xw && !pl->fused && (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV) &&
-        xw_launch(n, op, a, pl->tw2_x, st, &err)) {
-        if (err != cudaSuccess) return fail_cuda(err, "x transform launch");
-        return CANS_OK;
-    }
-    if (pl->use_yt && !pl->fused && (op == OP_Y_FWD || op == OP_Y_INV) &&
-        yt_launch(n, op, a, pl->tw2_y, pl->num_sms, st, &err)) {
-        if (err != cudaSuccess) return fail_cuda(err, "y transform launch");
-        return CANS_OK;
-    }
-    if (pl->use_yw && !pl->fused && (op == OP_Y_FWD || op == OP_Y_INV) && yw_launch(n, op, a, pl->tw2_y, st, &err)) {
-        if (err != cudaSuccess) return fail_cuda(err, "y transform launch");
-        return CANS_OK;
-    }
-    if (launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||
-        launch_xy_group_c(n, op, a, st, &err) || launch_xy_group_d(n, op, a, st, &err)) {
-        if (err != cudaSuccess) return fail_cuda(err, "x/y transform launch");
-        return CANS_OK;
-    }
-    return fail(CANS_ERR_UNSUPPORTED_SIZE, "transform length not instantiated");
-}
-
 static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
     ZArgs z = make_zargs(pl, p);
     LaunchScope scope(pl, st, "z_solve");
-    cudaError_t e = z_solve_launch(z, pl->z_grid, pl->z_smem, st);
+    cudaError_t e = z_solve_launch(z, pl->z_grid, pl->z_smem, &pl->tmap_z, st);
     if (e != cudaSuccess) return fail_cuda(e, "z solve launch");
     return CANS_OK;
 }
 
-static int launch_fused(cans_poisson_plan* pl, bool inv, double* p, const XYArgs* divargs, const GradArgs* grad,
-                        cudaStream_t st) {
-    FusedArgs f;
-    std::memset(&f, 0, sizeof(f));
-    f.ax = (divargs && !inv) ? *divargs : make_xyargs(pl, p, true);
-    f.ay = make_xyargs(pl, p, false);
-    if (grad) f.g = *grad;
-    const int nx = pl->nx, ny = pl->ny, nz = pl->nz;
-    const unsigned nxt = (unsigned)((ny / 2) / fused_nfx(nx));
-    const unsigned nyt = (unsigned)((nx / 2) / fused_txc(ny));
-    f.cstride = nz + 4;
-    f.grows = FUSED_GROWS;
-    const unsigned ngt = (unsigned)((ny + FUSED_GROWS - 1) / FUSED_GROWS);
-    auto slot = [&](int type, int off, unsigned count) {
-        f.slot_type[f.nslots] = type; f.slot_off[f.nslots] = off; f.slot_count[f.nslots] = count;
-        f.per_round += count;
-        ++f.nslots;
-    };
-    const char* name;
-    int maxoff;
-    if (!inv) {
-        f.counters = pl->sched + SCHED_PLANES;
-        f.ticket = pl->sched + SCHED_A_TICKET;
-        slot(TASK_X, 0, nxt); slot(TASK_Y, 2, nyt); maxoff = 2;
-        f.mode = divargs ? 1 : 0;
-        name = divargs ? "xy_fwd_div" : "xy_fwd";
-    } else {
-        f.counters = pl->sched + SCHED_PLANES + 3 * (nz + 4);
-        f.ticket = pl->sched + SCHED_C_TICKET;
-        slot(TASK_Y, 0, nyt); slot(TASK_X, 2, nxt); maxoff = 2;
-        if (grad) { slot(TASK_G, 5, ngt); maxoff = 5; }
-        name = grad ? "xy_inv_grad" : "xy_inv";
-    }
-    f.total = (unsigned)(nz + maxoff) * f.per_round;
-    LaunchScope scope(pl, st, name);
-    cudaError_t err = cudaSuccess;
-    if (!fused_dispatch(pl->nx, pl->ny, inv ? 2 : 1, &f, pl->num_sms, &pl->fused_grid, &pl->fused_smem, st, &err))
-        return fail(CANS_ERR_UNSUPPORTED_SIZE, "fused kernels not instantiated for this (nx, ny)");
-    if (err != cudaSuccess) return fail_cuda(err, "fused x/y launch");
-    return CANS_OK;
-}
-
-static int launch_grad(cans_poisson_plan* pl, const GradArgs& g, cudaStream_t st) {
+// a7 on the planes [k0, k1)
+static int launch_grad(cans_poisson_plan* pl, GradArgs g, int k0, int k1, cudaStream_t st, bool record) {
+    if (k1 <= k0) return CANS_OK;
+    g.k0 = k0; g.k1 = k1;
     const size_t cols = (size_t)pl->nx / 2 * pl->ny;
-    dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((pl->nz + GRAD_KC - 1) / GRAD_KC));
-    LaunchScope scope(pl, st, "grad_correct");
+    dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((k1 - k0 + GRAD_KC - 1) / GRAD_KC));
+    LaunchScope scope(pl, st, "grad_correct", record);
     grad_correct_kernel<<<grid, 256, 0, st>>>(g);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
+    return CANS_OK;
+}
+
+// TMA descriptors of the field: host-side encode only when the caller passes another buffer than last time
+static int ensure_tensor_maps(cans_poisson_plan* pl, double* p) {
+    if (pl->tmap_field == p) return CANS_OK;
+    cudaError_t e = z_make_tensor_map(&pl->tmap_z, p, (long)pl->nx * pl->ny, pl->nz, pl->nseg);
+    if (e == cudaSuccess && pl->use_yt) e = yt_make_tensor_map(&pl->tmap_y, p, pl->nx, pl->ny, pl->nz);
+    if (e != cudaSuccess) { pl->tmap_field = nullptr; return fail_cuda(e, "tensor map encode"); }
+    pl->tmap_field = p;
     return CANS_OK;
 }
 
@@ -459,37 +428,65 @@ static int launch_grad(cans_poisson_plan* pl, const GradArgs& g, cudaStream_t st
 // `grad` the velocity correction (a7)
 static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st) {
     int rc;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != pl->device)
+        return fail(CANS_ERR_INVALID_ARG, "the plan was created on another device than the current one");
     pl->nrec = 0;
     cudaError_t me = cudaMemsetAsync(pl->sched, 0, pl->sched_bytes, st);
     if (me != cudaSuccess) return fail_cuda(me, "scheduler reset");
-    if (pl->fused) {
-        if ((rc = launch_fused(pl, false, p, divargs, nullptr, st))) return rc;
-        if ((rc = launch_z(pl, p, st))) return rc;
-        return launch_fused(pl, true, p, nullptr, grad, st);
+    if ((rc = ensure_tensor_maps(pl, p))) return rc;
+    const int nz = pl->nz;
+    const int B = (pl->batch > 0 && pl->batch < nz) ? pl->batch : nz;
+    const bool batched = B < nz;
+    XYArgs ax = divargs ? *divargs : make_xyargs(pl, p, true);
+    XYArgs ay = make_xyargs(pl, p, false);
+    const int opx = divargs ? OP_X_FWD_DIV : OP_X_FWD;
+    {   // pass A: (a1 +) a2, a3 per batch of planes
+        LaunchScope scope(pl, st, divargs ? "pass_a_div" : "pass_a", batched);
+        for (int k0 = 0; k0 < nz; k0 += B) {
+            ax.k0 = ay.k0 = k0;
+            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
+            if ((rc = launch_xy_any(pl, pl->nx, opx, ax, st, !batched))) return rc;
+            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, ay, st, !batched))) return rc;
+        }
     }
-    if (divargs) rc = launch_xy_any(pl, pl->nx, OP_X_FWD_DIV, *divargs, st);
-    else rc = launch_xy_any(pl, pl->nx, OP_X_FWD, make_xyargs(pl, p, true), st);
-    if (rc) return rc;
-    if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, make_xyargs(pl, p, false), st))) return rc;
-    if ((rc = launch_z(pl, p, st))) return rc;
-    if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, make_xyargs(pl, p, false), st))) return rc;
-    if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, make_xyargs(pl, p, true), st))) return rc;
-    if (grad) return launch_grad(pl, *grad, st);
+    if ((rc = launch_z(pl, p, st))) return rc;          // pass B: a4
+    {   // pass C: a5, a6 (, a7) per batch of planes; the correction of plane k needs Phi(k+1), so it trails by one plane
+        LaunchScope scope(pl, st, grad ? "pass_c_grad" : "pass_c", batched);
+        ax = make_xyargs(pl, p, true);
+        for (int k0 = 0; k0 < nz; k0 += B) {
+            ax.k0 = ay.k0 = k0;
+            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
+            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, ay, st, !batched))) return rc;
+            if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, ax, st, !batched))) return rc;
+            if (grad && batched) {
+                const int g0 = k0 > 0 ? k0 - 1 : 0;
+                const int g1 = (k0 + ax.nk == nz) ? nz : k0 + ax.nk - 1;
+                if ((rc = launch_grad(pl, *grad, g0, g1, st, false))) return rc;
+            }
+        }
+    }
+    if (grad && !batched) return launch_grad(pl, *grad, 0, nz, st, true);
     return CANS_OK;
 }
 
-int cans_plan_set_fusion(cans_poisson_plan* plan, int enable) {
+int cans_plan_set_batch(cans_poisson_plan* plan, int planes) {
     g_status = CANS_OK;
     if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
-    plan->fused = (enable && plan->fused_ok) ? 1 : 0;
-    return plan->fused;
+    plan->batch = (planes > 0 && planes < plan->nz) ? planes : 0;
+    return plan->batch;
 }
 
-int cans_plan_launches_per_solve(const cans_poisson_plan* plan) { return (plan && plan->fused) ? 3 : 5; }
+static int batches_of(const cans_poisson_plan* plan) {
+    if (!plan || plan->batch <= 0) return 1;
+    return (plan->nz + plan->batch - 1) / plan->batch;
+}
+int cans_plan_launches_per_solve(const cans_poisson_plan* plan) { return 4 * batches_of(plan) + 1; }
 int cans_plan_launches_per_projection(const cans_poisson_plan* plan) {
-    if (!plan) return 6;
-    int n = plan->fused ? 3 : 6;
-    for (int d = 0; d < 3; ++d) n += (plan->bc[d][0] == 'D' && plan->face[d]) ? 1 : 0;   // lower-face corrections
+    const int nb = batches_of(plan);
+    int n = 4 * nb + 1 + (nb > 1 ? nb : 1);
+    if (plan)
+        for (int d = 0; d < 3; ++d) n += (plan->bc[d][0] == 'D' && plan->face[d]) ? 1 : 0;   // lower-face corrections
     return n;
 }
 
@@ -523,6 +520,7 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     a.fx = plan->face[0]; a.fy = plan->face[1]; a.fz = plan->face[2];
     GradArgs g;
     g.nx = plan->nx; g.ny = plan->ny; g.nz = plan->nz;
+    g.k0 = 0; g.k1 = plan->nz;
     g.u = u; g.v = v; g.w = w; g.phi = p;
     g.rdzc = plan->rdzc;
     g.dt = dt;
@@ -562,13 +560,13 @@ int cans_plan_set_profiling(cans_poisson_plan* plan, int enable) {
     g_status = CANS_OK;
     if (!plan) return fail(CANS_ERR_INVALID_ARG, "plan is NULL");
     if (enable && !plan->prof) {
-        for (int i = 0; i < 24; ++i) {
+        for (int i = 0; i < 2 * MAX_REC; ++i) {
             cudaError_t e = cudaEventCreate(&plan->ev[i]);
             if (e != cudaSuccess) return fail_cuda(e, "cudaEventCreate");
         }
         plan->prof = 1;
     } else if (!enable && plan->prof) {
-        for (int i = 0; i < 24; ++i) cudaEventDestroy(plan->ev[i]);
+        for (int i = 0; i < 2 * MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
         plan->prof = 0;
     }
     plan->nrec = 0;

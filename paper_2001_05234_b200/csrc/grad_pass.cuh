@@ -9,6 +9,7 @@ namespace cans {
 
 struct GradArgs {
     int nx, ny, nz;
+    int k0, k1;                // planes [k0, k1) corrected by this launch
     double* u; double* v; double* w;
     const double* phi;
     const double* rdzc;        // [nz] 1/dzc[k+1]
@@ -18,45 +19,13 @@ struct GradArgs {
     double gx_sgn, gy_sgn, gz_sgn;
 };
 
-// inputs of one pair of x-adjacent cells (t = pair index, x fastest), fetched before any of them is
-// used so that a caller can keep several pairs' loads in flight
+// inputs of one pair of x-adjacent cells, fetched before any of them is used
 struct GradIn {
     double2 ph, phy, phz, uu, vv, ww;
     double phx;
     size_t o;
     int k;
 };
-
-CANS_HD GradIn grad_load(const GradArgs& a, size_t t) {
-    GradIn in;
-    const size_t plane = (size_t)a.nx * a.ny;
-    const int hx = a.nx / 2;
-    const int i = 2 * (int)(t % hx);
-    const size_t row = t / hx;
-    const int j = (int)(row % a.ny);
-    const int k = (int)(row / a.ny);
-    const size_t o = (size_t)k * plane + (size_t)j * a.nx + i;
-    in.o = o;
-    in.k = k;
-    in.ph = *reinterpret_cast<const double2*>(a.phi + o);
-    // x neighbour of the second cell
-    in.phx = (i + 2 < a.nx) ? a.phi[o + 2] : a.gx_sgn * a.phi[o - i + a.gx_idx];
-    // y neighbours
-    if (j + 1 < a.ny) in.phy = *reinterpret_cast<const double2*>(a.phi + o + a.nx);
-    else {
-        in.phy = *reinterpret_cast<const double2*>(a.phi + (size_t)k * plane + (size_t)a.gy_idx * a.nx + i);
-        in.phy.x *= a.gy_sgn; in.phy.y *= a.gy_sgn;
-    }
-    if (k + 1 < a.nz) in.phz = *reinterpret_cast<const double2*>(a.phi + o + plane);
-    else {
-        in.phz = *reinterpret_cast<const double2*>(a.phi + (size_t)a.gz_idx * plane + (size_t)j * a.nx + i);
-        in.phz.x *= a.gz_sgn; in.phz.y *= a.gz_sgn;
-    }
-    in.uu = *reinterpret_cast<const double2*>(a.u + o);
-    in.vv = *reinterpret_cast<const double2*>(a.v + o);
-    in.ww = *reinterpret_cast<const double2*>(a.w + o);
-    return in;
-}
 
 CANS_HD void grad_apply(const GradArgs& a, const GradIn& in) {
     double2 uu = in.uu, vv = in.vv, ww = in.ww;

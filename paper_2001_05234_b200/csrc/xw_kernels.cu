@@ -13,8 +13,9 @@ __global__ void __launch_bounds__(XW_WARPS * 32, 2) xw_kernel(const XYArgs a, co
     const long pr = (long)blockIdx.x * XW_WARPS + warp;
     if (pr >= npairs) return;                           // whole warp leaves: no CTA barrier is used
     const int hp = a.ny >> 1;
-    const int k = (int)(pr / hp);
-    const int j = 2 * (int)(pr - (long)k * hp);
+    const int kl = (int)(pr / hp);
+    const int k = a.k0 + kl;
+    const int j = 2 * (int)(pr - (long)kl * hp);
     const size_t ro = ((size_t)k * a.ny + j) * (size_t)a.nx;
     if (MODE == 2) W::inverse(a, tw, buf, ro, lane);
     else W::template forward<MODE == 1>(a, tw, buf, ro, j, k, lane);
@@ -23,15 +24,13 @@ __global__ void __launch_bounds__(XW_WARPS * 32, 2) xw_kernel(const XYArgs a, co
 template <int N, int R1>
 static cudaError_t xw_launch_n(int op, const XYArgs& a, const cplx* tw, cudaStream_t st) {
     const size_t smem = sizeof(cplx) * (size_t)XW_WARPS * XWPass<N, R1>::BUF;
-    static bool once = false;
-    if (!once) {
+    if (op == OP_CONFIGURE) {
         cudaError_t e = cudaFuncSetAttribute(xw_kernel<N, R1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(xw_kernel<N, R1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(xw_kernel<N, R1, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        once = true;
+        return e;
     }
-    const long npairs = (long)(a.ny / 2) * a.nz;
+    const long npairs = (long)(a.ny / 2) * a.nk;
     const unsigned grid = (unsigned)((npairs + XW_WARPS - 1) / XW_WARPS);
     if (op == OP_X_FWD) xw_kernel<N, R1, 0><<<grid, XW_WARPS * 32, smem, st>>>(a, tw, npairs);
     else if (op == OP_X_FWD_DIV) xw_kernel<N, R1, 1><<<grid, XW_WARPS * 32, smem, st>>>(a, tw, npairs);

@@ -6,7 +6,7 @@
 
 namespace cans {
 
-// op: OP_X_FWD, OP_X_FWD_DIV or OP_X_INV (xy_kernels.cuh); tw = W_N^(p k1) table [R1][32] of the plan.
+// op: OP_X_FWD, OP_X_FWD_DIV, OP_X_INV, or OP_CONFIGURE at plan time (xy_kernels.cuh); tw = W_N^(p k1) table [R1][32] of the plan.
 // Returns false if length n has no warp-per-line kernel.
 bool xw_launch(int n, int op, const XYArgs& a, const cplx* tw, cudaStream_t st, cudaError_t* err);
 

@@ -7,7 +7,8 @@
 
 namespace cans {
 
-enum XYOp : int { OP_X_FWD = 0, OP_X_FWD_DIV = 1, OP_X_INV = 2, OP_Y_FWD = 3, OP_Y_INV = 4 };
+// OP_CONFIGURE (plan time, on the plan's device): opt in to the dynamic shared memory of every kernel of a length
+enum XYOp : int { OP_X_FWD = 0, OP_X_FWD_DIV = 1, OP_X_INV = 2, OP_Y_FWD = 3, OP_Y_INV = 4, OP_CONFIGURE = 5 };
 
 extern __shared__ __align__(16) unsigned char cans_dyn_smem[];
 
@@ -45,7 +46,7 @@ __global__ void __launch_bounds__(NT, 2) y_pass_kernel(const XYArgs a) {
     cplx* sm = reinterpret_cast<cplx*>(cans_dyn_smem);
     const int tid = threadIdx.x;
     const int ctile = blockIdx.x;
-    const int k = blockIdx.y;
+    const int k = a.k0 + blockIdx.y;
     Y::load_twiddles(a, sm, tid);
     if (INV) {
         Y::load_inverse(a, sm, ctile, k, tid);
@@ -80,34 +81,24 @@ cudaError_t launch_xy(int op, const XYArgs& a, cudaStream_t st) {
     typedef YPass<P, TXC, NTY> Y;
     const size_t smx = sizeof(cplx) * X::SMEM_CPLX;
     const size_t smy = sizeof(cplx) * Y::SMEM_CPLX;
-    cudaError_t e = cudaSuccess;
+    if (op == OP_CONFIGURE) {
+        cudaError_t e = set_smem(x_pass_kernel<P, NFX, NTX, 0>, smx);
+        if (e == cudaSuccess) e = set_smem(x_pass_kernel<P, NFX, NTX, 1>, smx);
+        if (e == cudaSuccess) e = set_smem(x_pass_kernel<P, NFX, NTX, 2>, smx);
+        if (e == cudaSuccess) e = set_smem(y_pass_kernel<P, TXC, NTY, false>, smy);
+        if (e == cudaSuccess) e = set_smem(y_pass_kernel<P, TXC, NTY, true>, smy);
+        return e;
+    }
     if (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV) {
-        const long npairs = (long)(a.ny / 2) * a.nz;
+        const long npairs = (long)(a.ny / 2) * a.nk;
         const unsigned grid = (unsigned)((npairs + NFX - 1) / NFX);
-        if (op == OP_X_FWD) {
-            static bool once = false;
-            if (!once) { e = set_smem(x_pass_kernel<P, NFX, NTX, 0>, smx); if (e) return e; once = true; }
-            x_pass_kernel<P, NFX, NTX, 0><<<grid, NTX, smx, st>>>(a, npairs);
-        } else if (op == OP_X_FWD_DIV) {
-            static bool once = false;
-            if (!once) { e = set_smem(x_pass_kernel<P, NFX, NTX, 1>, smx); if (e) return e; once = true; }
-            x_pass_kernel<P, NFX, NTX, 1><<<grid, NTX, smx, st>>>(a, npairs);
-        } else {
-            static bool once = false;
-            if (!once) { e = set_smem(x_pass_kernel<P, NFX, NTX, 2>, smx); if (e) return e; once = true; }
-            x_pass_kernel<P, NFX, NTX, 2><<<grid, NTX, smx, st>>>(a, npairs);
-        }
+        if (op == OP_X_FWD) x_pass_kernel<P, NFX, NTX, 0><<<grid, NTX, smx, st>>>(a, npairs);
+        else if (op == OP_X_FWD_DIV) x_pass_kernel<P, NFX, NTX, 1><<<grid, NTX, smx, st>>>(a, npairs);
+        else x_pass_kernel<P, NFX, NTX, 2><<<grid, NTX, smx, st>>>(a, npairs);
     } else {
-        dim3 grid((unsigned)(a.nx / 2 / TXC), (unsigned)a.nz);
-        if (op == OP_Y_FWD) {
-            static bool once = false;
-            if (!once) { e = set_smem(y_pass_kernel<P, TXC, NTY, false>, smy); if (e) return e; once = true; }
-            y_pass_kernel<P, TXC, NTY, false><<<grid, NTY, smy, st>>>(a);
-        } else {
-            static bool once = false;
-            if (!once) { e = set_smem(y_pass_kernel<P, TXC, NTY, true>, smy); if (e) return e; once = true; }
-            y_pass_kernel<P, TXC, NTY, true><<<grid, NTY, smy, st>>>(a);
-        }
+        dim3 grid((unsigned)(a.nx / 2 / TXC), (unsigned)a.nk);
+        if (op == OP_Y_FWD) y_pass_kernel<P, TXC, NTY, false><<<grid, NTY, smy, st>>>(a);
+        else y_pass_kernel<P, TXC, NTY, true><<<grid, NTY, smy, st>>>(a);
     }
     return cudaGetLastError();
 }

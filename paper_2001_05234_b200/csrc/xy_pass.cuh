@@ -9,13 +9,13 @@
 //   DD   : x_j -> (-1)^j x_j, then as NN; the slot of C'_q holds sine mode n-1-q.
 // Spectral ("slot") layout of a line of n reals: positions (2s, 2s+1), s = 1..n/2-1, hold
 // (Re A_s, Im A_s) for PP or (C_s, C_{n-s}) for NN/DD; positions (0, 1) hold modes (0, n/2).
-// The eigenvalue of every position is tabulated by the plan (plan.cu), so the layout is private.
+// The eigenvalue of every position is tabulated by the plan (plan_tables.hpp), so the layout is private.
 //
 // x pass: the pair is two adjacent rows (j, j+1) of a plane; line index runs along x (contiguous).
 // y pass: the pair is two adjacent columns (i, i+1), i.e. one double2 per row; line index runs along y.
 //
 // Every phase is a function of (tid, block coordinates); phases are separated by block barriers in
-// kernels.cu.  No value is carried in registers across phases.
+// xy_kernels.cuh.  No value is carried in registers across phases.
 #pragma once
 #include "fft_core.cuh"
 
@@ -24,6 +24,7 @@ namespace cans {
 // Geometry + tables shared by the x/y kernels (passed by value as a kernel parameter).
 struct XYArgs {
     int nx, ny, nz;
+    int k0, nk;             // planes [k0, k0 + nk) handled by this launch (a batch of consecutive k-planes)
     int kind;               // Kind of THIS direction
     const cplx* tw;         // pass twiddles, FftPlan::TW_TOTAL entries
     const cplx* wpost;      // exp(-i pi q / (2n)), q = 0..n/2-1 (NN / DD only)
@@ -91,8 +92,7 @@ struct XPass {
     static constexpr int WORK_CPLX = NF * P::NPAD;             // line buffers
     static constexpr int SMEM_CPLX = NF * P::NPAD + P::TW_TOTAL;
 
-    // TWOFF: where this direction's twiddles live relative to the work buffer (the fused kernels
-    // of fused_pass.cuh keep one work buffer and both directions' tables behind it)
+    // TWOFF: where this direction's twiddles live relative to the work buffer
     static CANS_HD cplx* tw_smem(cplx* sm) { return sm + TWOFF; }
 
     static CANS_HD void load_twiddles(const XYArgs& a, cplx* sm, int tid) {
@@ -103,8 +103,9 @@ struct XPass {
     // pair index -> offset of row a (row b = +nx)
     static CANS_HD size_t row_offset(const XYArgs& a, long pr, int& j, int& k) {
         const int hp = a.ny >> 1;
-        k = (int)(pr / hp);
-        j = 2 * (int)(pr - (long)k * hp);
+        const int kl = (int)(pr / hp);
+        k = a.k0 + kl;
+        j = 2 * (int)(pr - (long)kl * hp);
         return ((size_t)k * a.ny + j) * (size_t)a.nx;
     }
 

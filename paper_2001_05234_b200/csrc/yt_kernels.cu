@@ -23,8 +23,9 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     // FIRST: all boxes at once.  Otherwise box by box, each as soon as the write-back of the same box of the tile
     // that occupied this buffer (one bulk group per box, oldest first) has finished reading shared memory.
     auto issue_load = [&](long t, int bsel, bool first) {
-        const int k = (int)(t / ntx);
-        const int c = (int)(t - (long)k * ntx);
+        const int kl = (int)(t / ntx);
+        const int c = (int)(t - (long)kl * ntx);
+        const int k = a.k0 + kl;
         mbar_expect_tx(&s_bar[bsel], W::TILE_BYTES);
 #pragma unroll
         for (int box = 0; box < W::NBOX; ++box) {
@@ -62,8 +63,9 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
         fence_proxy_async_smem();               // this thread's shared-memory writes -> visible to the TMA unit
         __syncthreads();
         if (tid == 0) {
-            const int k = (int)(t / ntx);
-            const int c = (int)(t - (long)k * ntx);
+            const int kl = (int)(t / ntx);
+            const int c = (int)(t - (long)kl * ntx);
+            const int k = a.k0 + kl;
             for (int box = 0; box < W::NBOX; ++box)
             {
                 tma_store_2d(&tmap, 2 * YT_COLS * c, k * N + box * YT_BOX_ROWS, T + (size_t)box * YT_BOX_ROWS * YT_COLS);
@@ -76,33 +78,32 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
 }
 
 template <int N, int R1>
-static cudaError_t yt_launch_n(int op, const XYArgs& a, const cplx* tw, int num_sms, cudaStream_t st) {
+static cudaError_t yt_launch_n(int op, const XYArgs& a, const cplx* tw, const CUtensorMap* tmap, int max_ctas, cudaStream_t st) {
     const size_t smem = 2 * sizeof(cplx) * (size_t)YTPass<N, R1>::TILE;
-    static bool once = false;
-    if (!once) {
+    if (op == OP_CONFIGURE) {
         cudaError_t e = cudaFuncSetAttribute(yt_kernel<N, R1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(yt_kernel<N, R1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        once = true;
+        return e;
     }
-    // the field as a 2-D tensor: nx doubles per row, ny*nz rows
-    CUtensorMap tmap;
-    cudaError_t e = make_tensor_map_2d(&tmap, a.p, (unsigned long long)a.nx, (unsigned long long)a.ny * a.nz,
-                                       (unsigned long long)a.nx * sizeof(double), 2 * YT_COLS, YT_BOX_ROWS,
-                                       CU_TENSOR_MAP_SWIZZLE_128B);
-    if (e != cudaSuccess) return e;
     const int ntx = a.nx / 2 / YT_COLS;
-    const long ntiles = (long)ntx * a.nz;
-    const unsigned grid = (unsigned)(ntiles < num_sms ? ntiles : num_sms);
-    if (op == OP_Y_FWD) yt_kernel<N, R1, false><<<grid, YT_NT, smem, st>>>(a, tw, tmap, ntx, ntiles);
-    else yt_kernel<N, R1, true><<<grid, YT_NT, smem, st>>>(a, tw, tmap, ntx, ntiles);
+    const long ntiles = (long)ntx * a.nk;
+    const unsigned grid = (unsigned)(ntiles < max_ctas ? ntiles : max_ctas);
+    if (op == OP_Y_FWD) yt_kernel<N, R1, false><<<grid, YT_NT, smem, st>>>(a, tw, *tmap, ntx, ntiles);
+    else yt_kernel<N, R1, true><<<grid, YT_NT, smem, st>>>(a, tw, *tmap, ntx, ntiles);
     return cudaGetLastError();
 }
 
-bool yt_launch(int n, int op, const XYArgs& a, const cplx* tw, int num_sms, cudaStream_t st, cudaError_t* err) {
+// the field as a 2-D tensor: nx doubles per row, ny*nz rows; boxes of 16 doubles x 256 rows, 128-byte swizzle
+cudaError_t yt_make_tensor_map(CUtensorMap* tmap, const double* p, int nx, int ny, int nz) {
+    return make_tensor_map_2d(tmap, p, (unsigned long long)nx, (unsigned long long)ny * nz,
+                              (unsigned long long)nx * sizeof(double), 2 * YT_COLS, YT_BOX_ROWS, CU_TENSOR_MAP_SWIZZLE_128B);
+}
+
+bool yt_launch(int n, int op, const XYArgs& a, const cplx* tw, const CUtensorMap* tmap, int max_ctas, cudaStream_t st,
+               cudaError_t* err) {
     switch (n) {
-        case 512: *err = yt_launch_n<512, 16>(op, a, tw, num_sms, st); return true;
-        case 768: *err = yt_launch_n<768, 24>(op, a, tw, num_sms, st); return true;
+        case 512: *err = yt_launch_n<512, 16>(op, a, tw, tmap, max_ctas, st); return true;
+        case 768: *err = yt_launch_n<768, 24>(op, a, tw, tmap, max_ctas, st); return true;
         default: return false;
     }
 }

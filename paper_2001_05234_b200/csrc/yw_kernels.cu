@@ -12,7 +12,7 @@ __global__ void __launch_bounds__(YW_NT, 2) yw_kernel(const XYArgs a, const cplx
     const int tid = threadIdx.x;
     const int warp = tid >> 5, lane = tid & 31;
     const int ctile = blockIdx.x;
-    const int k = blockIdx.y;
+    const int k = a.k0 + blockIdx.y;
     if (INV) {
         W::load_inverse(a, tile, ctile, k, tid);
         __syncthreads();
@@ -31,14 +31,12 @@ __global__ void __launch_bounds__(YW_NT, 2) yw_kernel(const XYArgs a, const cplx
 template <int N, int R1>
 static cudaError_t yw_launch_n(int op, const XYArgs& a, const cplx* tw, cudaStream_t st) {
     const size_t smem = sizeof(cplx) * (size_t)YWPass<N, R1>::TILE;
-    static bool once = false;
-    if (!once) {
+    if (op == OP_CONFIGURE) {
         cudaError_t e = cudaFuncSetAttribute(yw_kernel<N, R1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(yw_kernel<N, R1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        once = true;
+        return e;
     }
-    dim3 grid((unsigned)(a.nx / 2 / YW_TXC), (unsigned)a.nz);
+    dim3 grid((unsigned)(a.nx / 2 / YW_TXC), (unsigned)a.nk);
     if (op == OP_Y_FWD) yw_kernel<N, R1, false><<<grid, YW_NT, smem, st>>>(a, tw);
     else yw_kernel<N, R1, true><<<grid, YW_NT, smem, st>>>(a, tw);
     return cudaGetLastError();

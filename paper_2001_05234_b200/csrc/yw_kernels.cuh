@@ -6,7 +6,7 @@
 
 namespace cans {
 
-// op: OP_Y_FWD or OP_Y_INV (xy_kernels.cuh); tw = W_N^(p k1) table [R1][32] of the plan.
+// op: OP_Y_FWD, OP_Y_INV, or OP_CONFIGURE at plan time (xy_kernels.cuh); tw = W_N^(p k1) table [R1][32] of the plan.
 // Returns false if length n has no warp-per-column kernel.
 bool yw_launch(int n, int op, const XYArgs& a, const cplx* tw, cudaStream_t st, cudaError_t* err);
 

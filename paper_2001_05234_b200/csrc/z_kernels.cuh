@@ -1,5 +1,6 @@
 // z_kernels.cuh -- host-callable launchers of the z-solve kernels (defined in z_solve.cu).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include "z_pass.cuh"
 
@@ -12,8 +13,10 @@ inline int z_tc_for(int nseg) { return nseg <= 16 ? 32 : (nseg <= 32 ? 16 : 8); 
 
 // plan time: opt in to the dynamic shared memory of the solve kernel and compute the persistent grid
 cudaError_t z_solve_configure(int nseg, int nz, int num_sms, int* grid_out, size_t* smem_out);
-// enqueue the solve (a.ticket must point at a zeroed counter)
-cudaError_t z_solve_launch(const ZArgs& a, int grid, size_t smem, cudaStream_t st);
+// tensor map of the (nz, nx*ny) view of the field p, boxes of z_tc_for(nseg) columns
+cudaError_t z_make_tensor_map(CUtensorMap* tmap, const double* p, long ncols, int nz, int nseg);
+// enqueue the solve (a.ticket must point at a zeroed counter; tmap from z_make_tensor_map for a.p)
+cudaError_t z_solve_launch(const ZArgs& a, int grid, size_t smem, const CUtensorMap* tmap, cudaStream_t st);
 // plan time: fill rstart / r00 (synchronous)
 cudaError_t z_setup_launch(const ZArgs& a, double* rstart, double* r00);
 

@@ -37,7 +37,7 @@ struct ZArgs {
     const double* lamx;       // [nx]  lam_x(position)/dx^2
     const double* lamy;       // [ny]  lam_y(position)/dy^2
     const double* az;         // [nseg*MROWS] sub-diagonal a_k        (0 beyond nz, a_0 = 0)
-    const double* bz;         // diagonal b_k with boundary rows folded in (1 beyond nz)
+    const double* bz;         // diagonal b_k with boundary rows folded in (-1 beyond nz: keeps the padded pivots finite)
     const double* cz;         // super-diagonal c_k                   (0 beyond nz, c_{nz-1} = 0)
     const double* gz;         // a_k * c_{k-1}                        (0 for k = 0 and beyond nz)
     const double* rstart;     // [nseg][ncols]  r_{s*MROWS-1}(column)  (0 for s = 0)

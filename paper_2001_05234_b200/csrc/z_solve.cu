@@ -1,4 +1,4 @@
-// z_solve.cu -- pass B: persistent, cp.async double-buffered partitioned Thomas solve (z_pass.cuh).
+// z_solve.cu -- pass B: persistent partitioned Thomas solve (z_pass.cuh) fed by double-buffered TMA tile loads.
 #include "z_kernels.cuh"
 #include "tma_util.cuh"
 
@@ -123,27 +123,33 @@ cudaError_t z_solve_configure(int nseg, int nz, int num_sms, int* grid_out, size
     }
 }
 
-cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, cudaStream_t st) {
+// TMA tiling of a column tile: the padded column length nseg*MROWS is covered exactly by nbox boxes of box_rows
+// (<= 256) rows, box_rows = MROWS * (largest divisor of nseg that is <= 256/MROWS)
+static void z_boxes(int nseg, int* nbox, int* box_rows) {
+    int d = 256 / Z_MROWS;
+    while (nseg % d) --d;
+    *box_rows = d * Z_MROWS;
+    *nbox = nseg / d;
+}
+
+cudaError_t z_make_tensor_map(CUtensorMap* tmap, const double* p, long ncols, int nz, int nseg) {
+    int nbox, box_rows;
+    z_boxes(nseg, &nbox, &box_rows);
+    return make_tensor_map_2d(tmap, p, (unsigned long long)ncols, (unsigned long long)nz,
+                              (unsigned long long)ncols * sizeof(double), (unsigned)z_tc_for(nseg), (unsigned)box_rows,
+                              CU_TENSOR_MAP_SWIZZLE_NONE);
+}
+
+cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, const CUtensorMap* tmap, cudaStream_t st) {
     ZArgs a = a_in;
     long g = grid;
     if (g > a.ntiles) g = a.ntiles;
     if (g < 1) g = 1;
-    // the padded column length nseg*MROWS is covered exactly by nbox boxes of box_rows (<= 256) rows:
-    // box_rows = MROWS * (largest divisor of nseg that is <= 256/MROWS)
-    int d = 256 / Z_MROWS;
-    while (a.nseg % d) --d;
-    a.box_rows = d * Z_MROWS;
-    a.nbox = a.nseg / d;
-    const int tc = z_tc_for(a.nseg);
-    CUtensorMap tmap;
-    cudaError_t e = make_tensor_map_2d(&tmap, a.p, (unsigned long long)a.ncols, (unsigned long long)a.nz,
-                                       (unsigned long long)a.ncols * sizeof(double), (unsigned)tc, (unsigned)a.box_rows,
-                                       CU_TENSOR_MAP_SWIZZLE_NONE);
-    if (e != cudaSuccess) return e;
-    switch (tc) {
-        case 32: z_solve_kernel<Z_MROWS, 32><<<(unsigned)g, 32 * a.nseg, smem, st>>>(a, tmap); break;
-        case 16: z_solve_kernel<Z_MROWS, 16><<<(unsigned)g, 16 * a.nseg, smem, st>>>(a, tmap); break;
-        default: z_solve_kernel<Z_MROWS, 8><<<(unsigned)g, 8 * a.nseg, smem, st>>>(a, tmap); break;
+    z_boxes(a.nseg, &a.nbox, &a.box_rows);
+    switch (z_tc_for(a.nseg)) {
+        case 32: z_solve_kernel<Z_MROWS, 32><<<(unsigned)g, 32 * a.nseg, smem, st>>>(a, *tmap); break;
+        case 16: z_solve_kernel<Z_MROWS, 16><<<(unsigned)g, 16 * a.nseg, smem, st>>>(a, *tmap); break;
+        default: z_solve_kernel<Z_MROWS, 8><<<(unsigned)g, 8 * a.nseg, smem, st>>>(a, *tmap); break;
     }
     return cudaGetLastError();
 }

@@ -122,7 +122,7 @@ def test_c4_full_size_eigenmodes_and_backward_error(B):
     torch.cuda.synchronize()
     got, ref = p.cpu().numpy(), sol_modes.cpu().numpy()
     assert rel_l2(got, ref) <= REL_L2
-    assert np.max(np.abs(got - ref)) <= MAX_ABS * max(1.0, np.max(np.abs(ref)))
+    assert np.max(np.abs(got - ref)) <= MAX_ABS          # |Phi| = O(1e-1) here: the bar applies to Phi directly
     del got, ref
     # (b) full C4 right-hand side (modes + 1e-3 Gaussian noise): backward error on sampled planes
     f = f_modes + w.fields["f"]
@@ -213,3 +213,56 @@ def test_c5_full_size_projection_sampled_planes(B):
         div = orc.divergence(u[sl].cpu().numpy(), v[sl].cpu().numpy(), ww[sl].cpu().numpy(),
                              lx, ly, lz, bc_lo, dzc[k0:k + 2], dzf[k0:k + 1])[k - k0]
         assert np.max(np.abs(div)) <= 1e-10 * float(u0.abs().max()) / hmin, k
+
+
+def _host_ram_gb():
+    import psutil
+    return psutil.virtual_memory().available / 2**30
+
+
+def test_c5_full_size_oracle_parity(B):
+    """The whole C5 step (1024x768x512, the configuration and launch sequence bench.py times) against the oracle on the
+    same buffers: u, v, w and dt*Phi element by element at the BASELINE.json bar (rel-L2 <= 1e-11 on the raw fields,
+    max-abs <= 1e-10 on u, v, w and dt*Phi -- reading S12)."""
+    if _host_ram_gb() < 96:
+        pytest.skip("the full-size oracle needs ~60 GB of host memory")
+    w = wl.make_workload("C5", device="cuda")
+    plan = B.plan_for(w)
+    u, v, ww = (w.fields[c].clone() for c in "uvw")
+    p = torch.empty_like(u)
+    plan.projection(u, v, ww, p, w.dt)
+    torch.cuda.synchronize()
+    plan.close()
+    got = [t.cpu().numpy() for t in (u, v, ww, p)]
+    del u, v, ww, p
+    host = [w.fields[c].cpu().numpy() for c in "uvw"]
+    w.fields.clear()
+    torch.cuda.empty_cache()
+    un, vn, wn, phi, _ = orc.projection(*host, w.dt, *w.lengths, w.bc, w.dzc.numpy(), w.dzf.numpy())
+    del host
+    for g, ref, scale, name in ((got[0], un, 1.0, "u"), (got[1], vn, 1.0, "v"), (got[2], wn, 1.0, "w"), (got[3], phi, w.dt, "dt*Phi")):
+        assert rel_l2(g, ref) <= REL_L2, name
+        assert np.max(np.abs(g - ref)) * scale <= MAX_ABS, name
+
+
+def test_c4_full_size_oracle_parity(B):
+    """Full C4 (1024x512x512, PP/DD/NN, tanh a = 2): 64 planted eigenmodes + 1e-3 Gaussian noise against orc.poisson_solve,
+    element by element."""
+    if _host_ram_gb() < 64:
+        pytest.skip("the full-size oracle needs ~40 GB of host memory")
+    w = wl.make_workload("C4", device="cuda")
+    f_modes, _ = _c4_modes(w)
+    f = f_modes + w.fields["f"]
+    del f_modes
+    plan = B.plan_for(w)
+    p = f.clone()
+    plan.poisson_solve(p)
+    torch.cuda.synchronize()
+    plan.close()
+    got = p.cpu().numpy()
+    fh = f.cpu().numpy()
+    del p, f
+    torch.cuda.empty_cache()
+    ref = orc.poisson_solve(fh, *w.lengths, w.bc, w.dzc.numpy(), w.dzf.numpy())
+    assert rel_l2(got, ref) <= REL_L2
+    assert np.max(np.abs(got - ref)) <= MAX_ABS

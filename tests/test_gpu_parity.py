@@ -374,3 +374,79 @@ def test_tallest_columns(B, nz):
     with pytest.raises(B.CansError) as ei:
         B.PoissonPlan(nx, ny, 1025, lx, ly, lz, bc)
     assert ei.value.status == B.CANS_ERR_UNSUPPORTED_SIZE
+
+
+# ----------------------------------------------------------------------------------------------
+# the z-solve instantiation bench.py times on C4 / C5: 257 <= nz <= 512 runs z_solve_kernel<16,16> (tiles of 16 columns,
+# up to 32 segments per column, two TMA boxes per tile).  48 x 32 columns = 96 tiles, so a persistent CTA sees several
+# tiles (both buffers, the ticket hand-over); heights just above the switch (257), ragged (300, 497, 511) and full (512).
+# ----------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("nz", [257, 300, 497, 511, 512])
+def test_z_tiles_of_16_columns_every_z_pair(B, nz):
+    nx, ny = 48, 32
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    seed = 9000 + nz
+    for pz in ZP:
+        for px, py in (("PP", "PP"), ("NN", "DD")):
+            bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+            seed += 1
+            f = random_rhs(nx, ny, nz, bc, dzf, seed)
+            plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+            p = torch.from_numpy(f).cuda()
+            plan.poisson_solve(p)
+            torch.cuda.synchronize()
+            ref = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+            check_field(np_of(p), ref, what=f"poisson {px}/{py}/{pz} nz={nz}")
+            if px == "PP":
+                rng = np.random.default_rng(seed)
+                u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+                faces = {}
+                if pz[0] == "D":
+                    faces[2] = rng.standard_normal((1, ny, nx))
+                ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+                fd = {d: torch.from_numpy(t).cuda() for d, t in faces.items()}
+                for d, t in fd.items():
+                    plan.set_lower_face(d, t)
+                pd = torch.empty_like(ud)
+                plan.projection(ud, vd, wd, pd, 1e-3)
+                torch.cuda.synchronize()
+                un, vn, wn, phi, fn = orc.projection(u, v, w, 1e-3, lx, ly, lz, bc, dzc, dzf, faces)
+                for got, refv, sc, nm in ((ud, un, 1.0, "u"), (vd, vn, 1.0, "v"), (wd, wn, 1.0, "w"), (pd, phi, 1e-3, "dt*Phi")):
+                    check_field(np_of(got), refv, scale=sc, what=f"projection {nm} {px}/{py}/{pz} nz={nz}")
+                for d in fd:
+                    check_field(np_of(fd[d]), fn[d], what=f"face {d} nz={nz}")
+            plan.close()
+
+
+@pytest.mark.parametrize("nx,ny,nz", [(1024, 768, 24), (512, 512, 17), (256, 128, 33), (768, 1024, 9), (96, 64, 40)])
+@pytest.mark.parametrize("batch", [1, 4, 5])
+def test_plane_batched_launches_are_bit_identical(B, nx, ny, nz, batch):
+    """cans_plan_set_batch only changes how many planes one launch covers: the batched sequence (x then y per batch;
+    y, x, then the correction trailing by one plane) must return the same bits as one launch per step, for the Poisson
+    solve and the projection, including batches that do not divide nz and lower-face planes."""
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    for bc in ((("P", "P"), ("P", "P"), ("N", "N")), (("N", "N"), ("D", "D"), ("D", "N"))):
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc_t, dzf_t)
+        g = torch.Generator(device="cuda").manual_seed(nx + nz)
+        f, u0, v0, w0 = (torch.randn((nz, ny, nx), dtype=torch.float64, device="cuda", generator=g) for _ in range(4))
+        shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+        faces0 = {d: torch.randn(shapes[d], dtype=torch.float64, device="cuda", generator=g) for d in range(3) if bc[d][0] == "D"}
+        results = []
+        for b in (0, batch):
+            assert plan.set_batch(b) == (b if b < nz else 0)
+            p = f.clone()
+            plan.poisson_solve(p)
+            u, v, w = u0.clone(), v0.clone(), w0.clone()
+            faces = {d: t.clone() for d, t in faces0.items()}
+            for d, t in faces.items():
+                plan.set_lower_face(d, t)
+            phi = torch.empty_like(u)
+            plan.projection(u, v, w, phi, 1e-3)
+            torch.cuda.synchronize()
+            results.append((p, u, v, w, phi, *faces.values()))
+        for a, b_ in zip(*results):
+            assert torch.equal(a, b_)
+        plan.close()

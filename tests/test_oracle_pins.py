@@ -403,3 +403,83 @@ def test_projection_annihilates_pure_gradient_and_keeps_poiseuille():
     up = np.broadcast_to((6 * (zc / lz) * (1 - zc / lz))[:, None, None], (nz, ny, nx)).copy()
     un, vn, wn, phi, _ = orc.projection(up, z, z, dt, lx, ly, lz, bc, dzc, dzf)
     assert np.max(np.abs(un - up)) < 1e-14 and np.max(np.abs(dt * phi)) < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------
+# divergence (eq. 2b) and correction (eq. 2c) pinned INDIVIDUALLY on linear fields, whose staggered differences
+# are known in closed form (the pair test above fixes only the product D.G)
+# ----------------------------------------------------------------------------------------------
+def _linear_setup(nx=6, ny=5, nz=7, a=1.7):
+    lx, ly, lz = 1.5, 2.5, 2.0
+    dzc, dzf = stretched(nz, lz, a)
+    zf = np.concatenate([[0.0], np.cumsum(dzf)])            # face heights, zf[k+1] = upper face of cell k
+    zc = 0.5 * (zf[1:] + zf[:-1])
+    xf = (np.arange(nx) + 1) * lx / nx                      # +x face of cell i
+    yf = (np.arange(ny) + 1) * ly / ny
+    xc = (np.arange(nx) + 0.5) * lx / nx
+    yc = (np.arange(ny) + 0.5) * ly / ny
+    return (nx, ny, nz), (lx, ly, lz), dzc, dzf, (xf, yf, zf[1:]), (xc, yc, zc)
+
+
+def test_divergence_of_linear_fields_is_their_slope():
+    """u = cu*x_face, v = cv*y_face, w = cw*z_face  =>  D u = cu + cv + cw exactly (sign, scale, spacing and
+    staggering of every term of eq. 2b; stretched z uses dzf).  Non-periodic sides: the lower face of an
+    'N' side is the wall at coordinate 0 (value 0 = the linear field there), of a 'D' side the registered plane."""
+    (nx, ny, nz), (lx, ly, lz), dzc, dzf, (xf, yf, zfu), _ = _linear_setup()
+    cu, cv, cw = 0.75, -1.25, 2.5
+    u = np.broadcast_to(cu * xf[None, None, :], (nz, ny, nx)).copy()
+    v = np.broadcast_to(cv * yf[None, :, None], (nz, ny, nx)).copy()
+    w = np.broadcast_to(cw * zfu[:, None, None], (nz, ny, nx)).copy()
+    bc = (("N", "N"), ("N", "N"), ("N", "N"))
+    d = orc.divergence(u, v, w, lx, ly, lz, bc, dzc, dzf)
+    assert np.max(np.abs(d - (cu + cv + cw))) < 1e-13
+    # each term alone: only one component non-zero
+    z = np.zeros_like(u)
+    assert np.max(np.abs(orc.divergence(u, z, z, lx, ly, lz, bc, dzc, dzf) - cu)) < 1e-13
+    assert np.max(np.abs(orc.divergence(z, v, z, lx, ly, lz, bc, dzc, dzf) - cv)) < 1e-13
+    assert np.max(np.abs(orc.divergence(z, z, w, lx, ly, lz, bc, dzc, dzf) - cw)) < 1e-13
+    # lower 'D' sides with registered planes holding the linear field's value there (0), and a shifted plane:
+    # a constant offset c0 on the lower plane changes only the first cell, by -c0/h
+    bcd = (("D", "D"), ("D", "N"), ("D", "D"))
+    faces = {0: np.zeros((nz, ny, 1)), 1: np.zeros((nz, 1, nx)), 2: np.zeros((1, ny, nx))}
+    d = orc.divergence(u, v, w, lx, ly, lz, bcd, dzc, dzf, faces)
+    assert np.max(np.abs(d - (cu + cv + cw))) < 1e-13
+    faces[2] = np.full((1, ny, nx), 0.5)
+    d2 = orc.divergence(u, v, w, lx, ly, lz, bcd, dzc, dzf, faces)
+    assert np.max(np.abs(d2[0] - (cu + cv + cw - 0.5 / dzf[0]))) < 1e-13 and np.array_equal(d2[1:], d[1:])
+    # prescribed inflow on a lower 'N' side is read the same way
+    d3 = orc.divergence(u, v, w, lx, ly, lz, bc, dzc, dzf, {0: np.full((nz, ny, 1), -2.0)})
+    assert np.max(np.abs(d3[:, :, 0] - (cu + cv + cw + 2.0 / (lx / nx)))) < 1e-13
+    # periodic: the lower face is the wrapped last value
+    bcp = (("P", "P"), ("N", "N"), ("N", "N"))
+    d4 = orc.divergence(u, z, z, lx, ly, lz, bcp, dzc, dzf)
+    assert np.max(np.abs(d4[:, :, 1:] - cu)) < 1e-13
+    assert np.max(np.abs(d4[:, :, 0] - (cu * xf[0] - cu * xf[-1]) / (lx / nx))) < 1e-13
+
+
+def test_gradient_of_linear_phi_is_constant():
+    """phi = gx*x_c + gy*y_c + gz*z_c  =>  eq. 2c subtracts dt*(gx, gy, gz) on every interior face
+    (stretched z: centre distances dzc); on the upper faces the ghost rule decides: 'N' leaves the value
+    bit-identical, 'D' subtracts dt*(-phi_last - phi_last)/h.  Lower 'D' planes: -= dt*2*phi_first/h."""
+    (nx, ny, nz), (lx, ly, lz), dzc, dzf, _, (xc, yc, zc) = _linear_setup()
+    gx, gy, gz = 1.5, -0.5, 2.0
+    phi = gx * xc[None, None, :] + gy * yc[None, :, None] + gz * zc[:, None, None]
+    rng = np.random.default_rng(3)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    dt = 0.125
+    bc = (("N", "N"), ("D", "D"), ("D", "N"))
+    faces = {1: rng.standard_normal((nz, 1, nx)), 2: rng.standard_normal((1, ny, nx))}
+    un, vn, wn, fn = orc.correct_velocity(u, v, w, phi, dt, lx, ly, lz, bc, dzc, dzf, faces)
+    assert np.max(np.abs(un[:, :, :-1] - (u[:, :, :-1] - dt * gx))) < 1e-13
+    assert np.max(np.abs(vn[:, :-1, :] - (v[:, :-1, :] - dt * gy))) < 1e-13
+    assert np.max(np.abs(wn[:-1] - (w[:-1] - dt * gz))) < 1e-13
+    assert np.array_equal(un[:, :, -1], u[:, :, -1])                      # upper 'N' in x
+    assert np.array_equal(wn[-1], w[-1])                                  # upper 'N' in z
+    dy = ly / ny
+    assert np.max(np.abs(vn[:, -1, :] - (v[:, -1, :] - dt * (-2.0 * phi[:, -1, :]) / dy))) < 1e-13   # upper 'D' in y
+    assert np.max(np.abs(fn[1] - (faces[1] - dt * 2.0 * phi[:, :1, :] / dy))) < 1e-13               # lower 'D' in y
+    assert np.max(np.abs(fn[2] - (faces[2] - dt * 2.0 * phi[:1] / dzc[0]))) < 1e-13                 # lower 'D' in z
+    # periodic x: the last face sees the wrapped phi
+    bcp = (("P", "P"), ("N", "N"), ("N", "N"))
+    un, _, _, _ = orc.correct_velocity(u, v, w, phi, dt, lx, ly, lz, bcp, dzc, dzf)
+    assert np.max(np.abs(un[:, :, -1] - (u[:, :, -1] - dt * (phi[:, :, 0] - phi[:, :, -1]) / (lx / nx)))) < 1e-13
