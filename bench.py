@@ -288,6 +288,8 @@ def run_ours(args):
     plan = binding.plan_for(w)
     if args.batch is not None:
         plan.set_batch(args.batch)
+    if args.pipeline:
+        plan.set_pipeline(True)
     u0, v0, w0 = (w.fields[c] for c in "uvw")
     u, v, ww = torch.empty_like(u0), torch.empty_like(u0), torch.empty_like(u0)
     p = torch.empty_like(u0)
@@ -435,6 +437,7 @@ def main():
     ap.add_argument("--batch", type=int, default=None,
                     help="planes per launch of the x / y / correction kernels (cans_plan_set_batch; 0 = one launch per step; "
                          "default: the plan's own choice)")
+    ap.add_argument("--pipeline", action="store_true", help="run the plane batches on the plan's own streams (producer/consumer overlap)")
     ap.add_argument("--no-extra", action="store_true", help="skip the Poisson-only timings of C2..C5")
     args = ap.parse_args()
     if args.impl == "reference":

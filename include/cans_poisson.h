@@ -152,6 +152,7 @@ const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
  * Returns the resulting batch size (0 if planes <= 0 or planes >= nz); a NULL plan sets CANS_ERR_INVALID_ARG and returns 0.
  */
 int cans_plan_set_batch(cans_poisson_plan* plan, int planes);
+int cans_plan_set_pipeline(cans_poisson_plan* plan, int enable);
 
 /* "x.y" version string of the library. */
 const char* cans_version(void);

@@ -133,6 +133,10 @@ struct cans_poisson_plan {
     int z_grid;               // persistent grid of the z solve
     size_t z_smem;
     int batch;                // planes per launch of the x / y / gradient kernels; 0: one launch per step over all planes
+    int pipeline;             // 1: the batches of a pass run on the plan's own streams, consumer kernels one batch behind
+    cudaStream_t lane[3];     // low / mid / high priority (producer ... consumer)
+    cudaEvent_t pev[3][4];    // per lane: ring of "batch done" events
+    cudaEvent_t fork_ev, join_ev;
     unsigned int* sched;      // scheduler state (z tile ticket), zeroed at the start of every call
     size_t sched_bytes;
     std::vector<void*> dev_allocs;
@@ -274,6 +278,12 @@ void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
     for (void* d : plan->dev_allocs) cudaFree(d);
     for (int i = 0; i < 4; ++i) if (plan->hostbuf[i]) cudaFree(plan->hostbuf[i]);
     if (plan->prof) for (int i = 0; i < 2 * MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
+    for (int l = 0; l < 3; ++l) {
+        if (plan->lane[l]) cudaStreamDestroy(plan->lane[l]);
+        for (int i = 0; i < 4; ++i) if (plan->pev[l][i]) cudaEventDestroy(plan->pev[l][i]);
+    }
+    if (plan->fork_ev) cudaEventDestroy(plan->fork_ev);
+    if (plan->join_ev) cudaEventDestroy(plan->join_ev);
     delete plan;
 }
 
@@ -322,6 +332,9 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->dzc0 = hdzc[0];
     pl->prof = 0; pl->nrec = 0;
     pl->batch = 0;
+    pl->pipeline = 0;
+    for (int l = 0; l < 3; ++l) { pl->lane[l] = nullptr; for (int i = 0; i < 4; ++i) pl->pev[l][i] = nullptr; }
+    pl->fork_ev = pl->join_ev = nullptr;
     pl->tmap_field = nullptr;
     pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
     pl->device = 0;
@@ -424,6 +437,65 @@ static int ensure_tensor_maps(cans_poisson_plan* pl, double* p) {
     return CANS_OK;
 }
 
+// Plane-batched passes on the plan's own streams: the producer of batch b+1 (x forward / y inverse) overlaps the consumer of
+// batch b (y forward / x inverse / correction), so that the drain of one short kernel is filled by the next one's CTAs;
+// a producer runs at most two batches ahead of its consumer, which bounds the intermediate planes waiting in L2.
+static int run_pipelined(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st, int B) {
+    int rc;
+    const int nz = pl->nz;
+    cudaStream_t lo = pl->lane[0], mid = pl->lane[1], hi = pl->lane[2];
+    auto ck = [&](cudaError_t e) { return e == cudaSuccess ? CANS_OK : fail_cuda(e, "pipeline event"); };
+    XYArgs ax = divargs ? *divargs : make_xyargs(pl, p, true);
+    XYArgs ay = make_xyargs(pl, p, false);
+    const int opx = divargs ? OP_X_FWD_DIV : OP_X_FWD;
+    {   // pass A: x(b) on the low lane, y(b) on the high lane
+        LaunchScope scope(pl, st, divargs ? "pass_a_div" : "pass_a");
+        if ((rc = ck(cudaEventRecord(pl->fork_ev, st)))) return rc;
+        if ((rc = ck(cudaStreamWaitEvent(lo, pl->fork_ev, 0)))) return rc;
+        int b = 0;
+        for (int k0 = 0; k0 < nz; k0 += B, ++b) {
+            ax.k0 = ay.k0 = k0;
+            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
+            if (b >= 2 && (rc = ck(cudaStreamWaitEvent(lo, pl->pev[2][(b - 2) & 3], 0)))) return rc;
+            if ((rc = launch_xy_any(pl, pl->nx, opx, ax, lo, false))) return rc;
+            if ((rc = ck(cudaEventRecord(pl->pev[0][b & 3], lo)))) return rc;
+            if ((rc = ck(cudaStreamWaitEvent(hi, pl->pev[0][b & 3], 0)))) return rc;
+            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, ay, hi, false))) return rc;
+            if ((rc = ck(cudaEventRecord(pl->pev[2][b & 3], hi)))) return rc;
+        }
+        if ((rc = ck(cudaStreamWaitEvent(st, pl->pev[2][(b - 1) & 3], 0)))) return rc;
+    }
+    if ((rc = launch_z(pl, p, st))) return rc;
+    {   // pass C: y inverse (low), x inverse (mid), correction of the planes whose Phi(k+1) exists (high)
+        LaunchScope scope(pl, st, grad ? "pass_c_grad" : "pass_c");
+        if ((rc = ck(cudaEventRecord(pl->fork_ev, st)))) return rc;
+        if ((rc = ck(cudaStreamWaitEvent(lo, pl->fork_ev, 0)))) return rc;
+        ax = make_xyargs(pl, p, true);
+        int b = 0;
+        for (int k0 = 0; k0 < nz; k0 += B, ++b) {
+            ax.k0 = ay.k0 = k0;
+            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
+            if (b >= 2 && (rc = ck(cudaStreamWaitEvent(lo, pl->pev[1][(b - 2) & 3], 0)))) return rc;
+            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, ay, lo, false))) return rc;
+            if ((rc = ck(cudaEventRecord(pl->pev[0][b & 3], lo)))) return rc;
+            if ((rc = ck(cudaStreamWaitEvent(mid, pl->pev[0][b & 3], 0)))) return rc;
+            if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, ax, mid, false))) return rc;
+            if ((rc = ck(cudaEventRecord(pl->pev[1][b & 3], mid)))) return rc;
+            if (grad) {
+                const int g0 = k0 > 0 ? k0 - 1 : 0;
+                const int g1 = (k0 + ax.nk == nz) ? nz : k0 + ax.nk - 1;
+                if ((rc = ck(cudaStreamWaitEvent(hi, pl->pev[1][b & 3], 0)))) return rc;
+                if ((rc = launch_grad(pl, *grad, g0, g1, hi, false))) return rc;
+            }
+        }
+        if (grad) {
+            if ((rc = ck(cudaEventRecord(pl->join_ev, hi)))) return rc;
+            if ((rc = ck(cudaStreamWaitEvent(st, pl->join_ev, 0)))) return rc;
+        } else if ((rc = ck(cudaStreamWaitEvent(st, pl->pev[1][(b - 1) & 3], 0)))) return rc;
+    }
+    return CANS_OK;
+}
+
 // the whole path shared by both entry points; `divargs` selects the fused-divergence load (a1),
 // `grad` the velocity correction (a7)
 static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st) {
@@ -441,6 +513,7 @@ static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, con
     XYArgs ax = divargs ? *divargs : make_xyargs(pl, p, true);
     XYArgs ay = make_xyargs(pl, p, false);
     const int opx = divargs ? OP_X_FWD_DIV : OP_X_FWD;
+    if (batched && pl->pipeline) return run_pipelined(pl, p, divargs, grad, st, B);
     {   // pass A: (a1 +) a2, a3 per batch of planes
         LaunchScope scope(pl, st, divargs ? "pass_a_div" : "pass_a", batched);
         for (int k0 = 0; k0 < nz; k0 += B) {
@@ -475,6 +548,26 @@ int cans_plan_set_batch(cans_poisson_plan* plan, int planes) {
     if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
     plan->batch = (planes > 0 && planes < plan->nz) ? planes : 0;
     return plan->batch;
+}
+
+int cans_plan_set_pipeline(cans_poisson_plan* plan, int enable) {
+    g_status = CANS_OK;
+    if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
+    if (enable && !plan->lane[0]) {
+        int least = 0, greatest = 0;
+        cudaError_t e = cudaDeviceGetStreamPriorityRange(&least, &greatest);
+        for (int l = 0; l < 3 && e == cudaSuccess; ++l) {
+            int prio = least - l;                          // numerically lower = higher priority
+            if (prio < greatest) prio = greatest;
+            e = cudaStreamCreateWithPriority(&plan->lane[l], cudaStreamNonBlocking, prio);
+            for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&plan->pev[l][i], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->fork_ev, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->join_ev, cudaEventDisableTiming);
+        if (e != cudaSuccess) { fail_cuda(e, "pipeline streams"); return 0; }
+    }
+    plan->pipeline = enable ? 1 : 0;
+    return plan->pipeline;
 }
 
 static int batches_of(const cans_poisson_plan* plan) {

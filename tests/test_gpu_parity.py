@@ -435,8 +435,9 @@ def test_plane_batched_launches_are_bit_identical(B, nx, ny, nz, batch):
         shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
         faces0 = {d: torch.randn(shapes[d], dtype=torch.float64, device="cuda", generator=g) for d in range(3) if bc[d][0] == "D"}
         results = []
-        for b in (0, batch):
+        for b, pipe in ((0, False), (batch, False), (batch, True)):
             assert plan.set_batch(b) == (b if b < nz else 0)
+            assert plan.set_pipeline(pipe) == pipe
             p = f.clone()
             plan.poisson_solve(p)
             u, v, w = u0.clone(), v0.clone(), w0.clone()
@@ -447,6 +448,7 @@ def test_plane_batched_launches_are_bit_identical(B, nx, ny, nz, batch):
             plan.projection(u, v, w, phi, 1e-3)
             torch.cuda.synchronize()
             results.append((p, u, v, w, phi, *faces.values()))
-        for a, b_ in zip(*results):
-            assert torch.equal(a, b_)
+        for other in results[1:]:
+            for a, b_ in zip(results[0], other):
+                assert torch.equal(a, b_)
         plan.close()
