@@ -38,11 +38,6 @@ KERNEL_BYTES_PER_CELL = {
     "y_inv": 16.0,
     "x_inv": 16.0,
     "grad_correct": 56.0,  # read Phi (8) + u, v, w (24), write u, v, w (24)
-    # plane-batched passes (cans_plan_set_batch): the intermediate planes stay in L2 between the launches of a batch
-    "pass_a_div": 32.0,    # pass A: read u, v, w (24) + write f^ (8)
-    "pass_a": 16.0,
-    "pass_c": 16.0,
-    "pass_c_grad": 64.0,   # pass C: read Phi^ (8) + u, v, w (24), write Phi (8) + u, v, w (24)
 }
 STEP_MIN_BYTES_PER_CELL = {"projection": 112.0, "poisson": 48.0}   # structural minimum, SURVEY.md 8(d)
 
@@ -286,10 +281,6 @@ def run_ours(args):
     nx, ny, nz = w.n
     cells = w.cells
     plan = binding.plan_for(w)
-    if args.batch is not None:
-        plan.set_batch(args.batch)
-    if args.pipeline:
-        plan.set_pipeline(True)
     u0, v0, w0 = (w.fields[c] for c in "uvw")
     u, v, ww = torch.empty_like(u0), torch.empty_like(u0), torch.empty_like(u0)
     p = torch.empty_like(u0)
@@ -434,10 +425,6 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg")
     ap.add_argument("--no-cpu", action="store_true", help="skip the CPU-oracle baseline leg")
-    ap.add_argument("--batch", type=int, default=None,
-                    help="planes per launch of the x / y / correction kernels (cans_plan_set_batch; 0 = one launch per step; "
-                         "default: the plan's own choice)")
-    ap.add_argument("--pipeline", action="store_true", help="run the plane batches on the plan's own streams (producer/consumer overlap)")
     ap.add_argument("--no-extra", action="store_true", help="skip the Poisson-only timings of C2..C5")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -128,9 +128,8 @@ int cans_plan_launches_per_projection(const cans_poisson_plan* plan);
 
 /*
  * Optional per-kernel timing for bench.py.  With profiling enabled every kernel launch of the next
- * cans_poisson_solve / cans_projection call (with plane batches: every pass -- "pass_a[_div]", "z_solve",
- * "pass_c[_grad]") is bracketed by a cudaEvent pair on the caller's stream; at most CANS_MAX_KERNEL_RECORDS
- * records per call.  cans_plan_kernel_times waits for those events and writes the duration (ms) of each record of
+ * cans_poisson_solve / cans_projection call is bracketed by a cudaEvent pair on the caller's stream; at most
+ * CANS_MAX_KERNEL_RECORDS records per call.  cans_plan_kernel_times waits for those events and writes the duration (ms) of each record of
  * the LAST call, in launch order, into ms[0..capacity); returns the number written, or -1 on error.
  * cans_plan_kernel_name returns the name of record idx of the last call ("" if out of range).
  */
@@ -138,21 +137,6 @@ int cans_plan_launches_per_projection(const cans_poisson_plan* plan);
 int cans_plan_set_profiling(cans_poisson_plan* plan, int enable);
 int cans_plan_kernel_times(cans_poisson_plan* plan, float* ms, int capacity);
 const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
-
-/*
- * cans_plan_set_batch -- choose the launch granularity of the x / y transforms and of the correction (pass A and pass C of
- * SURVEY 8(d)).  Both sequences run the same kernels on the same data in the same order per plane, so their results are
- * bit-identical:
- *   planes = 0 (default until tuned per size)  one launch per step of SURVEY 8(a) over all nz planes: 5 launches per
- *           solve, 6 per projection; every intermediate makes a round trip through HBM (80 / 152 B per cell);
- *   planes = B > 0  the same kernels launched per batch of B consecutive k-planes: x then y forward (pass A); y, x
- *           inverse, then the correction of the planes whose Phi(k+1) is complete (pass C).  The dependency between the
- *           steps is stream order; the batch (B*nx*ny*8 bytes) stays in the 126 MB L2 between its launches, which brings
- *           the HBM traffic towards the structural minimum (48 / 112 B per cell).
- * Returns the resulting batch size (0 if planes <= 0 or planes >= nz); a NULL plan sets CANS_ERR_INVALID_ARG and returns 0.
- */
-int cans_plan_set_batch(cans_poisson_plan* plan, int planes);
-int cans_plan_set_pipeline(cans_poisson_plan* plan, int enable);
 
 /* "x.y" version string of the library. */
 const char* cans_version(void);

@@ -29,7 +29,6 @@ EXPORTED_SYMBOLS = (
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
     "cans_plan_set_profiling", "cans_plan_kernel_times", "cans_plan_kernel_name",
-    "cans_plan_set_batch", "cans_plan_set_pipeline",
 )
 
 
@@ -70,10 +69,6 @@ def _load() -> ctypes.CDLL:
     lib.cans_plan_launches_per_projection.argtypes = [vp]
     lib.cans_plan_set_profiling.restype = i32
     lib.cans_plan_set_profiling.argtypes = [vp, i32]
-    lib.cans_plan_set_batch.restype = i32
-    lib.cans_plan_set_batch.argtypes = [vp, i32]
-    lib.cans_plan_set_pipeline.restype = i32
-    lib.cans_plan_set_pipeline.argtypes = [vp, i32]
     lib.cans_plan_kernel_times.restype = i32
     lib.cans_plan_kernel_times.argtypes = [vp, ctypes.POINTER(ctypes.c_float), i32]
     lib.cans_plan_kernel_name.restype = ctypes.c_char_p
@@ -194,13 +189,6 @@ class PoissonPlan:
 
     def set_profiling(self, enable: bool):
         _check(_lib.cans_plan_set_profiling(self._h, 1 if enable else 0))
-
-    def set_batch(self, planes: int) -> int:
-        """cans_plan_set_batch: planes per launch of the x / y / correction kernels (0: all planes in one launch)."""
-        return int(_lib.cans_plan_set_batch(self._h, int(planes)))
-
-    def set_pipeline(self, enable: bool) -> bool:
-        return bool(_lib.cans_plan_set_pipeline(self._h, 1 if enable else 0))
 
     def kernel_times(self):
         """[(kernel name, ms)] of the last call, in launch order (profiling must be enabled)."""

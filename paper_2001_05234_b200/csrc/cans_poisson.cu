@@ -10,8 +10,8 @@
 //   a7     grad_correct_kernel                   u -= dt G Phi
 // (xw / yw: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
 //  FFTs for the other lengths.)
-// Plane-batched sequence (cans_plan_set_batch): the same kernels launched per batch of consecutive k-planes, x then y
-// (pass A) and y, x, gradient (pass C), so that the intermediate planes stay in L2 between the launches.
+// Every x / y / correction kernel takes a range of k-planes (XYArgs::k0, nk; GradArgs::k0, k1); the entry points launch each
+// once over all planes -- per-batch launches through L2 were measured and are slower (profiles/r02a_plane_batching.md).
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -132,11 +132,6 @@ struct cans_poisson_plan {
     int num_sms;
     int z_grid;               // persistent grid of the z solve
     size_t z_smem;
-    int batch;                // planes per launch of the x / y / gradient kernels; 0: one launch per step over all planes
-    int pipeline;             // 1: the batches of a pass run on the plan's own streams, consumer kernels one batch behind
-    cudaStream_t lane[3];     // low / mid / high priority (producer ... consumer)
-    cudaEvent_t pev[3][4];    // per lane: ring of "batch done" events
-    cudaEvent_t fork_ev, join_ev;
     unsigned int* sched;      // scheduler state (z tile ticket), zeroed at the start of every call
     size_t sched_bytes;
     std::vector<void*> dev_allocs;
@@ -156,21 +151,20 @@ struct cans_poisson_plan {
     double dzc0;              // dzc[0]: distance from the lower z face's ghost centre to the first centre
     // device buffers for the *_host entry points (lazily allocated)
     double* hostbuf[4];
-    // optional timing (cans_plan_set_profiling): an event pair around every kernel launch (one launch per step) or around
-    // every pass (plane-batched sequence)
+    // optional timing (cans_plan_set_profiling): an event pair around every kernel launch
     int prof;
     int nrec;
     cudaEvent_t ev[2 * MAX_REC];
     const char* kname[MAX_REC];
 };
 
-// bracket one kernel launch (or one pass of batched launches) with events when profiling is on
+// bracket one kernel launch with events when profiling is on
 struct LaunchScope {
     cans_poisson_plan* pl;
     cudaStream_t st;
     bool on;
-    LaunchScope(cans_poisson_plan* p, cudaStream_t s, const char* name, bool enable = true)
-        : pl(p), st(s), on(enable && p->prof && p->nrec < MAX_REC) {
+    LaunchScope(cans_poisson_plan* p, cudaStream_t s, const char* name)
+        : pl(p), st(s), on(p->prof && p->nrec < MAX_REC) {
         if (on) { pl->kname[pl->nrec] = name; cudaEventRecord(pl->ev[2 * pl->nrec], st); }
     }
     ~LaunchScope() {
@@ -234,10 +228,10 @@ static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
 static const char* const XY_NAMES[5] = {"x_fwd", "x_fwd_div", "x_inv", "y_fwd", "y_inv"};
 
 // one x / y transform launch over the planes [a.k0, a.k0 + a.nk)
-static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, cudaStream_t st, bool record) {
+static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, cudaStream_t st) {
     cudaError_t err = cudaSuccess;
     const bool xdir = (op == OP_X_FWD || op == OP_X_FWD_DIV || op == OP_X_INV);
-    LaunchScope scope(pl, st, XY_NAMES[op], record);
+    LaunchScope scope(pl, st, XY_NAMES[op]);
     bool done = false;
     if (xdir && pl->use_xw) done = xw_launch(n, op, a, pl->tw2_x, st, &err);
     else if (!xdir && pl->use_yt) done = yt_launch(n, op, a, pl->tw2_y, &pl->tmap_y, pl->num_sms, st, &err);
@@ -278,12 +272,6 @@ void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
     for (void* d : plan->dev_allocs) cudaFree(d);
     for (int i = 0; i < 4; ++i) if (plan->hostbuf[i]) cudaFree(plan->hostbuf[i]);
     if (plan->prof) for (int i = 0; i < 2 * MAX_REC; ++i) cudaEventDestroy(plan->ev[i]);
-    for (int l = 0; l < 3; ++l) {
-        if (plan->lane[l]) cudaStreamDestroy(plan->lane[l]);
-        for (int i = 0; i < 4; ++i) if (plan->pev[l][i]) cudaEventDestroy(plan->pev[l][i]);
-    }
-    if (plan->fork_ev) cudaEventDestroy(plan->fork_ev);
-    if (plan->join_ev) cudaEventDestroy(plan->join_ev);
     delete plan;
 }
 
@@ -331,10 +319,6 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     for (int i = 0; i < 3; ++i) pl->face[i] = nullptr;
     pl->dzc0 = hdzc[0];
     pl->prof = 0; pl->nrec = 0;
-    pl->batch = 0;
-    pl->pipeline = 0;
-    for (int l = 0; l < 3; ++l) { pl->lane[l] = nullptr; for (int i = 0; i < 4; ++i) pl->pev[l][i] = nullptr; }
-    pl->fork_ev = pl->join_ev = nullptr;
     pl->tmap_field = nullptr;
     pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
     pl->device = 0;
@@ -414,13 +398,10 @@ static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
     return CANS_OK;
 }
 
-// a7 on the planes [k0, k1)
-static int launch_grad(cans_poisson_plan* pl, GradArgs g, int k0, int k1, cudaStream_t st, bool record) {
-    if (k1 <= k0) return CANS_OK;
-    g.k0 = k0; g.k1 = k1;
+static int launch_grad(cans_poisson_plan* pl, const GradArgs& g, cudaStream_t st) {
     const size_t cols = (size_t)pl->nx / 2 * pl->ny;
-    dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((k1 - k0 + GRAD_KC - 1) / GRAD_KC));
-    LaunchScope scope(pl, st, "grad_correct", record);
+    dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((g.k1 - g.k0 + GRAD_KC - 1) / GRAD_KC));
+    LaunchScope scope(pl, st, "grad_correct");
     grad_correct_kernel<<<grid, 256, 0, st>>>(g);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
@@ -437,65 +418,6 @@ static int ensure_tensor_maps(cans_poisson_plan* pl, double* p) {
     return CANS_OK;
 }
 
-// Plane-batched passes on the plan's own streams: the producer of batch b+1 (x forward / y inverse) overlaps the consumer of
-// batch b (y forward / x inverse / correction), so that the drain of one short kernel is filled by the next one's CTAs;
-// a producer runs at most two batches ahead of its consumer, which bounds the intermediate planes waiting in L2.
-static int run_pipelined(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st, int B) {
-    int rc;
-    const int nz = pl->nz;
-    cudaStream_t lo = pl->lane[0], mid = pl->lane[1], hi = pl->lane[2];
-    auto ck = [&](cudaError_t e) { return e == cudaSuccess ? CANS_OK : fail_cuda(e, "pipeline event"); };
-    XYArgs ax = divargs ? *divargs : make_xyargs(pl, p, true);
-    XYArgs ay = make_xyargs(pl, p, false);
-    const int opx = divargs ? OP_X_FWD_DIV : OP_X_FWD;
-    {   // pass A: x(b) on the low lane, y(b) on the high lane
-        LaunchScope scope(pl, st, divargs ? "pass_a_div" : "pass_a");
-        if ((rc = ck(cudaEventRecord(pl->fork_ev, st)))) return rc;
-        if ((rc = ck(cudaStreamWaitEvent(lo, pl->fork_ev, 0)))) return rc;
-        int b = 0;
-        for (int k0 = 0; k0 < nz; k0 += B, ++b) {
-            ax.k0 = ay.k0 = k0;
-            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
-            if (b >= 2 && (rc = ck(cudaStreamWaitEvent(lo, pl->pev[2][(b - 2) & 3], 0)))) return rc;
-            if ((rc = launch_xy_any(pl, pl->nx, opx, ax, lo, false))) return rc;
-            if ((rc = ck(cudaEventRecord(pl->pev[0][b & 3], lo)))) return rc;
-            if ((rc = ck(cudaStreamWaitEvent(hi, pl->pev[0][b & 3], 0)))) return rc;
-            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, ay, hi, false))) return rc;
-            if ((rc = ck(cudaEventRecord(pl->pev[2][b & 3], hi)))) return rc;
-        }
-        if ((rc = ck(cudaStreamWaitEvent(st, pl->pev[2][(b - 1) & 3], 0)))) return rc;
-    }
-    if ((rc = launch_z(pl, p, st))) return rc;
-    {   // pass C: y inverse (low), x inverse (mid), correction of the planes whose Phi(k+1) exists (high)
-        LaunchScope scope(pl, st, grad ? "pass_c_grad" : "pass_c");
-        if ((rc = ck(cudaEventRecord(pl->fork_ev, st)))) return rc;
-        if ((rc = ck(cudaStreamWaitEvent(lo, pl->fork_ev, 0)))) return rc;
-        ax = make_xyargs(pl, p, true);
-        int b = 0;
-        for (int k0 = 0; k0 < nz; k0 += B, ++b) {
-            ax.k0 = ay.k0 = k0;
-            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
-            if (b >= 2 && (rc = ck(cudaStreamWaitEvent(lo, pl->pev[1][(b - 2) & 3], 0)))) return rc;
-            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, ay, lo, false))) return rc;
-            if ((rc = ck(cudaEventRecord(pl->pev[0][b & 3], lo)))) return rc;
-            if ((rc = ck(cudaStreamWaitEvent(mid, pl->pev[0][b & 3], 0)))) return rc;
-            if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, ax, mid, false))) return rc;
-            if ((rc = ck(cudaEventRecord(pl->pev[1][b & 3], mid)))) return rc;
-            if (grad) {
-                const int g0 = k0 > 0 ? k0 - 1 : 0;
-                const int g1 = (k0 + ax.nk == nz) ? nz : k0 + ax.nk - 1;
-                if ((rc = ck(cudaStreamWaitEvent(hi, pl->pev[1][b & 3], 0)))) return rc;
-                if ((rc = launch_grad(pl, *grad, g0, g1, hi, false))) return rc;
-            }
-        }
-        if (grad) {
-            if ((rc = ck(cudaEventRecord(pl->join_ev, hi)))) return rc;
-            if ((rc = ck(cudaStreamWaitEvent(st, pl->join_ev, 0)))) return rc;
-        } else if ((rc = ck(cudaStreamWaitEvent(st, pl->pev[1][(b - 1) & 3], 0)))) return rc;
-    }
-    return CANS_OK;
-}
-
 // the whole path shared by both entry points; `divargs` selects the fused-divergence load (a1),
 // `grad` the velocity correction (a7)
 static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st) {
@@ -507,77 +429,21 @@ static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, con
     cudaError_t me = cudaMemsetAsync(pl->sched, 0, pl->sched_bytes, st);
     if (me != cudaSuccess) return fail_cuda(me, "scheduler reset");
     if ((rc = ensure_tensor_maps(pl, p))) return rc;
-    const int nz = pl->nz;
-    const int B = (pl->batch > 0 && pl->batch < nz) ? pl->batch : nz;
-    const bool batched = B < nz;
-    XYArgs ax = divargs ? *divargs : make_xyargs(pl, p, true);
-    XYArgs ay = make_xyargs(pl, p, false);
-    const int opx = divargs ? OP_X_FWD_DIV : OP_X_FWD;
-    if (batched && pl->pipeline) return run_pipelined(pl, p, divargs, grad, st, B);
-    {   // pass A: (a1 +) a2, a3 per batch of planes
-        LaunchScope scope(pl, st, divargs ? "pass_a_div" : "pass_a", batched);
-        for (int k0 = 0; k0 < nz; k0 += B) {
-            ax.k0 = ay.k0 = k0;
-            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
-            if ((rc = launch_xy_any(pl, pl->nx, opx, ax, st, !batched))) return rc;
-            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, ay, st, !batched))) return rc;
-        }
-    }
-    if ((rc = launch_z(pl, p, st))) return rc;          // pass B: a4
-    {   // pass C: a5, a6 (, a7) per batch of planes; the correction of plane k needs Phi(k+1), so it trails by one plane
-        LaunchScope scope(pl, st, grad ? "pass_c_grad" : "pass_c", batched);
-        ax = make_xyargs(pl, p, true);
-        for (int k0 = 0; k0 < nz; k0 += B) {
-            ax.k0 = ay.k0 = k0;
-            ax.nk = ay.nk = (k0 + B < nz) ? B : nz - k0;
-            if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, ay, st, !batched))) return rc;
-            if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, ax, st, !batched))) return rc;
-            if (grad && batched) {
-                const int g0 = k0 > 0 ? k0 - 1 : 0;
-                const int g1 = (k0 + ax.nk == nz) ? nz : k0 + ax.nk - 1;
-                if ((rc = launch_grad(pl, *grad, g0, g1, st, false))) return rc;
-            }
-        }
-    }
-    if (grad && !batched) return launch_grad(pl, *grad, 0, nz, st, true);
+    const XYArgs ax = make_xyargs(pl, p, true), ay = make_xyargs(pl, p, false);
+    if (divargs) rc = launch_xy_any(pl, pl->nx, OP_X_FWD_DIV, *divargs, st);      // a1 + a2
+    else rc = launch_xy_any(pl, pl->nx, OP_X_FWD, ax, st);                          // a2
+    if (rc) return rc;
+    if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, ay, st))) return rc;              // a3
+    if ((rc = launch_z(pl, p, st))) return rc;                                      // a4
+    if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, ay, st))) return rc;              // a5
+    if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, ax, st))) return rc;              // a6
+    if (grad) return launch_grad(pl, *grad, st);                                    // a7
     return CANS_OK;
 }
 
-int cans_plan_set_batch(cans_poisson_plan* plan, int planes) {
-    g_status = CANS_OK;
-    if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
-    plan->batch = (planes > 0 && planes < plan->nz) ? planes : 0;
-    return plan->batch;
-}
-
-int cans_plan_set_pipeline(cans_poisson_plan* plan, int enable) {
-    g_status = CANS_OK;
-    if (!plan) { fail(CANS_ERR_INVALID_ARG, "plan is NULL"); return 0; }
-    if (enable && !plan->lane[0]) {
-        int least = 0, greatest = 0;
-        cudaError_t e = cudaDeviceGetStreamPriorityRange(&least, &greatest);
-        for (int l = 0; l < 3 && e == cudaSuccess; ++l) {
-            int prio = least - l;                          // numerically lower = higher priority
-            if (prio < greatest) prio = greatest;
-            e = cudaStreamCreateWithPriority(&plan->lane[l], cudaStreamNonBlocking, prio);
-            for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&plan->pev[l][i], cudaEventDisableTiming);
-        }
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->fork_ev, cudaEventDisableTiming);
-        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&plan->join_ev, cudaEventDisableTiming);
-        if (e != cudaSuccess) { fail_cuda(e, "pipeline streams"); return 0; }
-    }
-    plan->pipeline = enable ? 1 : 0;
-    return plan->pipeline;
-}
-
-static int batches_of(const cans_poisson_plan* plan) {
-    if (!plan || plan->batch <= 0) return 1;
-    return (plan->nz + plan->batch - 1) / plan->batch;
-}
-int cans_plan_launches_per_solve(const cans_poisson_plan* plan) { return 4 * batches_of(plan) + 1; }
+int cans_plan_launches_per_solve(const cans_poisson_plan*) { return 5; }
 int cans_plan_launches_per_projection(const cans_poisson_plan* plan) {
-    const int nb = batches_of(plan);
-    int n = 4 * nb + 1 + (nb > 1 ? nb : 1);
+    int n = 6;
     if (plan)
         for (int d = 0; d < 3; ++d) n += (plan->bc[d][0] == 'D' && plan->face[d]) ? 1 : 0;   // lower-face corrections
     return n;

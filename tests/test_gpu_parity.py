@@ -418,37 +418,3 @@ def test_z_tiles_of_16_columns_every_z_pair(B, nz):
                 for d in fd:
                     check_field(np_of(fd[d]), fn[d], what=f"face {d} nz={nz}")
             plan.close()
-
-
-@pytest.mark.parametrize("nx,ny,nz", [(1024, 768, 24), (512, 512, 17), (256, 128, 33), (768, 1024, 9), (96, 64, 40)])
-@pytest.mark.parametrize("batch", [1, 4, 5])
-def test_plane_batched_launches_are_bit_identical(B, nx, ny, nz, batch):
-    """cans_plan_set_batch only changes how many planes one launch covers: the batched sequence (x then y per batch;
-    y, x, then the correction trailing by one plane) must return the same bits as one launch per step, for the Poisson
-    solve and the projection, including batches that do not divide nz and lower-face planes."""
-    lx, ly, lz = 2 * np.pi, np.pi, 2.0
-    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
-    for bc in ((("P", "P"), ("P", "P"), ("N", "N")), (("N", "N"), ("D", "D"), ("D", "N"))):
-        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc_t, dzf_t)
-        g = torch.Generator(device="cuda").manual_seed(nx + nz)
-        f, u0, v0, w0 = (torch.randn((nz, ny, nx), dtype=torch.float64, device="cuda", generator=g) for _ in range(4))
-        shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
-        faces0 = {d: torch.randn(shapes[d], dtype=torch.float64, device="cuda", generator=g) for d in range(3) if bc[d][0] == "D"}
-        results = []
-        for b, pipe in ((0, False), (batch, False), (batch, True)):
-            assert plan.set_batch(b) == (b if b < nz else 0)
-            assert plan.set_pipeline(pipe) == pipe
-            p = f.clone()
-            plan.poisson_solve(p)
-            u, v, w = u0.clone(), v0.clone(), w0.clone()
-            faces = {d: t.clone() for d, t in faces0.items()}
-            for d, t in faces.items():
-                plan.set_lower_face(d, t)
-            phi = torch.empty_like(u)
-            plan.projection(u, v, w, phi, 1e-3)
-            torch.cuda.synchronize()
-            results.append((p, u, v, w, phi, *faces.values()))
-        for other in results[1:]:
-            for a, b_ in zip(results[0], other):
-                assert torch.equal(a, b_)
-        plan.close()
