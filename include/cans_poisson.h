@@ -49,13 +49,15 @@ typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the li
  *   nx, ny, nz   cells per direction (x, y uniform: "uniformly-spaced in two directions").
  *                nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048
  *                (512, 768 and 1024 run the warp-level 2-pass kernels, the others the 3-pass kernels);
- *                2 <= nz <= 1024.
+ *                2 <= nz <= 1024 (periodic z: <= 960).
  *   lx, ly, lz   domain lengths (> 0); dx = lx/nx, dy = ly/ny.
  *   bc           bc[d][0] / bc[d][1] = PRESSURE boundary condition on the lower / upper face of
  *                direction d (0 = x, 1 = y, 2 = z), homogeneous, imposed at the boundary face:
  *                'P' periodic (both sides), 'N' dPhi/dn = 0, 'D' Phi = 0.
- *                Implemented: x, y in {PP, NN, DD}; z in {NN, DD, ND, DN}.
- *                Mixed N/D pairs in x, y and periodic z return NULL with CANS_ERR_UNSUPPORTED_BC.
+ *                Implemented: x, y in {PP, NN, DD}; z in {NN, DD, ND, DN, PP}.  Periodic z (the triperiodic
+ *                Taylor-Green case) solves cyclic tridiagonal systems; for the projection to stay exact its
+ *                wrap spacing must be single-valued, dzc[0] == dzc[nz] (uniform grids satisfy this).
+ *                Mixed N/D pairs in x, y return NULL with CANS_ERR_UNSUPPORTED_BC.
  *   dzc          HOST, nz+1 doubles: dzc[k] = distance between the centres of cells k-1 and k
  *                (k = 0 and k = nz reach the mirror ghost centres), or NULL.
  *   dzf          HOST, nz doubles: dzf[k] = width of cell k, or NULL.  Both NULL => uniform lz/nz.

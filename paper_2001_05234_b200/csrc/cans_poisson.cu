@@ -127,6 +127,8 @@ struct cans_poisson_plan {
     char bc[3][2];
     int kind_x, kind_y;
     int singular;
+    int cyclic;               // z periodic: cyclic tridiagonal systems (z_pass.cuh)
+    double a0w, cw;           // their wrap couplings
     int nseg, nzp;
     int device;               // the device the plan was created on (tables, kernel attributes)
     int num_sms;
@@ -210,6 +212,7 @@ static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
     const int tc = z_tc_for(pl->nseg);
     z.ntiles = (z.ncols + tc - 1) / tc;
     z.ticket = pl->sched + SCHED_Z_TICKET;
+    z.cyclic = pl->cyclic; z.a0w = pl->a0w; z.cw = pl->cw;
     return z;
 }
 
@@ -295,7 +298,6 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         fail(CANS_ERR_UNSUPPORTED_BC, "mixed Neumann/Dirichlet pairs in x or y are not implemented (DCT-IV/DST-IV)");
         return nullptr;
     }
-    if (bc[2][0] == 'P') { fail(CANS_ERR_UNSUPPORTED_BC, "periodic z is not implemented (cyclic tridiagonal)"); return nullptr; }
     FftRadices fx, fy;
     if (!fft_lookup(nx, &fx) || !fft_lookup(ny, &fy)) {
         fail(CANS_ERR_UNSUPPORTED_SIZE, "nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048");
@@ -303,6 +305,10 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     }
     const int nseg = (nz + Z_MROWS - 1) / Z_MROWS;
     if (nseg > 64) { fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the z-solve tiling (max 1024)"); return nullptr; }
+    if (z_solve_smem_bytes(nseg, bc[2][0] == 'P') > Z_SMEM_LIMIT) {
+        fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the periodic z solve (three tile buffers in shared memory: max 960)");
+        return nullptr;
+    }
     std::vector<double> hdzc(nz + 1), hdzf(nz);
     for (int k = 0; k < nz; ++k) hdzf[k] = dzf ? dzf[k] : lz / nz;
     for (int k = 0; k <= nz; ++k) hdzc[k] = dzc ? dzc[k] : lz / nz;
@@ -320,7 +326,8 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->dzc0 = hdzc[0];
     pl->prof = 0; pl->nrec = 0;
     pl->tmap_field = nullptr;
-    pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] == 'N' && bc[2][1] == 'N';
+    pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] != 'D' && bc[2][1] != 'D';
+    pl->cyclic = bc[2][0] == 'P';
     pl->device = 0;
     cudaGetDevice(&pl->device);
     pl->num_sms = 148;
@@ -329,6 +336,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     const double dx = lx / nx, dy = ly / ny;
     ZRows zr = make_z_rows(nz, pl->nzp, hdzc.data(), hdzf.data(), bc[2][0], bc[2][1]);
     pl->inv_lz = 1.0 / zr.lz_sum;
+    pl->a0w = zr.a0w; pl->cw = zr.cw;
     std::vector<double> rdzc(nz);
     for (int k = 0; k < nz; ++k) rdzc[k] = 1.0 / hdzc[k + 1];
 
@@ -375,9 +383,9 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         ZArgs z = make_zargs(pl, nullptr);
         e = z_setup_launch(z, pl->rstart, pl->r00);
     }
-    if (e == cudaSuccess) e = z_solve_configure(nseg, nz, pl->num_sms, &pl->z_grid, &pl->z_smem);
-    if (e == cudaSuccess) e = configure_kernels(pl);
     const int rc = CANS_OK;
+    if (e == cudaSuccess) e = z_solve_configure(nseg, pl->cyclic, pl->num_sms, &pl->z_grid, &pl->z_smem);
+    if (e == cudaSuccess) e = configure_kernels(pl);
     if (e != cudaSuccess || rc != CANS_OK) {
         const bool oom = (e == cudaErrorMemoryAllocation);
         std::string msg = (rc != CANS_OK) ? g_err : std::string("plan creation: ") + cudaGetErrorString(e);

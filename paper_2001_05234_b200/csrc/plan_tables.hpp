@@ -126,9 +126,11 @@ inline std::vector<double> make_lambda_positions(int n, int kind, double h) {
 struct ZRows {
     std::vector<double> a, b, c, g, rdzf, dzf;   // a,b,c,g padded to nzp; rdzf, dzf of length nz
     double lz_sum;
+    double a0w, cw;                              // a_0 and c_{nz-1} before they were zeroed
 };
 
-// lo / up: 'N' or 'D'.  nzp >= nz: rows beyond nz are decoupled identity-like rows (a = c = g = 0, b = -1).
+// lo / up: 'N' or 'D', or both 'P' (cyclic system: no boundary folding, the wrap couplings a_0 and c_{nz-1} are returned
+// separately and zeroed in the rows).  nzp >= nz: rows beyond nz are decoupled identity-like rows (a = c = g = 0, b = -1).
 inline ZRows make_z_rows(int nz, int nzp, const double* dzc, const double* dzf, char lo, char up) {
     ZRows z;
     z.a.assign(nzp, 0.0); z.b.assign(nzp, -1.0); z.c.assign(nzp, 0.0); z.g.assign(nzp, 0.0);
@@ -142,8 +144,12 @@ inline ZRows make_z_rows(int nz, int nzp, const double* dzc, const double* dzf, 
         z.dzf[k] = dzf[k];
         z.lz_sum += dzf[k];
     }
-    z.b[0] += (lo == 'N') ? z.a[0] : -z.a[0];
-    z.b[nz - 1] += (up == 'N') ? z.c[nz - 1] : -z.c[nz - 1];
+    z.a0w = z.a[0];
+    z.cw = z.c[nz - 1];
+    if (lo != 'P') {
+        z.b[0] += (lo == 'N') ? z.a[0] : -z.a[0];
+        z.b[nz - 1] += (up == 'N') ? z.c[nz - 1] : -z.c[nz - 1];
+    }
     z.a[0] = 0.0;
     z.c[nz - 1] = 0.0;
     for (int k = 1; k < nz; ++k) z.g[k] = z.a[k] * z.c[k - 1];

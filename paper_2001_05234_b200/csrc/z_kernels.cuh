@@ -11,8 +11,11 @@ constexpr int Z_MROWS = 16;   // rows per thread in the z solve
 // columns per CTA for a given segment count (threads = TC * nseg <= 512)
 inline int z_tc_for(int nseg) { return nseg <= 16 ? 32 : (nseg <= 32 ? 16 : 8); }
 
+// dynamic shared memory of the solve kernel (the periodic-z kernel keeps a third tile buffer); host arithmetic only
+size_t z_solve_smem_bytes(int nseg, int cyclic);
+constexpr size_t Z_SMEM_LIMIT = 227u * 1024u;
 // plan time: opt in to the dynamic shared memory of the solve kernel and compute the persistent grid
-cudaError_t z_solve_configure(int nseg, int nz, int num_sms, int* grid_out, size_t* smem_out);
+cudaError_t z_solve_configure(int nseg, int cyclic, int num_sms, int* grid_out, size_t* smem_out);   // cudaErrorInvalidConfiguration: the tile buffers do not fit
 // tensor map of the (nz, nx*ny) view of the field p, boxes of z_tc_for(nseg) columns
 cudaError_t z_make_tensor_map(CUtensorMap* tmap, const double* p, long ncols, int nz, int nseg);
 // enqueue the solve (a.ticket must point at a zeroed counter; tmap from z_make_tensor_map for a.p)

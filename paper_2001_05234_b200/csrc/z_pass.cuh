@@ -23,6 +23,13 @@
 //   * results go straight from registers to global memory (coalesced rows).
 // The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_column
 // (CTA 0, before it joins the tile loop).
+//
+// Periodic z (the triperiodic Taylor-Green case of P:L222): the system is cyclic, row 0 couples to
+// x_{nz-1} through a_0 and row nz-1 to x_0 through c_{nz-1}.  Sherman-Morrison on the same partitioned Thomas: with
+// gamma = -(b_0 + lam), the open matrix T' = T - u v^T (u = (gamma, 0, .., 0, c_{nz-1}), v = (1, 0, .., 0, a_0/gamma))
+// has b'_0 = 2 (b_0 + lam) and b'_{nz-1} = b_{nz-1} + lam + c_{nz-1} a_0 / (b_0 + lam); per tile the kernel solves
+// T' q = u (no field data needed: it runs while the tile is still in flight, result kept in a third shared-memory
+// buffer), then T' y = d with the same pivots, and stores x = y - q (y_0 + v_n y_{nz-1}) / (1 + q_0 + v_n q_{nz-1}).
 #pragma once
 #include "common.cuh"
 
@@ -47,6 +54,8 @@ struct ZArgs {
     const double* dzf;        // [nz]
     double inv_lz;            // 1 / sum(dzf)
     unsigned int* ticket;     // tile ticket counter (zeroed before the launch)
+    int cyclic;               // 1: z is periodic (az[0] = cz[nz-1] = 0 in the tables, the wrap couplings are below)
+    double a0w, cw;           // a_0 = 1/(dzf_0 dzc_0) and c_{nz-1} = 1/(dzf_{nz-1} dzc_nz) of the cyclic system
     int nbox, box_rows;       // TMA tiling of a column tile: nbox boxes of box_rows rows (set by z_solve_launch)
 };
 
@@ -54,8 +63,8 @@ struct ZArgs {
 // The reciprocal is the hardware seed (rcp.approx, ~20 bits) refined by two Newton steps: full double precision
 // to about one unit in the last place for these well-scaled, strictly negative denominators, without the range
 // checks and the slow path of the IEEE division -- the pivot chain is the longest dependency chain of the solve.
-CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) {
-    const double den = (bk + lam) - gk * rprev;
+CANS_HD double z_pivot_bl(double bl, double gk, double rprev) {
+    const double den = bl - gk * rprev;
 #if defined(__CUDA_ARCH__)
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(den));
@@ -65,6 +74,15 @@ CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) {
 #else
     return 1.0 / den;
 #endif
+}
+CANS_HD double z_pivot(double bk, double lam, double gk, double rprev) { return z_pivot_bl(bk + lam, gk, rprev); }
+
+// diagonal entry of row k of the cyclic system's open matrix T' (b0 = table entry of row 0)
+CANS_HD double z_cyclic_diag(const ZArgs& a, int k, double bk, double b0, double lam) {
+    double bl = bk + lam;
+    if (k == 0) bl += bl;
+    if (k == a.nz - 1) bl += a.cw * a.a0w / (b0 + lam);
+    return bl;
 }
 
 template <int MROWS>
@@ -78,12 +96,13 @@ struct ZState {
 
 // shared memory (doubles): tables az,bz,cz,gz [4][nzp]; scan arrays end[TC*P], fac[TC*P] of the forward sweep and a
 // second pair for the backward sweep (so that no barrier is needed between reading one and writing the other);
-// two tile buffers [nzp][TC]
+// (y_0, y_{nz-1}) per column of the cyclic solve [2*TC]; two tile buffers [nzp][TC]; cyclic: a third one for q
 template <int MROWS, int TC>
 struct ZPass {
-    static CANS_HD size_t table_doubles(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)4 * TC * nseg; }
+    static CANS_HD size_t edge_offset(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)4 * TC * nseg; }
+    static CANS_HD size_t table_doubles(int nseg) { return edge_offset(nseg) + 2 * TC; }
     static CANS_HD size_t tile_doubles(int nseg) { return (size_t)nseg * MROWS * TC; }
-    static CANS_HD size_t smem_doubles(int nseg) { return table_doubles(nseg) + 2 * tile_doubles(nseg); }
+    static CANS_HD size_t smem_doubles(int nseg, int cyclic) { return table_doubles(nseg) + (2 + (cyclic ? 1 : 0)) * tile_doubles(nseg); }
 
     static CANS_HD void load_tables(const ZArgs& a, double* sm, int tid, int nthreads) {
         const int nzp = a.nseg * MROWS;
@@ -96,7 +115,9 @@ struct ZPass {
     }
 
     // phase 1: take the segment from the tile buffer, pivots, local forward sweep from a zero start;
-    // publish (end, factor)
+    // publish (end, factor).  MODE 0: open system.  Cyclic system: MODE 1 = right-hand side u with the pivots of T'
+    // (no tile data), MODE 2 = the tile's right-hand side with the pivots MODE 1 left in st.r.
+    template <int MODE>
     static CANS_HD void phase1(const ZArgs& a, double* sm, const double* buf, ZState<MROWS>& st, long tile,
                                double rstart_val, double lam, int tid) {
         const int nzp = a.nseg * MROWS;
@@ -114,14 +135,17 @@ struct ZPass {
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
                 const int k = k0 + r;
-                st.d[r] = (k < a.nz) ? buf[(size_t)k * TC + c] * a.scale : 0.0;
+                if (MODE == 1) st.d[r] = (k == 0) ? -(sbz[0] + lam) : ((k == a.nz - 1) ? a.cw : 0.0);
+                else st.d[r] = (k < a.nz) ? buf[(size_t)k * TC + c] * a.scale : 0.0;
             }
             double rp = rstart_val;
             double dp = 0.0, fac = 1.0;
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
                 const int k = k0 + r;
-                rp = z_pivot(sbz[k], lam, sgz[k], rp);
+                if (MODE == 0) rp = z_pivot(sbz[k], lam, sgz[k], rp);
+                else if (MODE == 1) rp = z_pivot_bl(z_cyclic_diag(a, k, sbz[k], sbz[0], lam), sgz[k], rp);
+                else rp = st.r[r];
                 st.r[r] = rp;
                 const double e = saz[k] * rp;
                 dp = st.d[r] * rp - e * dp;
@@ -179,8 +203,10 @@ struct ZPass {
         }
     }
 
-    // phase 3: scan from the bottom -> true x below the segment; propagate; store
-    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
+    // phase 3: scan from the bottom -> true x below the segment; propagate; DEST 0: store to the field (open system),
+    // 1: store to the shared-memory buffer qbuf (cyclic: the correction vector q), 2: keep in st.d (cyclic: y)
+    template <int DEST>
+    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, double* qbuf = nullptr) {
         const int nzp = a.nseg * MROWS;
         const double* scz = sm + 2 * nzp;
         const double2* s_scan = reinterpret_cast<const double2*>(sm + 4 * nzp + 2 * TC * a.nseg);   // backward pairs
@@ -193,7 +219,7 @@ struct ZPass {
             const double2 ef = s_scan[q * TC + c];
             X = ef.x + ef.y * X;
         }
-        if (st.active) {
+        if (DEST == 0 ? st.active : (st.col < a.ncols)) {
             const size_t plane = (size_t)a.ncols;
             double g = 1.0;
 #pragma unroll
@@ -201,11 +227,46 @@ struct ZPass {
                 g *= -(scz[k0 + r] * st.r[r]);
                 st.d[r] += g * X;
             }
+            if (DEST == 0) {
 #pragma unroll
-            for (int r = 0; r < MROWS; ++r) {
-                const int k = k0 + r;
-                if (k < a.nz) a.p[(size_t)k * plane + st.col] = st.d[r];
+                for (int r = 0; r < MROWS; ++r) {
+                    const int k = k0 + r;
+                    if (k < a.nz) a.p[(size_t)k * plane + st.col] = st.d[r];
+                }
+            } else if (DEST == 1) {
+#pragma unroll
+                for (int r = 0; r < MROWS; ++r) qbuf[(size_t)(k0 + r) * TC + c] = st.d[r];
             }
+        }
+    }
+
+    // cyclic system, after phase3<2>: publish y_0 and y_{nz-1} of the column ...
+    static CANS_HD void cyclic_publish(const ZArgs& a, double* sm, const ZState<MROWS>& st, int tid) {
+        double* edge = sm + edge_offset(a.nseg);
+        const int c = tid % TC;
+        const int s = tid / TC;
+        if (s == 0) edge[2 * c] = st.d[0];
+        if (s == (a.nz - 1) / MROWS) {
+            double yn = 0.0;
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) if (s * MROWS + r == a.nz - 1) yn = st.d[r];
+            edge[2 * c + 1] = yn;
+        }
+    }
+    // ... and (behind a barrier) combine: x = y - q (y_0 + v y_n) / (1 + q_0 + v q_n), v = a_0 / gamma
+    static CANS_HD void cyclic_store(const ZArgs& a, double* sm, const ZState<MROWS>& st, double lam, int tid, const double* qbuf) {
+        if (!st.active) return;
+        const double* edge = sm + edge_offset(a.nseg);
+        const int nzp = a.nseg * MROWS;
+        const int c = tid % TC;
+        const int k0 = (tid / TC) * MROWS;
+        const double v = a.a0w / -(sm[nzp] + lam);                     // sm[nzp] = bz[0]
+        const double fact = (edge[2 * c] + v * edge[2 * c + 1]) / (1.0 + qbuf[c] + v * qbuf[(size_t)(a.nz - 1) * TC + c]);
+        const size_t plane = (size_t)a.ncols;
+#pragma unroll
+        for (int r = 0; r < MROWS; ++r) {
+            const int k = k0 + r;
+            if (k < a.nz) a.p[(size_t)k * plane + st.col] = st.d[r] - qbuf[(size_t)k * TC + c] * fact;
         }
     }
 };
@@ -220,8 +281,14 @@ CANS_HD void z_setup_column(const ZArgs& a, double* rstart_out, double* r00_out,
     const int nzp = a.nseg * MROWS;
     for (int k = 0; k < nzp; ++k) {
         if (k % MROWS == 0) rstart_out[(size_t)(k / MROWS) * a.ncols + col] = rp;
-        rp = z_pivot(a.bz[k], lam, a.gz[k], rp);
-        if (col == 0 && k < a.nz && r00_out) r00_out[k] = rp;
+        if (a.cyclic) rp = z_pivot_bl(z_cyclic_diag(a, k, a.bz[k], a.bz[0], lam), a.gz[k], rp);
+        else rp = z_pivot(a.bz[k], lam, a.gz[k], rp);
+        if (col == 0 && k < a.nz && r00_out && !a.cyclic) r00_out[k] = rp;
+    }
+    if (col == 0 && r00_out && a.cyclic) {
+        // singular column of a periodic-z problem: the open system of rows 0..nz-2 with the unmodified diagonal
+        rp = 0.0;
+        for (int k = 0; k < a.nz; ++k) { rp = z_pivot(a.bz[k], 0.0, a.gz[k], rp); r00_out[k] = rp; }
     }
 }
 

@@ -4,7 +4,7 @@
 
 namespace cans {
 
-template <int MROWS, int TC>
+template <int MROWS, int TC, bool CYC>
 __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __grid_constant__ CUtensorMap tmap) {
     extern __shared__ __align__(128) double zsm[];
     typedef ZPass<MROWS, TC> Z;
@@ -14,6 +14,7 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
     const int nthreads = blockDim.x;
     double* bufs = zsm + Z::table_doubles(a.nseg);
     const size_t tile_sz = Z::tile_doubles(a.nseg);
+    double* qbuf = bufs + 2 * tile_sz;          // cyclic systems only
 
     if (a.singular && blockIdx.x == 0) {
         // the singular (0,0) column, staged in shared memory, solved by one thread (reading S3)
@@ -75,17 +76,34 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
         if (tid == 0 && nxt < a.ntiles) issue_tile(nxt, b ^ 1);
         double rs_n, l1_n, l2_n;
         tile_scalars(nxt, rs_n, l1_n, l2_n);   // consumed in the next iteration
+        ZState<MROWS> st;
+        if (CYC) {
+            // the correction vector q of this tile's modes (needs no field data) while the tile is still in flight
+            Z::template phase1<1>(a, zsm, nullptr, st, cur, rs, l1 + l2, tid);
+            __syncthreads();
+            Z::phase2a(a, zsm, st, tid);
+            Z::phase2b(a, zsm, st, tid);
+            __syncthreads();
+            Z::template phase3<1>(a, zsm, st, tid, qbuf);
+        }
         mbar_wait(&s_bar[b], (phases >> b) & 1u);   // the current tile has landed (the next may still fly)
         phases ^= 1u << b;
-        ZState<MROWS> st;
-        Z::phase1(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2, tid);
+        if (CYC) Z::template phase1<2>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2, tid);
+        else Z::template phase1<0>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2, tid);
         __syncthreads();
         // every thread has read s_next (before the barrier above): thread 0 may now draw the ticket after next
         if (tid == 0 && nxt < a.ntiles) s_next = (long)atomicAdd(a.ticket, 1u);
         Z::phase2a(a, zsm, st, tid);
         Z::phase2b(a, zsm, st, tid);
         __syncthreads();
-        Z::phase3(a, zsm, st, tid);
+        if (CYC) {
+            Z::template phase3<2>(a, zsm, st, tid);
+            Z::cyclic_publish(a, zsm, st, tid);
+            __syncthreads();
+            Z::cyclic_store(a, zsm, st, l1 + l2, tid, qbuf);
+        } else {
+            Z::template phase3<0>(a, zsm, st, tid);
+        }
         if (nxt >= a.ntiles) break;
         cur = nxt;
         rs = rs_n; l1 = l1_n; l2 = l2_n;
@@ -99,14 +117,14 @@ __global__ void z_setup_kernel(const ZArgs a, double* rstart, double* r00) {
     if (col < a.ncols) z_setup_column<MROWS>(a, rstart, r00, col);
 }
 
-template <int TC>
-static cudaError_t configure_tc(int nseg, int nz, int num_sms, int* grid_out, size_t* smem_out) {
-    size_t smem = sizeof(double) * ZPass<Z_MROWS, TC>::smem_doubles(nseg);
-    (void)nz;
-    cudaError_t e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, TC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+template <int TC, bool CYC>
+static cudaError_t configure_tc(int nseg, int num_sms, int* grid_out, size_t* smem_out) {
+    size_t smem = sizeof(double) * ZPass<Z_MROWS, TC>::smem_doubles(nseg, CYC ? 1 : 0);
+    if (smem > Z_SMEM_LIMIT) return cudaErrorInvalidConfiguration;       // the plan checks z_solve_smem_bytes first
+    cudaError_t e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, TC, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, z_solve_kernel<Z_MROWS, TC>, TC * nseg, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, z_solve_kernel<Z_MROWS, TC, CYC>, TC * nseg, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     if (per_sm > 4) per_sm = 4;
@@ -115,11 +133,19 @@ static cudaError_t configure_tc(int nseg, int nz, int num_sms, int* grid_out, si
     return cudaSuccess;
 }
 
-cudaError_t z_solve_configure(int nseg, int nz, int num_sms, int* grid_out, size_t* smem_out) {
+size_t z_solve_smem_bytes(int nseg, int cyclic) {
     switch (z_tc_for(nseg)) {
-        case 32: return configure_tc<32>(nseg, nz, num_sms, grid_out, smem_out);
-        case 16: return configure_tc<16>(nseg, nz, num_sms, grid_out, smem_out);
-        default: return configure_tc<8>(nseg, nz, num_sms, grid_out, smem_out);
+        case 32: return sizeof(double) * ZPass<Z_MROWS, 32>::smem_doubles(nseg, cyclic);
+        case 16: return sizeof(double) * ZPass<Z_MROWS, 16>::smem_doubles(nseg, cyclic);
+        default: return sizeof(double) * ZPass<Z_MROWS, 8>::smem_doubles(nseg, cyclic);
+    }
+}
+
+cudaError_t z_solve_configure(int nseg, int cyclic, int num_sms, int* grid_out, size_t* smem_out) {
+    switch (z_tc_for(nseg)) {
+        case 32: return cyclic ? configure_tc<32, true>(nseg, num_sms, grid_out, smem_out) : configure_tc<32, false>(nseg, num_sms, grid_out, smem_out);
+        case 16: return cyclic ? configure_tc<16, true>(nseg, num_sms, grid_out, smem_out) : configure_tc<16, false>(nseg, num_sms, grid_out, smem_out);
+        default: return cyclic ? configure_tc<8, true>(nseg, num_sms, grid_out, smem_out) : configure_tc<8, false>(nseg, num_sms, grid_out, smem_out);
     }
 }
 
@@ -146,11 +172,11 @@ cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, const CUten
     if (g > a.ntiles) g = a.ntiles;
     if (g < 1) g = 1;
     z_boxes(a.nseg, &a.nbox, &a.box_rows);
-    switch (z_tc_for(a.nseg)) {
-        case 32: z_solve_kernel<Z_MROWS, 32><<<(unsigned)g, 32 * a.nseg, smem, st>>>(a, *tmap); break;
-        case 16: z_solve_kernel<Z_MROWS, 16><<<(unsigned)g, 16 * a.nseg, smem, st>>>(a, *tmap); break;
-        default: z_solve_kernel<Z_MROWS, 8><<<(unsigned)g, 8 * a.nseg, smem, st>>>(a, *tmap); break;
-    }
+    const int tc = z_tc_for(a.nseg);
+#define CANS_Z_LAUNCH(TC, CYC) z_solve_kernel<Z_MROWS, TC, CYC><<<(unsigned)g, TC * a.nseg, smem, st>>>(a, *tmap)
+    if (a.cyclic) { if (tc == 32) CANS_Z_LAUNCH(32, true); else if (tc == 16) CANS_Z_LAUNCH(16, true); else CANS_Z_LAUNCH(8, true); }
+    else { if (tc == 32) CANS_Z_LAUNCH(32, false); else if (tc == 16) CANS_Z_LAUNCH(16, false); else CANS_Z_LAUNCH(8, false); }
+#undef CANS_Z_LAUNCH
     return cudaGetLastError();
 }
 

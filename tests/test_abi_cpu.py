@@ -50,7 +50,7 @@ PP_NN = (("P", "P"), ("P", "P"), ("N", "N"))
     (dict(nx=32, ny=32, nz=32, bc=(("P", "N"), ("P", "P"), ("N", "N"))), 1),      # one-sided periodic
     (dict(nx=32, ny=32, nz=32, bc=(("X", "X"), ("P", "P"), ("N", "N"))), 1),      # unknown letter
     (dict(nx=32, ny=32, nz=32, bc=(("N", "D"), ("P", "P"), ("N", "N"))), 2),      # mixed pair in x (NEXT f2)
-    (dict(nx=32, ny=32, nz=32, bc=(("P", "P"), ("P", "P"), ("P", "P"))), 2),      # periodic z (NEXT f1)
+    (dict(nx=32, ny=32, nz=1000, bc=(("P", "P"), ("P", "P"), ("P", "P"))), 3),    # periodic z: nz <= 960
     (dict(nx=40, ny=32, nz=32), 3),                                                # 40 = 2^3*5
     (dict(nx=32, ny=32, nz=2000), 3),
     (dict(nx=32, ny=32, nz=4, dzf=[0.5, 0.5, -0.5, 0.5], dzc=[0.5] * 5), 1),

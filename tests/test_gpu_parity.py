@@ -85,7 +85,7 @@ def test_config_full_parity(B, name):
 # (nz = 33: three z segments, the last with one row; 48/96: radix-3 lengths; tiles of 16 columns)
 # ----------------------------------------------------------------------------------------------
 XY = ["PP", "NN", "DD"]
-ZP = ["NN", "DD", "ND", "DN"]
+ZP = ["NN", "DD", "ND", "DN", "PP"]       # "PP": cyclic tridiagonal systems
 
 
 @pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 96, 33, 1.6), (128, 32, 40, None), (16, 16, 2, None),
@@ -130,7 +130,8 @@ def test_every_transform_length_in_x_and_y(B, n):
 # projection (eqs. 2b-2c) against the oracle, plus its invariants evaluated with the oracle's operators
 # ----------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("px,py,pz", [("PP", "PP", "NN"), ("PP", "NN", "NN"), ("NN", "NN", "NN"),
-                                      ("PP", "PP", "ND"), ("NN", "PP", "NN")])
+                                      ("PP", "PP", "ND"), ("NN", "PP", "NN"),
+                                      ("PP", "PP", "PP"), ("NN", "PP", "PP"), ("PP", "NN", "PP")])
 def test_projection_parity_and_invariants(B, px, py, pz):
     nx, ny, nz = 96, 64, 40
     lx, ly, lz = 2 * np.pi, np.pi, 2.0
@@ -418,3 +419,22 @@ def test_z_tiles_of_16_columns_every_z_pair(B, nz):
                 for d in fd:
                     check_field(np_of(fd[d]), fn[d], what=f"face {d} nz={nz}")
             plan.close()
+
+
+@pytest.mark.parametrize("nz", [960, 513])
+def test_tallest_periodic_columns(B, nz):
+    """Periodic z keeps a third tile buffer in shared memory: nz up to 960 (tiles of 8 columns), beyond that the plan refuses."""
+    nx, ny = 48, 32
+    lx, ly, lz = 1.0, 1.0, 2.0
+    for bc in ((("P", "P"), ("P", "P"), ("P", "P")), (("N", "N"), ("D", "D"), ("P", "P"))):
+        f = random_rhs(nx, ny, nz, bc, None, nz + 1)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        torch.cuda.synchronize()
+        plan.close()
+        ref = orc.poisson_solve(f, lx, ly, lz, bc)
+        check_field(np_of(p), ref, what=f"nz={nz} {bc}")
+    with pytest.raises(B.CansError) as ei:
+        B.PoissonPlan(nx, ny, 961, lx, ly, lz, bc)
+    assert ei.value.status == B.CANS_ERR_UNSUPPORTED_SIZE
