@@ -37,7 +37,7 @@ typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the li
 /* Return codes of the int-valued entry points. */
 #define CANS_OK                    0
 #define CANS_ERR_INVALID_ARG       1   /* null pointer, n < 2, non-positive length/spacing/dt, bad bc letter, one-sided 'P' */
-#define CANS_ERR_UNSUPPORTED_BC    2   /* boundary pair the kernels do not implement yet (see cans_poisson_plan_create) */
+#define CANS_ERR_UNSUPPORTED_BC    2   /* reserved (no longer returned: every boundary pair is implemented) */
 #define CANS_ERR_UNSUPPORTED_SIZE  3   /* nx or ny not in the instantiated transform sizes, or nz too large */
 #define CANS_ERR_ALLOC             4   /* device or host allocation failed */
 #define CANS_ERR_CUDA              5   /* a CUDA runtime call or kernel launch failed */
@@ -54,10 +54,10 @@ typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the li
  *   bc           bc[d][0] / bc[d][1] = PRESSURE boundary condition on the lower / upper face of
  *                direction d (0 = x, 1 = y, 2 = z), homogeneous, imposed at the boundary face:
  *                'P' periodic (both sides), 'N' dPhi/dn = 0, 'D' Phi = 0.
- *                Implemented: x, y in {PP, NN, DD}; z in {NN, DD, ND, DN, PP}.  Periodic z (the triperiodic
+ *                Implemented: every pair in every direction -- x, y, z in {PP, NN, DD, ND, DN} ("all combinations of
+ *                pressure boundary conditions"; mixed pairs in x, y run DCT-IV / DST-IV).  Periodic z (the triperiodic
  *                Taylor-Green case) solves cyclic tridiagonal systems; for the projection to stay exact its
  *                wrap spacing must be single-valued, dzc[0] == dzc[nz] (uniform grids satisfy this).
- *                Mixed N/D pairs in x, y return NULL with CANS_ERR_UNSUPPORTED_BC.
  *   dzc          HOST, nz+1 doubles: dzc[k] = distance between the centres of cells k-1 and k
  *                (k = 0 and k = nz reach the mirror ghost centres), or NULL.
  *   dzf          HOST, nz doubles: dzf[k] = width of cell k, or NULL.  Both NULL => uniform lz/nz.

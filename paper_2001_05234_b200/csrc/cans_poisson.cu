@@ -139,7 +139,7 @@ struct cans_poisson_plan {
     std::vector<void*> dev_allocs;
     // device tables
     double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc, *rstart, *r00;
-    cplx *tw_x, *tw_y, *wpost_x, *wpost_y;
+    cplx *tw_x, *tw_y, *wpost_x, *wpost_y, *wpre_x, *wpre_y;
     cplx* tw2_x;              // W_nx^(p k1), [nx/32][32]: warp-per-line x kernels (xw_pass.cuh), or NULL
     int use_xw;               // 1: x transforms run the warp-per-line kernels
     cplx* tw2_y;              // the same for ny (yw_pass.cuh), or NULL
@@ -178,7 +178,9 @@ static int kind_of(char lo, char up, int* kind) {
     if (lo == 'P' && up == 'P') { *kind = KIND_PP; return CANS_OK; }
     if (lo == 'N' && up == 'N') { *kind = KIND_NN; return CANS_OK; }
     if (lo == 'D' && up == 'D') { *kind = KIND_DD; return CANS_OK; }
-    return CANS_ERR_UNSUPPORTED_BC;
+    if (lo == 'N' && up == 'D') { *kind = KIND_ND; return CANS_OK; }
+    if (lo == 'D' && up == 'N') { *kind = KIND_DN; return CANS_OK; }
+    return CANS_ERR_INVALID_ARG;
 }
 
 template <class T>
@@ -224,6 +226,7 @@ static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
     a.kind = xdir ? pl->kind_x : pl->kind_y;
     a.tw = xdir ? pl->tw_x : pl->tw_y;
     a.wpost = xdir ? pl->wpost_x : pl->wpost_y;
+    a.wpre = xdir ? pl->wpre_x : pl->wpre_y;
     a.p = p;
     return a;
 }
@@ -295,7 +298,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
         if ((bc[d][0] == 'P') != (bc[d][1] == 'P')) { fail(CANS_ERR_INVALID_ARG, "periodic boundaries must be two-sided"); return nullptr; }
     int kx, ky;
     if (kind_of(bc[0][0], bc[0][1], &kx) != CANS_OK || kind_of(bc[1][0], bc[1][1], &ky) != CANS_OK) {
-        fail(CANS_ERR_UNSUPPORTED_BC, "mixed Neumann/Dirichlet pairs in x or y are not implemented (DCT-IV/DST-IV)");
+        fail(CANS_ERR_INVALID_ARG, "unknown boundary pair");
         return nullptr;
     }
     FftRadices fx, fy;
@@ -326,7 +329,7 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->dzc0 = hdzc[0];
     pl->prof = 0; pl->nrec = 0;
     pl->tmap_field = nullptr;
-    pl->singular = (kx != KIND_DD) && (ky != KIND_DD) && bc[2][0] != 'D' && bc[2][1] != 'D';
+    pl->singular = (kx == KIND_PP || kx == KIND_NN) && (ky == KIND_PP || ky == KIND_NN) && bc[2][0] != 'D' && bc[2][1] != 'D';
     pl->cyclic = bc[2][0] == 'P';
     pl->device = 0;
     cudaGetDevice(&pl->device);
@@ -348,8 +351,11 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     up(zr.rdzf, &pl->rdzf); up(zr.dzf, &pl->dzf); up(rdzc, &pl->rdzc);
     up(make_pass_twiddles(fx), &pl->tw_x);
     up(make_pass_twiddles(fy), &pl->tw_y);
-    up(make_post_twiddles(nx), &pl->wpost_x);
-    up(make_post_twiddles(ny), &pl->wpost_y);
+    up(kind_mixed(kx) ? make_post_twiddles_mixed(nx) : make_post_twiddles(nx), &pl->wpost_x);
+    up(kind_mixed(ky) ? make_post_twiddles_mixed(ny) : make_post_twiddles(ny), &pl->wpost_y);
+    pl->wpre_x = pl->wpre_y = nullptr;
+    if (kind_mixed(kx)) up(make_pre_twiddles_mixed(nx), &pl->wpre_x);
+    if (kind_mixed(ky)) up(make_pre_twiddles_mixed(ny), &pl->wpre_y);
     pl->tw2_x = nullptr;
     pl->use_xw = 0;
     if (xw_supported(nx)) {

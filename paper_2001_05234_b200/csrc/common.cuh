@@ -50,6 +50,10 @@ CANS_HD double2 ld_p2(const double* p) {
 }
 
 // Transform kind of one direction (pressure boundary pair), see DESIGN.md "Transforms".
-enum Kind : int { KIND_PP = 0, KIND_NN = 1, KIND_DD = 2 };
+// KIND_ND / KIND_DN: the mixed pairs (lower Neumann, upper Dirichlet and the reverse), DCT-IV / DST-IV.
+enum Kind : int { KIND_PP = 0, KIND_NN = 1, KIND_DD = 2, KIND_ND = 3, KIND_DN = 4 };
+CANS_HD bool kind_mixed(int kind) { return kind >= KIND_ND; }
+// odd samples enter the FFT negated
+CANS_HD bool kind_neg_odd(int kind) { return kind == KIND_DD || kind == KIND_ND; }
 
 }  // namespace cans

@@ -98,6 +98,27 @@ inline std::vector<double> make_post_twiddles(int n) {
     return t;
 }
 
+// mixed pairs (DCT-IV / DST-IV): post-twiddles exp(-i pi (2q+1) / (4n)), q = 0..n/2-1 ...
+inline std::vector<double> make_post_twiddles_mixed(int n) {
+    std::vector<double> t;
+    for (int q = 0; q < n / 2; ++q) {
+        double re, im;
+        unit_root(2 * q + 1, 8LL * n, &re, &im);
+        t.push_back(re); t.push_back(im);
+    }
+    return t;
+}
+// ... and pre-twiddles exp(-i pi m / n), m = 0..n-1
+inline std::vector<double> make_pre_twiddles_mixed(int n) {
+    std::vector<double> t;
+    for (int m = 0; m < n; ++m) {
+        double re, im;
+        unit_root(m, 2LL * n, &re, &im);
+        t.push_back(re); t.push_back(im);
+    }
+    return t;
+}
+
 // -4 sin^2(pi num / den)
 inline double lam_sin2(long long num, long long den) {
     double re, im;
@@ -105,10 +126,19 @@ inline double lam_sin2(long long num, long long den) {
     return -4.0 * im * im;
 }
 
-// eigenvalue of the mode stored at every slot position of a line of n (kind: 0 PP, 1 NN, 2 DD), divided by h^2
+// eigenvalue of the mode stored at every slot position of a line of n (kind: 0 PP, 1 NN, 2 DD, 3 ND, 4 DN), divided by h^2
 inline std::vector<double> make_lambda_positions(int n, int kind, double h) {
     std::vector<double> lam(n);
     const double ih2 = 1.0 / (h * h);
+    if (kind >= 3) {
+        // mixed pairs: mode q has -4 sin^2(pi (2q+1) / (4n)); positions (2s, 2s+1) hold modes (s, n-1-s) for ND, (n-1-s, s) for DN
+        for (int s = 0; s < n / 2; ++s) {
+            const double lo = lam_sin2(2LL * s + 1, 4LL * n) * ih2, hi = lam_sin2(2LL * (n - 1 - s) + 1, 4LL * n) * ih2;
+            lam[2 * s] = (kind == 3) ? lo : hi;
+            lam[2 * s + 1] = (kind == 3) ? hi : lo;
+        }
+        return lam;
+    }
     auto mode = [&](int q) -> double {
         if (kind == 0) return lam_sin2(q, n);                 // PP: frequency q
         if (kind == 1) return lam_sin2(q, 2LL * n);           // NN: cosine mode q

@@ -182,7 +182,11 @@ struct XWPass {
             for (int m = 0; m < R1; ++m) {
                 const int i = index_of_elem(lane + 32 * m, a.kind);
                 v[m] = buf[i];
-                if (a.kind == KIND_DD && (i & 1)) v[m] = cneg(v[m]);
+                if (kind_neg_odd(a.kind) && (i & 1)) v[m] = cneg(v[m]);
+            }
+            if (kind_mixed(a.kind)) {
+#pragma unroll
+                for (int m = 0; m < R1; ++m) v[m] = cmul(v[m], __ldg(a.wpre + lane + 32 * m));
             }
         }
         __syncwarp();                                   // natural-order rows fully read: reuse the buffer for the exchange
@@ -206,7 +210,9 @@ struct XWPass {
 #pragma unroll 4
         for (int s = lane; s < H; s += 32) {
             double2 oa, ob;
-            if (s == 0) {
+            if (kind_mixed(a.kind)) {
+                post_forward(buf[s], buf[N - 1 - s], __ldg(a.wpost + s), a.kind, oa.x, oa.y, ob.x, ob.y);
+            } else if (s == 0) {
                 const cplx Z0 = buf[0], Zh = buf[H];
                 const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
                 oa = make_double2(Z0.x, c * Zh.x);
@@ -235,7 +241,12 @@ struct XWPass {
 #pragma unroll
             for (int m = 0; m < NQ; ++m) {
                 const int s = lane + 32 * m;
-                if (s == 0) {
+                if (kind_mixed(a.kind)) {
+                    cplx Zq, Zm;
+                    pre_inverse(ia[m].x, ia[m].y, ib[m].x, ib[m].y, __ldg(a.wpost + s), a.kind, Zq, Zm);
+                    buf[s] = Zq;
+                    buf[N - 1 - s] = Zm;
+                } else if (s == 0) {
                     const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
                     buf[0] = make_double2(ia[m].x, ib[m].x);
                     buf[H] = make_double2(c * ia[m].y, c * ib[m].y);
@@ -279,10 +290,14 @@ struct XWPass {
             return;
         }
         __syncwarp();                                   // exchange buffer fully read: reuse it in natural order
+        if (kind_mixed(a.kind)) {
+#pragma unroll
+            for (int m = 0; m < R1; ++m) v[m] = cmulc(v[m], __ldg(a.wpre + lane + 32 * m));
+        }
 #pragma unroll
         for (int m = 0; m < R1; ++m) {
             const int i = index_of_elem(lane + 32 * m, a.kind);
-            buf[i] = (a.kind == KIND_DD && (i & 1)) ? cneg(v[m]) : v[m];
+            buf[i] = (kind_neg_odd(a.kind) && (i & 1)) ? cneg(v[m]) : v[m];
         }
         __syncwarp();
 #pragma unroll

@@ -7,8 +7,13 @@
 //   NN   : v_j = x_{2j}, v_{n-1-j} = x_{2j+1} (Makhoul's permutation, P:L222 ref [21]);
 //          C_q = Re(w^q V_q), C_{n-q} = -Im(w^q V_q), w = exp(-i pi/(2n))
 //   DD   : x_j -> (-1)^j x_j, then as NN; the slot of C'_q holds sine mode n-1-q.
+//   ND/DN: (mixed pairs, DCT-IV / DST-IV) the same permutation (ND also negates the odd samples), a
+//          pre-twiddle v_m -> v_m exp(-i pi m / n), V = FFT(v): V_{n-1-q} = conj V_q for a real line, and with
+//          G_q = exp(-i pi (2q+1)/(4n)) V_q the coefficients are (Re G_q, -Im G_q) = cosine modes (q, n-1-q) for ND,
+//          sine modes (n-1-q, q) for DN.  The inverse runs the same steps backwards (conjugated).
 // Spectral ("slot") layout of a line of n reals: positions (2s, 2s+1), s = 1..n/2-1, hold
-// (Re A_s, Im A_s) for PP or (C_s, C_{n-s}) for NN/DD; positions (0, 1) hold modes (0, n/2).
+// (Re A_s, Im A_s) for PP or (C_s, C_{n-s}) for NN/DD; positions (0, 1) hold modes (0, n/2).  Mixed pairs: positions
+// (2s, 2s+1), s = 0..n/2-1, hold (Re G_s, -Im G_s).
 // The eigenvalue of every position is tabulated by the plan (plan_tables.hpp), so the layout is private.
 //
 // x pass: the pair is two adjacent rows (j, j+1) of a plane; line index runs along x (contiguous).
@@ -27,7 +32,8 @@ struct XYArgs {
     int k0, nk;             // planes [k0, k0 + nk) handled by this launch (a batch of consecutive k-planes)
     int kind;               // Kind of THIS direction
     const cplx* tw;         // pass twiddles, FftPlan::TW_TOTAL entries
-    const cplx* wpost;      // exp(-i pi q / (2n)), q = 0..n/2-1 (NN / DD only)
+    const cplx* wpost;      // NN / DD: exp(-i pi q / (2n)); ND / DN: exp(-i pi (2q+1) / (4n)); q = 0..n/2-1
+    const cplx* wpre;       // ND / DN only: exp(-i pi m / n), m = 0..n-1
     double* p;              // field transformed in place
     // fused divergence (x forward only): f = (du*rdx + dv*rdy + dw*rdzf[k]) * rdt
     const double* u;
@@ -183,7 +189,10 @@ struct XPass {
                 const int idx = tid + (it0 + u) * NT;
                 const int f = idx / H;
                 const int e2 = idx - f * H;
-                if (idx < NF * H && pair0 + f < npairs) put_forward(sm + f * P::NPAD, e2, va[u], vb[u], a.kind);
+                if (idx < NF * H && pair0 + f < npairs) {
+                    if (kind_mixed(a.kind)) put_forward_mixed(a, sm + f * P::NPAD, e2, va[u], vb[u]);
+                    else put_forward(sm + f * P::NPAD, e2, va[u], vb[u], a.kind);
+                }
             }
         }
     }
@@ -194,9 +203,17 @@ struct XPass {
         cplx z1 = make_double2(va.y, vb.y);      // index 2*e2+1
         int d0, d1;
         if (kind == KIND_PP) { d0 = 2 * e2; d1 = 2 * e2 + 1; }
-        else { d0 = e2; d1 = N - 1 - e2; if (kind == KIND_DD) z1 = cneg(z1); }
+        else { d0 = e2; d1 = N - 1 - e2; if (kind_neg_odd(kind)) z1 = cneg(z1); }
         line[P::pad(d0)] = z0;
         line[P::pad(d1)] = z1;
+    }
+    // the same for the mixed pairs: with the pre-twiddle of the element
+    static CANS_HD void put_forward_mixed(const XYArgs& a, cplx* line, int e2, double2 va, double2 vb) {
+        const cplx z0 = make_double2(va.x, vb.x);
+        cplx z1 = make_double2(va.y, vb.y);
+        if (a.kind == KIND_ND) z1 = cneg(z1);
+        line[P::pad(e2)] = cmul(z0, a.wpre[e2]);
+        line[P::pad(N - 1 - e2)] = cmul(z1, a.wpre[N - 1 - e2]);
     }
 
     // ---- passes ----
@@ -228,7 +245,10 @@ struct XPass {
             const size_t ro = row_offset(a, pr, j, k);
             const cplx* line = sm + f * P::NPAD;
             double2 oa, ob;
-            if (s == 0) {
+            if (kind_mixed(a.kind)) {
+                post_forward(line[P::pad(P::loc_of_freq(s))], line[P::pad(P::loc_of_freq(N - 1 - s))], a.wpost[s], a.kind,
+                             oa.x, oa.y, ob.x, ob.y);
+            } else if (s == 0) {
                 const cplx Z0 = line[P::pad(P::loc_of_freq(0))];
                 const cplx Zh = line[P::pad(P::loc_of_freq(H))];
                 const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
@@ -276,7 +296,12 @@ struct XPass {
 
     // slot s of rows a and b -> Z at the digit-reversed locations
     static CANS_HD void put_inverse(const XYArgs& a, cplx* line, int s, double2 ia, double2 ib) {
-        if (s == 0) {
+        if (kind_mixed(a.kind)) {
+            cplx Zq, Zm;
+            pre_inverse(ia.x, ia.y, ib.x, ib.y, a.wpost[s], a.kind, Zq, Zm);
+            line[P::pad(P::loc_of_freq(s))] = Zq;
+            line[P::pad(P::loc_of_freq(N - 1 - s))] = Zm;
+        } else if (s == 0) {
             const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
             line[P::pad(P::loc_of_freq(0))] = make_double2(ia.x, ib.x);
             line[P::pad(P::loc_of_freq(H))] = make_double2(c * ia.y, c * ib.y);
@@ -303,9 +328,10 @@ struct XPass {
             int d0, d1;
             if (a.kind == KIND_PP) { d0 = 2 * e2; d1 = 2 * e2 + 1; }
             else { d0 = e2; d1 = N - 1 - e2; }
-            const cplx z0 = line[P::pad(d0)];
+            cplx z0 = line[P::pad(d0)];
             cplx z1 = line[P::pad(d1)];
-            if (a.kind == KIND_DD) z1 = cneg(z1);
+            if (kind_mixed(a.kind)) { z0 = cmulc(z0, a.wpre[d0]); z1 = cmulc(z1, a.wpre[d1]); }
+            if (kind_neg_odd(a.kind)) z1 = cneg(z1);
             *reinterpret_cast<double2*>(a.p + ro + 2 * e2) = make_double2(z0.x, z1.x);
             *reinterpret_cast<double2*>(a.p + ro + a.nx + 2 * e2) = make_double2(z0.y, z1.y);
         }
@@ -358,7 +384,8 @@ struct YPass {
 
     static CANS_HD void put_forward(const XYArgs& a, cplx* sm, int j, int f, cplx z) {
         const int e = elem_of_index<N>(j, a.kind);
-        if (a.kind == KIND_DD && (j & 1)) z = cneg(z);
+        if (kind_neg_odd(a.kind) && (j & 1)) z = cneg(z);
+        if (kind_mixed(a.kind)) z = cmul(z, a.wpre[e]);
         sm[e * TXC + f] = z;
     }
 
@@ -384,7 +411,13 @@ struct YPass {
             const int s = idx / TXC;
             const int f = idx - s * TXC;
             double2 r0, r1;   // rows 2s and 2s+1: (column a, column b)
-            if (s == 0) {
+            if (kind_mixed(a.kind)) {
+                double A0, A1, B0, B1;
+                post_forward(sm[P::loc_of_freq(s) * TXC + f], sm[P::loc_of_freq(N - 1 - s) * TXC + f], a.wpost[s], a.kind,
+                             A0, A1, B0, B1);
+                r0 = make_double2(A0, B0);
+                r1 = make_double2(A1, B1);
+            } else if (s == 0) {
                 const cplx Z0 = sm[P::loc_of_freq(0) * TXC + f];
                 const cplx Zh = sm[P::loc_of_freq(H) * TXC + f];
                 const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
@@ -432,7 +465,12 @@ struct YPass {
     }
 
     static CANS_HD void put_inverse(const XYArgs& a, cplx* sm, int s, int f, double2 r0, double2 r1) {
-        if (s == 0) {
+        if (kind_mixed(a.kind)) {
+            cplx Zq, Zm;
+            pre_inverse(r0.x, r1.x, r0.y, r1.y, a.wpost[s], a.kind, Zq, Zm);
+            sm[P::loc_of_freq(s) * TXC + f] = Zq;
+            sm[P::loc_of_freq(N - 1 - s) * TXC + f] = Zm;
+        } else if (s == 0) {
             const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
             sm[P::loc_of_freq(0) * TXC + f] = make_double2(r0.x, r0.y);
             sm[P::loc_of_freq(H) * TXC + f] = make_double2(c * r1.x, c * r1.y);
@@ -453,7 +491,8 @@ struct YPass {
             const int f = idx - j * TXC;
             const int e = elem_of_index<N>(j, a.kind);
             cplx z = sm[e * TXC + f];
-            if (a.kind == KIND_DD && (j & 1)) z = cneg(z);
+            if (kind_mixed(a.kind)) z = cmulc(z, a.wpre[e]);
+            if (kind_neg_odd(a.kind) && (j & 1)) z = cneg(z);
             *reinterpret_cast<double2*>(base + (size_t)j * a.nx + 2 * f) = z;
         }
     }

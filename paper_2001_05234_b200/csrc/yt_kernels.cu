@@ -54,9 +54,9 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
         if (INV) {
             W::slots_in(a, T, warp, lane);
             W::column_inverse(T, warp, tw, lane);
-            W::permute_out(T, warp, a.kind, lane);
+            W::permute_out(T, warp, a.kind, a.wpre, lane);
         } else {
-            W::permute_in(T, warp, a.kind, lane);
+            W::permute_in(T, warp, a.kind, a.wpre, lane);
             W::column_forward(T, warp, tw, lane);
             W::slots_out(a, T, warp, lane);
         }

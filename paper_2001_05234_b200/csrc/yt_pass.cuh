@@ -98,7 +98,7 @@ struct YTPass {
     }
 
     // rows j (as loaded) -> FFT input elements e, in place through registers (NN / DD only; PP is the identity)
-    static CANS_D void permute_in(cplx* t, int f, int kind, int lane) {
+    static CANS_D void permute_in(cplx* t, int f, int kind, const cplx* __restrict__ wpre, int lane) {
         if (kind == KIND_PP) return;
         cplx v[R1];
 #pragma unroll
@@ -107,19 +107,24 @@ struct YTPass {
 #pragma unroll
         for (int m = 0; m < R1; ++m) {
             const int j = lane + 32 * m;
-            t[at(elem_of_index<N>(j, kind), f)] = (kind == KIND_DD && (j & 1)) ? cneg(v[m]) : v[m];
+            const int e = elem_of_index<N>(j, kind);
+            cplx z = (kind_neg_odd(kind) && (j & 1)) ? cneg(v[m]) : v[m];
+            if (kind_mixed(kind)) z = cmul(z, __ldg(wpre + e));
+            t[at(e, f)] = z;
         }
         __syncwarp();
     }
     // FFT output elements e -> rows j (inverse of permute_in)
-    static CANS_D void permute_out(cplx* t, int f, int kind, int lane) {
+    static CANS_D void permute_out(cplx* t, int f, int kind, const cplx* __restrict__ wpre, int lane) {
         if (kind == KIND_PP) return;
         cplx v[R1];
 #pragma unroll
         for (int m = 0; m < R1; ++m) {
             const int j = lane + 32 * m;
-            const cplx z = t[at(elem_of_index<N>(j, kind), f)];
-            v[m] = (kind == KIND_DD && (j & 1)) ? cneg(z) : z;
+            const int e = elem_of_index<N>(j, kind);
+            cplx z = t[at(e, f)];
+            if (kind_mixed(kind)) z = cmulc(z, __ldg(wpre + e));
+            v[m] = (kind_neg_odd(kind) && (j & 1)) ? cneg(z) : z;
         }
         __syncwarp();
 #pragma unroll
@@ -134,14 +139,14 @@ struct YTPass {
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
             zq[m] = t[at(s, f)];
-            zm[m] = t[at(s == 0 ? H : N - s, f)];
+            zm[m] = t[at(kind_mixed(a.kind) ? N - 1 - s : (s == 0 ? H : N - s), f)];
         }
         __syncwarp();
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
             cplx r0, r1;
-            if (s == 0) {
+            if (s == 0 && !kind_mixed(a.kind)) {
                 const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
                 r0 = make_double2(zq[m].x, zq[m].y);
                 r1 = make_double2(c * zm[m].x, c * zm[m].y);
@@ -178,7 +183,7 @@ struct YTPass {
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
-            if (s == 0) {
+            if (s == 0 && !kind_mixed(a.kind)) {
                 const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
                 t[at(0, f)] = make_double2(r0[m].x, r0[m].y);
                 t[at(H, f)] = make_double2(c * r1[m].x, c * r1[m].y);
@@ -188,7 +193,7 @@ struct YTPass {
                 cplx Zq, Zm;
                 pre_inverse(r0[m].x, r1[m].x, r0[m].y, r1[m].y, wq, a.kind, Zq, Zm);
                 t[at(s, f)] = Zq;
-                t[at(N - s, f)] = Zm;
+                t[at(kind_mixed(a.kind) ? N - 1 - s : N - s, f)] = Zm;
             }
         }
         __syncwarp();

@@ -118,7 +118,9 @@ struct YWPass {
             for (int u = 0; u < UB; ++u) {
                 const int j = j0 + YW_ROWS * (it0 + u);
                 const int e = elem_of_index<N>(j, a.kind);
-                tile[e * RS + f] = (a.kind == KIND_DD && (j & 1)) ? cneg(z[u]) : z[u];
+                cplx zz = (kind_neg_odd(a.kind) && (j & 1)) ? cneg(z[u]) : z[u];
+                if (kind_mixed(a.kind)) zz = cmul(zz, __ldg(a.wpre + e));
+                tile[e * RS + f] = zz;
             }
         }
     }
@@ -129,7 +131,12 @@ struct YWPass {
 #pragma unroll 4
         for (int s = tid / YW_TXC; s < H; s += YW_ROWS) {
             double2 r0, r1;
-            if (s == 0) {
+            if (kind_mixed(a.kind)) {
+                double A0, A1, B0, B1;
+                post_forward(tile[s * RS + f], tile[(N - 1 - s) * RS + f], __ldg(a.wpost + s), a.kind, A0, A1, B0, B1);
+                r0 = make_double2(A0, B0);
+                r1 = make_double2(A1, B1);
+            } else if (s == 0) {
                 const cplx Z0 = tile[f], Zh = tile[H * RS + f];
                 const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
                 r0 = make_double2(Z0.x, Z0.y);
@@ -166,7 +173,12 @@ struct YWPass {
 #pragma unroll
             for (int u = 0; u < UB; ++u) {
                 const int s = s0 + YW_ROWS * (it0 + u);
-                if (s == 0) {
+                if (kind_mixed(a.kind)) {
+                    cplx Zq, Zm;
+                    pre_inverse(r0[u].x, r1[u].x, r0[u].y, r1[u].y, __ldg(a.wpost + s), a.kind, Zq, Zm);
+                    tile[s * RS + f] = Zq;
+                    tile[(N - 1 - s) * RS + f] = Zm;
+                } else if (s == 0) {
                     const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
                     tile[f] = make_double2(r0[u].x, r0[u].y);
                     tile[H * RS + f] = make_double2(c * r1[u].x, c * r1[u].y);
@@ -189,7 +201,8 @@ struct YWPass {
         for (int j = tid / YW_TXC; j < N; j += YW_ROWS) {
             const int e = elem_of_index<N>(j, a.kind);
             cplx z = tile[e * RS + f];
-            if (a.kind == KIND_DD && (j & 1)) z = cneg(z);
+            if (kind_mixed(a.kind)) z = cmulc(z, __ldg(a.wpre + e));
+            if (kind_neg_odd(a.kind) && (j & 1)) z = cneg(z);
             *reinterpret_cast<double2*>(base + (size_t)j * a.nx + 2 * f) = z;
         }
     }

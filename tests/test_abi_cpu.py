@@ -49,7 +49,6 @@ PP_NN = (("P", "P"), ("P", "P"), ("N", "N"))
     (dict(nx=32, ny=32, nz=32, lx=-1.0), 1),
     (dict(nx=32, ny=32, nz=32, bc=(("P", "N"), ("P", "P"), ("N", "N"))), 1),      # one-sided periodic
     (dict(nx=32, ny=32, nz=32, bc=(("X", "X"), ("P", "P"), ("N", "N"))), 1),      # unknown letter
-    (dict(nx=32, ny=32, nz=32, bc=(("N", "D"), ("P", "P"), ("N", "N"))), 2),      # mixed pair in x (NEXT f2)
     (dict(nx=32, ny=32, nz=1000, bc=(("P", "P"), ("P", "P"), ("P", "P"))), 3),    # periodic z: nz <= 960
     (dict(nx=40, ny=32, nz=32), 3),                                                # 40 = 2^3*5
     (dict(nx=32, ny=32, nz=2000), 3),
@@ -77,7 +76,7 @@ int main() {
         if (f.r1 * f.r2 * f.r3 != n) return 2;
         auto t = make_pass_twiddles(f);
         printf("tw %d %zu %.17g %.17g\n", n, t.size() / 2, t[2 * 5], t[2 * 5 + 1]);
-        for (int kind = 0; kind < 3; ++kind) {
+        for (int kind = 0; kind < 5; ++kind) {
             auto lam = make_lambda_positions(n, kind, 1.0);
             double s = 0; for (double v : lam) s += v;
             printf("lam %d %d %.17g %.17g %.17g\n", n, kind, s, lam[0], lam[1]);
@@ -110,9 +109,15 @@ int main() {
             seen += 1
         if w[0] == "lam":
             n, kind = int(w[1]), int(w[2])
-            # trace of the n x n second-difference matrix with the ghost rule: PP -2n, NN -2n+2, DD -2n-2
-            trace = {0: -2.0 * n, 1: -2.0 * n + 2, 2: -2.0 * n - 2}[kind]
+            # trace of the n x n second-difference matrix with the ghost rule: PP -2n, NN -2n+2, DD -2n-2, ND / DN -2n
+            trace = {0: -2.0 * n, 1: -2.0 * n + 2, 2: -2.0 * n - 2, 3: -2.0 * n, 4: -2.0 * n}[kind]
             assert abs(float(w[3]) - trace) < 1e-9 * n
-            assert float(w[4]) == (0.0 if kind != 2 else -4.0)
+            if kind < 3:
+                assert float(w[4]) == (0.0 if kind != 2 else -4.0)
+            else:
+                # positions (0, 1) hold modes (0, n-1) for ND and (n-1, 0) for DN: -4 sin^2(pi (2q+1) / (4n))
+                lo, hi = (-4 * np.sin(np.pi * (2 * q + 1) / (4 * n)) ** 2 for q in (0, n - 1))
+                want = (lo, hi) if kind == 3 else (hi, lo)
+                assert abs(float(w[4]) - want[0]) < 1e-15 and abs(float(w[5]) - want[1]) < 1e-14
             seen += 1
-    assert seen == 16
+    assert seen == 24
