@@ -14,6 +14,8 @@ Source: /root/reference/PAPER.md ("P:L<n>" = line n of that file).
   * eq. 6   P:L102  (lam_i/dx^2+lam_j/dy^2) Phi^ + d_zz Phi^ = f^, "Gauss elimination"
                     P:L98-100                              -> ``poisson_solve``
   * P:L104  "the grid in z can be non-uniform"             -> ``z_coefficients``
+  * eq. 2d  P:L64   p^{k+1/2} = p^{k-1/2} + Phi             -> ``pressure_update``
+  * eq. 4   P:L87 and Listing 1 P:L142-205 (``chkdt``)     -> ``chkdt_fields``, ``chkdt``
 
 The paper delegates the eigenfunction tables to its refs [11,17], which are
 not available; the tables below are the DESIGN.md reading S1 and are *pinned* in
@@ -37,7 +39,7 @@ import numpy as np
 __all__ = [
     "pair_of", "basis", "z_coefficients", "z_matrix_rows", "thomas",
     "apply_laplacian", "poisson_solve", "divergence", "correct_velocity",
-    "projection", "is_singular", "uniform_spacing",
+    "projection", "is_singular", "uniform_spacing", "pressure_update", "chkdt_fields", "chkdt",
 ]
 
 
@@ -364,3 +366,83 @@ def projection(u, v, w, dt, lx, ly, lz, bc, dzc=None, dzf=None, lower_face=None)
     phi = poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
     un, vn, wn, faces = correct_velocity(u, v, w, phi, dt, lx, ly, lz, bc, dzc, dzf, lower_face)
     return un, vn, wn, phi, faces
+
+
+# --------------------------------------------------------------------------------------
+# NEXT row f3: pressure update (eq. 2d) and the stable-time-step reduction of Listing 1 (``chkdt``)
+# --------------------------------------------------------------------------------------
+def pressure_update(p, phi):
+    """p^{k+1/2} = p^{k-1/2} + Phi (eq. 2d, explicit diffusion)."""
+    return np.asarray(p, dtype=np.float64) + np.asarray(phi, dtype=np.float64)
+
+
+def _pad_velocity(vel, axis, pair, normal, face):
+    """One layer below and above `vel` along `axis` for the face averages of Listing 1 (reading S17): periodic ->
+    wrapped; non-periodic -> below: the lower boundary face (registered plane or 0) for the component normal to the
+    axis, 0 for a tangential one; above: 0."""
+    shape = list(vel.shape)
+    shape[axis] = 1
+    if pair == "PP":
+        lo, hi = np.take(vel, [-1], axis=axis), np.take(vel, [0], axis=axis)
+    else:
+        lo = _lower_face(vel, axis, pair, face) if normal else np.zeros(shape)
+        hi = np.zeros(shape)
+    return np.concatenate([lo, vel, hi], axis=axis)
+
+
+def chkdt_fields(u, v, w, lx, ly, lz, bc, dzc=None, dzf=None, lower_face=None):
+    """The three per-face sums of Listing 1, 0-based on the compact layout:
+
+      dtix(i,j,k) = |u(i,j,k)|/dx + 0.25|v(i,j,k)+v(i,j-1,k)+v(i+1,j,k)+v(i+1,j-1,k)|/dy
+                                  + 0.25|w(i,j,k)+w(i,j,k-1)+w(i+1,j,k)+w(i+1,j,k-1)|/dzf(k)        (P:L181-187, printed)
+      dtiy(i,j,k) = 0.25|u(i,j,k)+u(i,j+1,k)+u(i-1,j+1,k)+u(i-1,j,k)|/dx + |v(i,j,k)|/dy
+                                  + 0.25|w(i,j,k)+w(i,j+1,k)+w(i,j+1,k-1)+w(i,j,k-1)|/dzf(k)        (lines lost: by symmetry, S15)
+      dtiz(i,j,k) = 0.25|u(i,j,k)+u(i-1,j,k)+u(i-1,j,k+1)+u(i,j,k+1)|/dx
+                  + 0.25|v(i,j,k)+v(i,j-1,k)+v(i,j-1,k+1)+v(i,j,k+1)|/dy + |w(i,j,k)|/dzc(k+1)      (dzci(k) of the face k+1/2)
+
+    i.e. at the face a component lives on: its own magnitude plus the 4-point averages of the other two."""
+    u, v, w = (np.asarray(a, dtype=np.float64) for a in (u, v, w))
+    nz, ny, nx = u.shape
+    if dzc is None or dzf is None:
+        dzc, dzf = uniform_spacing(nz, lz)
+    dzc = np.asarray(dzc, dtype=np.float64)
+    dzf = np.asarray(dzf, dtype=np.float64)
+    lower_face = lower_face or {}
+    dxi, dyi = nx / lx, ny / ly
+    px, py, pz = pair_of(bc[0]), pair_of(bc[1]), pair_of(bc[2])
+
+    def pad3(a, comp):
+        a = _pad_velocity(a, 2, px, comp == 0, lower_face.get(0))
+        # the planes registered for y and z have the extent of the unpadded field: pad them with zeros along x
+        fy, fz = lower_face.get(1), lower_face.get(2)
+        if fy is not None:
+            fy = np.pad(np.asarray(fy, dtype=np.float64).reshape(nz, 1, nx), ((0, 0), (0, 0), (1, 1)))
+        a = _pad_velocity(a, 1, py, comp == 1, fy if comp == 1 else None)
+        if fz is not None:
+            fz = np.pad(np.asarray(fz, dtype=np.float64).reshape(1, ny, nx), ((0, 0), (1, 1), (1, 1)))
+        a = _pad_velocity(a, 0, pz, comp == 2, fz if comp == 2 else None)
+        return a                                    # index [k+1, j+1, i+1] = cell (i, j, k)
+
+    U, V, W = pad3(u, 0), pad3(v, 1), pad3(w, 2)
+    c = slice(1, -1)          # the cell itself
+    m = slice(0, -2)          # index - 1
+    q = slice(2, None)        # index + 1
+    dzfi = (1.0 / dzf)[:, None, None]
+    dzci = (1.0 / dzc[1:])[:, None, None]
+    dtix = (np.abs(U[c, c, c]) * dxi
+            + 0.25 * np.abs(V[c, c, c] + V[c, m, c] + V[c, c, q] + V[c, m, q]) * dyi
+            + 0.25 * np.abs(W[c, c, c] + W[m, c, c] + W[c, c, q] + W[m, c, q]) * dzfi)
+    dtiy = (0.25 * np.abs(U[c, c, c] + U[c, q, c] + U[c, q, m] + U[c, c, m]) * dxi
+            + np.abs(V[c, c, c]) * dyi
+            + 0.25 * np.abs(W[c, c, c] + W[c, q, c] + W[m, q, c] + W[m, c, c]) * dzfi)
+    dtiz = (0.25 * np.abs(U[c, c, c] + U[c, c, m] + U[q, c, m] + U[q, c, c]) * dxi
+            + 0.25 * np.abs(V[c, c, c] + V[c, m, c] + V[q, m, c] + V[q, c, c]) * dyi
+            + np.abs(W[c, c, c]) * dzci)
+    return dtix, dtiy, dtiz
+
+
+def chkdt(u, v, w, lx, ly, lz, bc, dzc=None, dzf=None, lower_face=None):
+    """dti = max(0, max_ijk(dtix, dtiy, dtiz)) of Listing 1; the stable step of eq. 4 follows
+    on the host as min(1.65 dl^2 / nu, sqrt(3) / dti)."""
+    dtix, dtiy, dtiz = chkdt_fields(u, v, w, lx, ly, lz, bc, dzc, dzf, lower_face)
+    return float(max(0.0, dtix.max(), dtiy.max(), dtiz.max()))

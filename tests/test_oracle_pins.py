@@ -483,3 +483,105 @@ def test_gradient_of_linear_phi_is_constant():
     bcp = (("P", "P"), ("N", "N"), ("N", "N"))
     un, _, _, _ = orc.correct_velocity(u, v, w, phi, dt, lx, ly, lz, bcp, dzc, dzf)
     assert np.max(np.abs(un[:, :, -1] - (u[:, :, -1] - dt * (phi[:, :, 0] - phi[:, :, -1]) / (lx / nx)))) < 1e-13
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT row f3: eq. 2d and the chkdt reduction of Listing 1, pinned on inputs whose per-face sums are
+# known by hand from the printed lines and their symmetric counterparts (reading S15)
+# ----------------------------------------------------------------------------------------------
+def test_pressure_update_is_a_plain_sum():
+    rng = np.random.default_rng(5)
+    p, phi = rng.standard_normal((3, 4, 5)), rng.standard_normal((3, 4, 5))
+    out = orc.pressure_update(p, phi)
+    assert np.array_equal(out, p + phi) and out is not p
+
+
+def test_chkdt_of_uniform_flow():
+    """u = a, v = b, w = c everywhere on a triperiodic grid: every face sum is |a|/dx + |b|/dy + |c|/dz."""
+    nz, ny, nx = 5, 6, 8
+    lx, ly, lz = 4.0, 1.5, 2.5
+    bc = (("P", "P"), ("P", "P"), ("P", "P"))
+    a, b, c = 2.0, -3.0, 0.5
+    u, v, w = (np.full((nz, ny, nx), t) for t in (a, b, c))
+    want = abs(a) * nx / lx + abs(b) * ny / ly + abs(c) * nz / lz
+    fx, fy, fz = orc.chkdt_fields(u, v, w, lx, ly, lz, bc)
+    for f in (fx, fy, fz):
+        assert np.max(np.abs(f - want)) < 1e-13
+    assert abs(orc.chkdt(u, v, w, lx, ly, lz, bc) - want) < 1e-13
+    # stretched z: dtix, dtiy weigh w with 1/dzf(k) (P:L187), dtiz with 1/dzc(k+1) (P:L189: dzci(k) of the face k+1/2)
+    dzc, dzf = stretched(nz, lz, 1.7)
+    dzc[0] = dzc[-1] = 0.5 * (dzf[0] + dzf[-1])          # single-valued wrap spacing
+    fx, fy, fz = orc.chkdt_fields(u, v, w, lx, ly, lz, bc, dzc, dzf)
+    base = abs(a) * nx / lx + abs(b) * ny / ly
+    assert np.max(np.abs(fx - (base + abs(c) / dzf)[:, None, None])) < 1e-13
+    assert np.max(np.abs(fy - (base + abs(c) / dzf)[:, None, None])) < 1e-13
+    assert np.max(np.abs(fz - (base + abs(c) / dzc[1:])[:, None, None])) < 1e-13
+    assert orc.chkdt(np.zeros_like(u), np.zeros_like(u), np.zeros_like(u), lx, ly, lz, bc) == 0.0
+
+
+def test_chkdt_stencils_from_unit_impulses():
+    """One non-zero velocity value: the faces that see it and with which weight, written out from Listing 1
+    (vx, wx: P:L183-185 as printed; the lost uy, wy, uz, vz lines by the same pattern rotated)."""
+    nz, ny, nx = 6, 7, 8
+    lx, ly, lz = 4.0, 3.5, 3.0
+    dx, dy = lx / nx, ly / ny
+    dzc, dzf = stretched(nz, lz, 1.4)
+    bc = (("N", "N"), ("N", "N"), ("N", "N"))
+    i0, j0, k0 = 3, 2, 3
+    z = np.zeros((nz, ny, nx))
+
+    def support(f):
+        return {(int(k), int(j), int(i)): f[k, j, i] for k, j, i in zip(*np.nonzero(f))}
+
+    # impulse in v
+    v = z.copy(); v[k0, j0, i0] = 2.0
+    fx, fy, fz = orc.chkdt_fields(z, v, z, lx, ly, lz, bc, dzc, dzf)
+    q = 0.25 * 2.0 / dy
+    assert support(fx) == {(k0, j0, i0): q, (k0, j0 + 1, i0): q, (k0, j0, i0 - 1): q, (k0, j0 + 1, i0 - 1): q}
+    assert support(fy) == {(k0, j0, i0): 2.0 / dy}
+    assert support(fz) == {(k0, j0, i0): q, (k0, j0 + 1, i0): q, (k0 - 1, j0, i0): q, (k0 - 1, j0 + 1, i0): q}
+    # impulse in w: 1/dzf of the face's own cell for dtix, dtiy; 1/dzc(k+1) for dtiz
+    w = z.copy(); w[k0, j0, i0] = -2.0
+    fx, fy, fz = orc.chkdt_fields(z, z, w, lx, ly, lz, bc, dzc, dzf)
+    qa, qb = 0.5 / dzf[k0], 0.5 / dzf[k0 + 1]
+    assert support(fx) == pytest.approx({(k0, j0, i0): qa, (k0, j0, i0 - 1): qa, (k0 + 1, j0, i0): qb, (k0 + 1, j0, i0 - 1): qb})
+    assert support(fy) == pytest.approx({(k0, j0, i0): qa, (k0, j0 - 1, i0): qa, (k0 + 1, j0, i0): qb, (k0 + 1, j0 - 1, i0): qb})
+    assert support(fz) == pytest.approx({(k0, j0, i0): 2.0 / dzc[k0 + 1]})
+    # impulse in u
+    u = z.copy(); u[k0, j0, i0] = 2.0
+    fx, fy, fz = orc.chkdt_fields(u, z, z, lx, ly, lz, bc, dzc, dzf)
+    q = 0.5 / dx
+    assert support(fx) == {(k0, j0, i0): 2.0 / dx}
+    assert support(fy) == {(k0, j0, i0): q, (k0, j0 - 1, i0): q, (k0, j0, i0 + 1): q, (k0, j0 - 1, i0 + 1): q}
+    assert support(fz) == {(k0, j0, i0): q, (k0, j0, i0 + 1): q, (k0 - 1, j0, i0): q, (k0 - 1, j0, i0 + 1): q}
+    # the magnitude is taken of the 4-point SUM (P:L183 "0.25*abs(v+v+v+v)"): opposite neighbours cancel
+    v = z.copy(); v[k0, j0, i0] = 1.0; v[k0, j0, i0 + 1] = -1.0
+    fx, _, _ = orc.chkdt_fields(z, v, z, lx, ly, lz, bc, dzc, dzf)
+    assert fx[k0, j0, i0] == 0.0 and fx[k0, j0, i0 - 1] == 0.25 / dy and fx[k0, j0, i0 + 1] == 0.25 / dy
+
+
+def test_chkdt_boundaries():
+    """Reading S17: periodic directions wrap; in a non-periodic direction the layer below index 0 is the lower boundary
+    face for the normal component (registered plane, else 0) and 0 for the tangential ones; the layer above is 0."""
+    nz, ny, nx = 4, 5, 6
+    lx, ly, lz = 3.0, 2.5, 2.0
+    dx, dy, dz = lx / nx, ly / ny, lz / nz
+    z = np.zeros((nz, ny, nx))
+    # periodic x: u(nx-1) is the face below cell 0
+    bc = (("P", "P"), ("N", "N"), ("N", "N"))
+    u = z.copy(); u[1, 2, nx - 1] = 4.0
+    _, fy, fz = orc.chkdt_fields(u, z, z, lx, ly, lz, bc)
+    assert fy[1, 2, 0] == 1.0 / dx and fy[1, 1, 0] == 1.0 / dx and fz[1, 2, 0] == 1.0 / dx and fz[0, 2, 0] == 1.0 / dx
+    # non-periodic x without a plane: nothing wraps
+    bcn = (("N", "N"), ("N", "N"), ("N", "N"))
+    _, fy, fz = orc.chkdt_fields(u, z, z, lx, ly, lz, bcn)
+    assert fy[1, 2, 0] == 0.0 and fz[1, 2, 0] == 0.0
+    # a registered lower plane in z enters the w averages of the first layer of cells
+    plane = np.zeros((1, ny, nx)); plane[0, 2, 3] = 4.0
+    fx, fy, fz = orc.chkdt_fields(z, z, z, lx, ly, lz, (("N", "N"), ("N", "N"), ("D", "N")), lower_face={2: plane})
+    assert fx[0, 2, 3] == 1.0 / dz and fx[0, 2, 2] == 1.0 / dz and fy[0, 2, 3] == 1.0 / dz and fy[0, 1, 3] == 1.0 / dz
+    assert np.count_nonzero(fx) == 2 and np.count_nonzero(fy) == 2 and np.count_nonzero(fz) == 0
+    # tangential components beyond the upper end are 0: the last u-face sees only its two interior v values
+    v = np.ones((nz, ny, nx))
+    fx, _, _ = orc.chkdt_fields(z, v, z, lx, ly, lz, bcn)
+    assert fx[1, 2, nx - 1] == 0.5 / dy and fx[1, 2, 0] == 1.0 / dy and fx[1, 0, 0] == 0.5 / dy
