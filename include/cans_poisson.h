@@ -99,6 +99,30 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
                     double dt, void* stream);
 
 /*
+ * cans_projection_step -- cans_projection plus the two bandwidth-only steps a time loop runs after it:
+ *   p_acc   DEVICE or NULL: the accumulated pressure; eq. 2d  p_acc += Phi  is done by the correction kernel itself
+ *           (the same pass that applies eq. 2c: +16 B/cell instead of a separate 24 B/cell sweep).  Must not alias p.
+ *   dti     DEVICE scalar (one double) or NULL: receives the reduction of Listing 1 (`chkdt`; eq. 4)
+ *           over the CORRECTED velocities, see cans_chkdt.
+ * Everything else as cans_projection (which is this call with p_acc = dti = NULL).
+ */
+int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double* p_acc,
+                         double dt, double* dti, void* stream);
+
+/*
+ * cans_chkdt -- the max-reduction of Listing 1:
+ *     dti = max over cells of max(dtix, dtiy, dtiz),
+ *     dtix = |u|/dx + |v(i,j)+v(i,j-1)+v(i+1,j)+v(i+1,j-1)|/(4 dy) + |w(i,j,k)+w(i,j,k-1)+w(i+1,j,k)+w(i+1,j,k-1)|/(4 dzf[k])
+ *     (P:L181-187), dtiy and dtiz the same pattern on the v and w faces, the latter with 1/dzc[k+1];
+ * the stable step of eq. 4 is then min(1.65 dl^2/nu, sqrt(3)/dti) on the host.  Neighbours outside the arrays:
+ * wrapped in a periodic direction; otherwise the lower boundary face (registered plane, else 0) for the component normal to
+ * it and 0 for every other out-of-range value.
+ *   u, v, w  DEVICE, read only.    dti  DEVICE, one double, overwritten (0 for a field at rest).
+ * A lower 'D' side without a registered plane returns CANS_ERR_NEEDS_FACE, as in cans_projection.
+ */
+int cans_chkdt(cans_poisson_plan* plan, const double* u, const double* v, const double* w, double* dti, void* stream);
+
+/*
  * cans_projection_set_lower_face -- register the boundary-normal velocity on the LOWER face of
  * direction dir (0,1,2): DEVICE plane of (product of the other two extents) doubles, x fastest among the
  * remaining indices (dir 0: j + ny*k; dir 1: i + nx*k; dir 2: i + nx*j), 16-byte aligned, or NULL to

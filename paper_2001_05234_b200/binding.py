@@ -25,6 +25,7 @@ MAX_KERNEL_RECORDS = 16      # CANS_MAX_KERNEL_RECORDS of the header
 
 EXPORTED_SYMBOLS = (
     "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
+    "cans_projection_step", "cans_chkdt",
     "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
@@ -67,6 +68,10 @@ def _load() -> ctypes.CDLL:
     lib.cans_plan_launches_per_solve.argtypes = [vp]
     lib.cans_plan_launches_per_projection.restype = i32
     lib.cans_plan_launches_per_projection.argtypes = [vp]
+    lib.cans_projection_step.restype = i32
+    lib.cans_projection_step.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_double, vp, vp]
+    lib.cans_chkdt.restype = i32
+    lib.cans_chkdt.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.cans_plan_set_profiling.restype = i32
     lib.cans_plan_set_profiling.argtypes = [vp, i32]
     lib.cans_plan_kernel_times.restype = i32
@@ -162,6 +167,19 @@ class PoissonPlan:
         _check(_lib.cans_projection(self._h, _dev_ptr(u, self.shape), _dev_ptr(v, self.shape),
                                     _dev_ptr(w, self.shape), _dev_ptr(p, self.shape), float(dt),
                                     _stream_ptr(stream)))
+
+    def projection_step(self, u, v, w, p, dt: float, p_acc=None, dti=None, stream=None):
+        """cans_projection_step: the projection, plus p_acc += Phi (eq. 2d) in the correction kernel when p_acc is
+        given, plus the chkdt reduction of the corrected velocities into the one-element CUDA tensor dti when given."""
+        _check(_lib.cans_projection_step(self._h, _dev_ptr(u, self.shape), _dev_ptr(v, self.shape),
+                                         _dev_ptr(w, self.shape), _dev_ptr(p, self.shape),
+                                         None if p_acc is None else _dev_ptr(p_acc, self.shape), float(dt),
+                                         None if dti is None else _dev_ptr(dti, (1,)), _stream_ptr(stream)))
+
+    def chkdt(self, u, v, w, dti, stream=None):
+        """cans_chkdt: dti[0] = max over cells of the per-face sums of Listing 1 (one-element CUDA float64 tensor)."""
+        _check(_lib.cans_chkdt(self._h, _dev_ptr(u, self.shape), _dev_ptr(v, self.shape), _dev_ptr(w, self.shape),
+                               _dev_ptr(dti, (1,)), _stream_ptr(stream)))
 
     def set_lower_face(self, direction: int, plane: Optional[torch.Tensor]):
         """cans_projection_set_lower_face: register (or, with None, unregister) the boundary-normal velocity on the

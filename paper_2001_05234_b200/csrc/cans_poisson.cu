@@ -26,6 +26,7 @@
 #include "xy_kernels.cuh"
 #include "z_kernels.cuh"
 #include "grad_pass.cuh"
+#include "chkdt_pass.cuh"
 #include "xw_kernels.cuh"
 #include "yw_kernels.cuh"
 #include "yt_kernels.cuh"
@@ -87,7 +88,58 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
         in.uu = *reinterpret_cast<const double2*>(a.u + o);
         in.vv = *reinterpret_cast<const double2*>(a.v + o);
         in.ww = *reinterpret_cast<const double2*>(a.w + o);
+        if (a.pacc) in.pa = *reinterpret_cast<const double2*>(a.pacc + o);
         grad_apply(a, in);
+    }
+}
+
+// chkdt (Listing 1): see chkdt_pass.cuh.  One thread per pair of x-adjacent cells, marching up CHK_KC planes.
+constexpr int CHK_KC = 32;
+
+__global__ void __launch_bounds__(256) chkdt_kernel(const ChkArgs a) {
+    const int hx = a.nx / 2;
+    const size_t cols = (size_t)hx * a.ny;
+    const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    double m = 0.0;
+    if (c < cols) {
+        const int i = 2 * (int)(c % hx);
+        const int j = (int)(c / hx);
+        const int k0 = (int)blockIdx.y * CHK_KC;
+        const int k1 = (k0 + CHK_KC < a.nz) ? k0 + CHK_KC : a.nz;
+        const double qx = 0.25 * a.rdx, qy = 0.25 * a.rdy;
+        // carried rows: u(i-1..i+1, j, k); v(i..i+2, j-1 and j, k); w(i..i+2, j, k-1); w(i, i+1; j+1, k-1)
+        Row3 uj = chk_row_u(a, i, j, k0);
+        Row3 vm = chk_row_v(a, i, j - 1, k0), vj = chk_row_v(a, i, j, k0);
+        Row3 wlj = chk_row_w(a, i, j, k0 - 1), wlp = chk_row_w(a, i, j + 1, k0 - 1);
+        for (int k = k0; k < k1; ++k) {
+            const Row3 up = chk_row_u(a, i, j + 1, k);            // u(i-1..i+1, j+1, k)
+            const Row3 un = chk_row_u(a, i, j, k + 1);            // u(i-1..i+1, j,   k+1)
+            const Row3 vmn = chk_row_v(a, i, j - 1, k + 1), vjn = chk_row_v(a, i, j, k + 1);
+            const Row3 wj = chk_row_w(a, i, j, k), wp = chk_row_w(a, i, j + 1, k);
+            const double rzf = a.rdzf[k], rzc = a.rdzc[k], qz = 0.25 * rzf;
+            // cell i (values .a / .b of the v, w rows; .b of the u rows) and cell i+1 (.b / .c; .c)
+            const double dtix0 = fabs(uj.b) * a.rdx + fabs(vj.a + vm.a + vj.b + vm.b) * qy + fabs(wj.a + wlj.a + wj.b + wlj.b) * qz;
+            const double dtix1 = fabs(uj.c) * a.rdx + fabs(vj.b + vm.b + vj.c + vm.c) * qy + fabs(wj.b + wlj.b + wj.c + wlj.c) * qz;
+            const double dtiy0 = fabs(uj.b + up.b + up.a + uj.a) * qx + fabs(vj.a) * a.rdy + fabs(wj.a + wp.a + wlp.a + wlj.a) * qz;
+            const double dtiy1 = fabs(uj.c + up.c + up.b + uj.b) * qx + fabs(vj.b) * a.rdy + fabs(wj.b + wp.b + wlp.b + wlj.b) * qz;
+            const double dtiz0 = fabs(uj.b + uj.a + un.a + un.b) * qx + fabs(vj.a + vm.a + vmn.a + vjn.a) * qy + fabs(wj.a) * rzc;
+            const double dtiz1 = fabs(uj.c + uj.b + un.b + un.c) * qx + fabs(vj.b + vm.b + vmn.b + vjn.b) * qy + fabs(wj.b) * rzc;
+            m = fmax(m, fmax(fmax(dtix0, dtix1), fmax(fmax(dtiy0, dtiy1), fmax(dtiz0, dtiz1))));
+            uj = un; vm = vmn; vj = vjn; wlj = wj; wlp = wp;
+        }
+    }
+    // CTA maximum, then one atomic per CTA -- and only if it can raise the global value (non-negative doubles order
+    // like their bit patterns)
+    __shared__ double s_max[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) s_max[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int q = 1; q < 8; ++q) m = fmax(m, s_max[q]);
+        const unsigned long long bits = (unsigned long long)__double_as_longlong(m);
+        if (bits > *reinterpret_cast<volatile unsigned long long*>(a.dti)) atomicMax(a.dti, bits);
     }
 }
 
@@ -470,9 +522,55 @@ int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream) {
     return run_core(plan, p, nullptr, nullptr, (cudaStream_t)stream);
 }
 
+static int chkdt_enqueue(cans_poisson_plan* plan, const double* u, const double* v, const double* w, double* dti, cudaStream_t st);
+
+int cans_chkdt(cans_poisson_plan* plan, const double* u, const double* v, const double* w, double* dti, void* stream) {
+    g_status = CANS_OK;
+    if (!plan) return fail(CANS_ERR_INVALID_ARG, "plan is NULL");
+    plan->nrec = 0;
+    return chkdt_enqueue(plan, u, v, w, dti, (cudaStream_t)stream);
+}
+
+static int chkdt_enqueue(cans_poisson_plan* plan, const double* u, const double* v, const double* w, double* dti, cudaStream_t st) {
+    if (!u || !v || !w || !dti) return fail(CANS_ERR_INVALID_ARG, "u, v, w, dti must be non-NULL");
+    if (((reinterpret_cast<size_t>(u) | reinterpret_cast<size_t>(v) | reinterpret_cast<size_t>(w)) & 15) != 0 ||
+        (reinterpret_cast<size_t>(dti) & 7) != 0)
+        return fail(CANS_ERR_INVALID_ARG, "fields must be 16-byte aligned, dti 8-byte aligned");
+    for (int d = 0; d < 3; ++d)
+        if (plan->bc[d][0] == 'D' && !plan->face[d])
+            return fail(CANS_ERR_NEEDS_FACE, "a lower 'D' side needs a lower-face plane (cans_projection_set_lower_face)");
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != plan->device)
+        return fail(CANS_ERR_INVALID_ARG, "the plan was created on another device than the current one");
+    ChkArgs c;
+    c.nx = plan->nx; c.ny = plan->ny; c.nz = plan->nz;
+    c.u = u; c.v = v; c.w = w;
+    c.fx = plan->face[0]; c.fy = plan->face[1]; c.fz = plan->face[2];
+    c.wrap_x = plan->bc[0][0] == 'P'; c.wrap_y = plan->bc[1][0] == 'P'; c.wrap_z = plan->bc[2][0] == 'P';
+    c.rdx = (double)plan->nx / plan->lx; c.rdy = (double)plan->ny / plan->ly;
+    c.rdzf = plan->rdzf; c.rdzc = plan->rdzc;
+    c.dti = reinterpret_cast<unsigned long long*>(dti);
+    cudaError_t e = cudaMemsetAsync(dti, 0, sizeof(double), st);
+    if (e != cudaSuccess) return fail_cuda(e, "dti reset");
+    const size_t cols = (size_t)plan->nx / 2 * plan->ny;
+    dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((plan->nz + CHK_KC - 1) / CHK_KC));
+    LaunchScope scope(plan, st, "chkdt");
+    chkdt_kernel<<<grid, 256, 0, st>>>(c);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return fail_cuda(e, "chkdt launch");
+    return CANS_OK;
+}
+
 int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double dt, void* stream) {
+    return cans_projection_step(plan, u, v, w, p, nullptr, dt, nullptr, stream);
+}
+
+int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double* p_acc, double dt,
+                         double* dti, void* stream) {
     g_status = CANS_OK;
     if (!plan || !u || !v || !w || !p) return fail(CANS_ERR_INVALID_ARG, "plan, u, v, w, p must be non-NULL");
+    if (p_acc && ((reinterpret_cast<size_t>(p_acc) & 15) != 0 || p_acc == p))
+        return fail(CANS_ERR_INVALID_ARG, "p_acc must be 16-byte aligned and distinct from p");
     if (!(dt > 0.0)) return fail(CANS_ERR_INVALID_ARG, "dt must be > 0");
     if (((reinterpret_cast<size_t>(p) | reinterpret_cast<size_t>(u) | reinterpret_cast<size_t>(v) |
           reinterpret_cast<size_t>(w)) & 15) != 0)
@@ -495,6 +593,7 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
     g.nx = plan->nx; g.ny = plan->ny; g.nz = plan->nz;
     g.k0 = 0; g.k1 = plan->nz;
     g.u = u; g.v = v; g.w = w; g.phi = p;
+    g.pacc = p_acc;
     g.rdzc = plan->rdzc;
     g.dt = dt;
     g.dt_rdx = dt * a.rdx;
@@ -525,6 +624,12 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
         face_correct_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(fa);
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return fail_cuda(e, "lower-face correction launch");
+    }
+    if (dti) {
+        // chkdt on the corrected velocities: its own kernel -- the face averages need the corrected values of the
+        // neighbouring threads' cells, which an in-place correction cannot provide race-free
+        rc = chkdt_enqueue(plan, u, v, w, dti, (cudaStream_t)stream);
+        if (rc) return rc;
     }
     return CANS_OK;
 }

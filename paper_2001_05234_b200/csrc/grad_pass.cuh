@@ -12,6 +12,7 @@ struct GradArgs {
     int k0, k1;                // planes [k0, k1) corrected by this launch
     double* u; double* v; double* w;
     const double* phi;
+    double* pacc;              // eq. 2d: pacc += Phi in the same pass, or NULL
     const double* rdzc;        // [nz] 1/dzc[k+1]
     double dt_rdx, dt_rdy, dt;
     // ghost rule beyond the upper face: value = sgn * phi[idx]  (P: idx 0, sgn 1; N: idx n-1, sgn 1; D: idx n-1, sgn -1)
@@ -21,7 +22,7 @@ struct GradArgs {
 
 // inputs of one pair of x-adjacent cells, fetched before any of them is used
 struct GradIn {
-    double2 ph, phy, phz, uu, vv, ww;
+    double2 ph, phy, phz, uu, vv, ww, pa;
     double phx;
     size_t o;
     int k;
@@ -40,6 +41,7 @@ CANS_HD void grad_apply(const GradArgs& a, const GradIn& in) {
     *reinterpret_cast<double2*>(a.u + in.o) = uu;
     *reinterpret_cast<double2*>(a.v + in.o) = vv;
     *reinterpret_cast<double2*>(a.w + in.o) = ww;
+    if (a.pacc) *reinterpret_cast<double2*>(a.pacc + in.o) = make_double2(in.pa.x + ph.x, in.pa.y + ph.y);
 }
 
 }  // namespace cans

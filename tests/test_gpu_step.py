@@ -1,0 +1,124 @@
+"""GPU parity of the two steps that follow the projection in a time loop: eq. 2d fused into the
+correction kernel and the chkdt reduction of Listing 1, both through the C ABI against the CPU oracle."""
+import itertools
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import cans_oracle as orc
+from paper_2001_05234_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2001_05234_b200 import binding
+    return binding
+
+
+def _faces(rng, bc, shape, inflow=()):
+    nz, ny, nx = shape
+    shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+    return {d: rng.standard_normal(shapes[d]) for d in range(3) if bc[d][0] == "D" or d in inflow}
+
+
+ALL_PAIRS = ["PP", "NN", "DD", "ND", "DN"]
+
+
+@pytest.mark.parametrize("nx,ny,nz", [(48, 32, 37), (16, 16, 2), (512, 64, 5), (96, 1024, 3)])
+def test_chkdt_matches_the_oracle_for_every_boundary_combination(B, nx, ny, nz):
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    rng = np.random.default_rng(nx * 7 + nz)
+    u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+    dti = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+    combos = list(itertools.product(ALL_PAIRS, ALL_PAIRS, ALL_PAIRS))
+    if nx * ny * nz > 200000:
+        combos = combos[::9]
+    for n, (px, py, pz) in enumerate(combos):
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        inflow = tuple(d for d in range(3) if bc[d][0] == "N" and (n + d) % 3 == 0)     # some prescribed-inflow planes too
+        faces = _faces(rng, bc, (nz, ny, nx), inflow)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        fd = {d: torch.from_numpy(f).cuda() for d, f in faces.items()}
+        for d, t in fd.items():
+            plan.set_lower_face(d, t)
+        plan.chkdt(ud, vd, wd, dti)
+        torch.cuda.synchronize()
+        want = orc.chkdt(u, v, w, lx, ly, lz, bc, dzc, dzf, faces)
+        assert abs(float(dti[0]) - want) <= 1e-13 * want, (px, py, pz)
+        plan.close()
+
+
+def test_chkdt_special_values_and_errors(B):
+    nx, ny, nz = 32, 16, 8
+    bc = (("P", "P"), ("P", "P"), ("N", "N"))
+    plan = B.PoissonPlan(nx, ny, nz, 1.0, 1.0, 1.0, bc)
+    z = torch.zeros((nz, ny, nx), dtype=torch.float64, device="cuda")
+    dti = torch.full((1,), 7.0, dtype=torch.float64, device="cuda")
+    plan.chkdt(z, z, z, dti)
+    assert float(dti[0]) == 0.0                                           # field at rest: "dti = 0."
+    # uniform flow: |a|/dx + |b|/dy (w = 0), reached on the interior faces
+    a, b = 1.5, -0.25
+    plan.chkdt(z + a, z + b, z, dti)
+    assert abs(float(dti[0]) - (abs(a) * nx + abs(b) * ny)) < 1e-12
+    plan.close()
+    pland = B.PoissonPlan(nx, ny, nz, 1.0, 1.0, 1.0, (("D", "N"), ("P", "P"), ("N", "N")))
+    with pytest.raises(B.CansError) as ei:
+        pland.chkdt(z, z, z, dti)
+    assert ei.value.status == B.CANS_ERR_NEEDS_FACE
+    pland.close()
+
+
+@pytest.mark.parametrize("nx,ny,nz,bcs", [(96, 64, 40, ("PP", "PP", "NN")), (512, 32, 9, ("NN", "DN", "ND")),
+                                          (48, 768, 6, ("ND", "PP", "PP")), (1024, 32, 4, ("PP", "NN", "DD"))])
+def test_projection_step_fuses_eq_2d_and_returns_chkdt(B, nx, ny, nz, bcs):
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    bc = tuple((p[0], p[1]) for p in bcs)
+    rng = np.random.default_rng(nx + nz)
+    u, v, w, pacc = (rng.standard_normal((nz, ny, nx)) for _ in range(4))
+    pacc *= 100.0
+    faces = _faces(rng, bc, (nz, ny, nx))
+    dt = 1e-3
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    # plain projection first: the step variant must return the same bits for u, v, w, Phi and the planes
+    ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+    fd = {d: torch.from_numpy(f).cuda() for d, f in faces.items()}
+    for d, t in fd.items():
+        plan.set_lower_face(d, t)
+    pd = torch.empty_like(ud)
+    plan.projection(ud, vd, wd, pd, dt)
+    us, vs, ws = (torch.from_numpy(a).cuda() for a in (u, v, w))
+    fs = {d: torch.from_numpy(f).cuda() for d, f in faces.items()}
+    for d, t in fs.items():
+        plan.set_lower_face(d, t)
+    ps = torch.empty_like(us)
+    pa = torch.from_numpy(pacc).cuda()
+    dti = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+    plan.projection_step(us, vs, ws, ps, dt, p_acc=pa, dti=dti)
+    torch.cuda.synchronize()
+    for a, b in ((ud, us), (vd, vs), (wd, ws), (pd, ps)):
+        assert torch.equal(a, b)
+    for d in fd:
+        assert torch.equal(fd[d], fs[d])
+    # eq. 2d against the oracle; |Phi| ~ 1/dt, so the absolute bar applies to dt * p (reading S12)
+    un, vn, wn, phi, fn = orc.projection(u, v, w, dt, lx, ly, lz, bc, dzc, dzf, faces)
+    want = orc.pressure_update(pacc, phi)
+    got = pa.cpu().numpy()
+    assert np.linalg.norm(got - want) <= 1e-11 * np.linalg.norm(want)
+    assert np.max(np.abs(got - want)) * dt <= 1e-10
+    assert np.array_equal(got, pacc + ps.cpu().numpy())                   # exactly one rounding: the sum of the two fields
+    # chkdt of the corrected velocities (Listing 1) against the oracle on the oracle's corrected fields
+    want_dti = orc.chkdt(un, vn, wn, lx, ly, lz, bc, dzc, dzf, fn)
+    assert abs(float(dti[0]) - want_dti) <= 1e-10 * want_dti
+    # p_acc must not alias p
+    with pytest.raises(B.CansError) as ei:
+        plan.projection_step(us, vs, ws, ps, dt, p_acc=ps)
+    assert ei.value.status == B.CANS_ERR_INVALID_ARG
+    plan.close()
