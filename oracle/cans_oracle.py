@@ -16,6 +16,8 @@ Source: /root/reference/PAPER.md ("P:L<n>" = line n of that file).
   * P:L104  "the grid in z can be non-uniform"             -> ``z_coefficients``
   * eq. 2d  P:L64   p^{k+1/2} = p^{k-1/2} + Phi             -> ``pressure_update``
   * eq. 4   P:L87 and Listing 1 P:L142-205 (``chkdt``)     -> ``chkdt_fields``, ``chkdt``
+  * eq. 3b  P:L73, P:L106 (implicit diffusion: "solved with the same type of direct solver")
+                                                           -> ``z_face_coefficients``, ``helmholtz_solve``
 
 The paper delegates the eigenfunction tables to its refs [11,17], which are
 not available; the tables below are the DESIGN.md reading S1 and are *pinned* in
@@ -40,6 +42,7 @@ __all__ = [
     "pair_of", "basis", "z_coefficients", "z_matrix_rows", "thomas",
     "apply_laplacian", "poisson_solve", "divergence", "correct_velocity",
     "projection", "is_singular", "uniform_spacing", "pressure_update", "chkdt_fields", "chkdt",
+    "z_face_coefficients", "helmholtz_solve",
 ]
 
 
@@ -446,3 +449,72 @@ def chkdt(u, v, w, lx, ly, lz, bc, dzc=None, dzf=None, lower_face=None):
     on the host as min(1.65 dl^2 / nu, sqrt(3) / dti)."""
     dtix, dtiy, dtiz = chkdt_fields(u, v, w, lx, ly, lz, bc, dzc, dzf, lower_face)
     return float(max(0.0, dtix.max(), dtiy.max(), dtiz.max()))
+
+
+# --------------------------------------------------------------------------------------
+# NEXT row f4: the Helmholtz solve of the implicit-diffusion step (eq. 3b, P:L73; "solved with the same type of
+# direct solver", P:L106):  (L + alpha I) Phi = f,  alpha = -2/(gamma_k nu dt) < 0 after dividing eq. 3b by -gamma nu dt/2
+# --------------------------------------------------------------------------------------
+def z_face_coefficients(dzc, dzf, periodic):
+    """Second difference in z of a quantity living on the +z FACES (the wall-normal velocity w, staggered arrangement
+    P:L53): face k sits between centres k and k+1, at distance dzf_k from the face below and dzf_{k+1} from the one
+    above, and its control volume has height dzc_{k+1}:
+        (d_zz w)_k = [ (w_{k+1} - w_k)/dzf_{k+1} - (w_k - w_{k-1})/dzf_k ] / dzc_{k+1}
+    => a_k = 1/(dzc_{k+1} dzf_k), c_k = 1/(dzc_{k+1} dzf_{k+1}) (dzf wrapped if periodic).  Non-periodic: the unknowns are
+    the interior faces k = 0..nz-2 (the face nz-1 is the upper wall); the last returned entry is unused."""
+    dzc = np.asarray(dzc, dtype=np.float64)
+    dzf = np.asarray(dzf, dtype=np.float64)
+    nz = dzf.shape[0]
+    up = np.roll(dzf, -1) if periodic else np.concatenate([dzf[1:], [np.inf]])
+    a = 1.0 / (dzc[1:] * dzf)
+    c = 1.0 / (dzc[1:] * up)
+    return a, c
+
+
+def helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc=None, dzf=None, stagger=None):
+    """(L + alpha I) Phi = f with the eigenfunction expansion of eq. 6: the same transforms in x and y, the
+    tridiagonal systems shifted by lam_qr + alpha.  alpha < 0 (eq. 3b); with alpha = 0 this is ``poisson_solve`` for a
+    non-singular boundary set.  ``bc`` is the ghost rule of the unknown itself ('D': zero on the boundary face, e.g. a
+    no-slip wall for a tangential velocity; 'N': zero normal derivative; 'P').
+
+    ``stagger`` = None for a cell-centred unknown, or the direction (0, 1, 2) along which the unknown lives on the
+    faces (u: 0, v: 1, w: 2 -- "face-located unknowns in the wall-normal direction").  Along a periodic direction the
+    operator is the same as for centres (x, y uniform).  Along z: rows of ``z_face_coefficients``; 'PP' cyclic, 'DD' = walls
+    at the lower boundary and at face nz-1 (homogeneous: the wall values do not enter the right-hand side), slot nz-1 is
+    returned as it came.  Other staggered cases (face-located along a non-periodic x or y, or z pairs with 'N') are not
+    implemented (they need the node-based DST-I / DCT-I family): NotImplementedError."""
+    f = np.asarray(f, dtype=np.float64)
+    nz, ny, nx = f.shape
+    if dzc is None or dzf is None:
+        dzc, dzf = uniform_spacing(nz, lz)
+    dzc = np.asarray(dzc, dtype=np.float64)
+    dzf = np.asarray(dzf, dtype=np.float64)
+    dx, dy = lx / nx, ly / ny
+    px, py, pz = pair_of(bc[0]), pair_of(bc[1]), pair_of(bc[2])
+    if stagger in (0, 1) and (px, py)[stagger] != "PP":
+        raise NotImplementedError("face-located unknowns along a non-periodic x or y")
+    if stagger == 2 and pz not in ("PP", "DD"):
+        raise NotImplementedError("face-located unknowns along z need PP or DD")
+    Bx, lamx, wx = basis(px, nx)
+    By, lamy, wy = basis(py, ny)
+    fh = np.matmul(By, np.matmul(f, Bx.T))
+    lam = lamy[:, None] / dy**2 + lamx[None, :] / dx**2 + alpha
+    n_solve = nz
+    if stagger == 2:
+        a, c = z_face_coefficients(dzc, dzf, pz == "PP")
+        b = -(a + c)
+        if pz == "DD":
+            n_solve = nz - 1                   # wall nodes below face 0 and at face nz-1: their couplings drop out
+            a, b, c = a[:n_solve], b[:n_solve], c[:n_solve]
+        solver = _cyclic_thomas if pz == "PP" else thomas
+    elif pz == "PP":
+        a, c = z_coefficients(dzc, dzf)
+        b = -(a + c)
+        solver = _cyclic_thomas
+    else:
+        a, b, c = z_matrix_rows(pz, dzc, dzf)
+        solver = thomas
+    ph = np.array(fh, copy=True)
+    ph[:n_solve] = solver(a, b[:, None, None] + lam[None, :, :], c, fh[:n_solve])
+    ph = np.matmul(By.T * wy[None, :], ph)
+    return np.matmul(ph, wx[:, None] * Bx)

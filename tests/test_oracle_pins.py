@@ -585,3 +585,100 @@ def test_chkdt_boundaries():
     v = np.ones((nz, ny, nx))
     fx, _, _ = orc.chkdt_fields(z, v, z, lx, ly, lz, bcn)
     assert fx[1, 2, nx - 1] == 0.5 / dy and fx[1, 2, 0] == 1.0 / dy and fx[1, 0, 0] == 0.5 / dy
+
+
+# ----------------------------------------------------------------------------------------------
+# NEXT row f4: the Helmholtz solve of eq. 3b, cell-centred and with the unknown on the z faces
+# ----------------------------------------------------------------------------------------------
+def face_second_difference_1d(nz, dzc, dzf, periodic):
+    """nz x nz matrix of the second difference of a FACE-located quantity, written from the geometry alone: face k at
+    height zf_{k+1}, neighbours dzf_k below and dzf_{k+1} above, control volume dzc_{k+1}.  Non-periodic: wall nodes below
+    face 0 and at face nz-1 (value 0), so row nz-1 is left empty."""
+    M = np.zeros((nz, nz))
+    rows = nz if periodic else nz - 1
+    for k in range(rows):
+        lo = 1.0 / (dzc[k + 1] * dzf[k])
+        up = 1.0 / (dzc[k + 1] * dzf[(k + 1) % nz])
+        M[k, k] = -(lo + up)
+        if periodic:
+            M[k, (k - 1) % nz] += lo
+            M[k, (k + 1) % nz] += up
+        else:
+            if k - 1 >= 0:
+                M[k, k - 1] += lo
+            if k + 1 <= nz - 2:
+                M[k, k + 1] += up
+    return M
+
+
+@pytest.mark.parametrize("grid", ["uniform", "stretched"])
+def test_helmholtz_vs_dense_lu(grid):
+    nx, ny, nz = 6, 8, 7
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc, dzf = orc.uniform_spacing(nz, lz) if grid == "uniform" else stretched(nz, lz, 1.6)
+    rng = np.random.default_rng(23)
+    Ix, Iy, Iz = np.eye(nx), np.eye(ny), np.eye(nz)
+    # cell-centred unknown: every boundary combination, two shifts
+    for px, py, pz in itertools.product(PAIRS_XY, PAIRS_XY, PAIRS_Z):
+        bc = bc_of(px, py, pz)
+        if pz == "PP":
+            dzc_u = dzc.copy(); dzc_u[0] = dzc_u[-1] = 0.5 * (dzf[0] + dzf[-1])
+        else:
+            dzc_u = dzc
+        M = laplacian_matrix(nx, ny, nz, lx, ly, lz, bc, dzc_u, dzf)
+        f = rng.uniform(-1, 1, (nz, ny, nx))
+        for alpha in (-0.37, -2.0e4):
+            ref = np.linalg.solve(M + alpha * np.eye(M.shape[0]), f.ravel()).reshape(f.shape)
+            got = orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc_u, dzf)
+            assert np.max(np.abs(got - ref)) < 2e-12 * np.max(np.abs(ref)), (px, py, pz, alpha)
+    # unknown on the z faces (w): walls (DD) and periodic, x / y any pair
+    for px, py, pz in itertools.product(["PP", "DD", "ND"], ["PP", "NN"], ["DD", "PP"]):
+        bc = bc_of(px, py, pz)
+        dzc_u = dzc.copy()
+        if pz == "PP":
+            dzc_u[0] = dzc_u[-1] = 0.5 * (dzf[0] + dzf[-1])
+        Lx = second_difference_1d(nx, px) / (lx / nx) ** 2
+        Ly = second_difference_1d(ny, py) / (ly / ny) ** 2
+        Lz = face_second_difference_1d(nz, dzc_u, dzf, pz == "PP")
+        f = rng.uniform(-1, 1, (nz, ny, nx))
+        alpha = -3.5
+        rows = np.ones(nz) if pz == "PP" else np.concatenate([np.ones(nz - 1), [0.0]])     # row nz-1 of DD: identity
+        R = np.diag(rows)
+        M = (np.kron(R, np.kron(Iy, Lx)) + np.kron(R, np.kron(Ly, Ix)) + np.kron(Lz, np.kron(Iy, Ix))
+             + np.kron(alpha * R + (Iz - R), np.kron(Iy, Ix)))
+        ref = np.linalg.solve(M, f.ravel()).reshape(f.shape)
+        got = orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc_u, dzf, stagger=2)
+        assert np.max(np.abs(got - ref)) < 2e-12 * np.max(np.abs(ref)), (px, py, pz)
+        if pz == "DD":
+            assert np.max(np.abs(got[-1] - f[-1])) < 1e-13                # the wall slot comes back as it went in
+    # staggered along a periodic x or y: same operator as for centres
+    bc = bc_of("PP", "PP", "DD")
+    f = rng.uniform(-1, 1, (nz, ny, nx))
+    assert np.array_equal(orc.helmholtz_solve(f, -1.0, lx, ly, lz, bc, dzc, dzf, stagger=0),
+                          orc.helmholtz_solve(f, -1.0, lx, ly, lz, bc, dzc, dzf))
+    with pytest.raises(NotImplementedError):
+        orc.helmholtz_solve(f, -1.0, lx, ly, lz, bc_of("NN", "PP", "DD"), dzc, dzf, stagger=0)
+    with pytest.raises(NotImplementedError):
+        orc.helmholtz_solve(f, -1.0, lx, ly, lz, bc_of("PP", "PP", "NN"), dzc, dzf, stagger=2)
+
+
+def test_helmholtz_closed_forms():
+    """(i) a constant right-hand side under all-Neumann / periodic conditions: L c = 0, so Phi = f / alpha exactly;
+    (ii) alpha -> 0 on a non-singular boundary set reproduces the Poisson solve; (iii) eq. 3b itself: with
+    alpha = -2/(gamma nu dt) and f = -rhs * 2/(gamma nu dt), u* - (gamma nu dt/2) L u* = rhs to rounding."""
+    nx, ny, nz = 8, 6, 9
+    lx, ly, lz = 1.0, 2.0, 1.5
+    dzc, dzf = stretched(nz, lz, 1.3)
+    f = np.full((nz, ny, nx), 2.5)
+    got = orc.helmholtz_solve(f, -4.0, lx, ly, lz, bc_of("PP", "NN", "NN"), dzc, dzf)
+    assert np.max(np.abs(got - 2.5 / -4.0)) < 1e-14
+    rng = np.random.default_rng(2)
+    f = rng.standard_normal((nz, ny, nx))
+    bc = bc_of("PP", "DD", "DN")
+    assert np.max(np.abs(orc.helmholtz_solve(f, 0.0, lx, ly, lz, bc, dzc, dzf) - orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf))) < 1e-15
+    gamma, nu, dt = 8.0 / 15.0, 1e-3, 2e-2
+    cdiff = gamma * nu * dt / 2
+    rhs = rng.standard_normal((nz, ny, nx))
+    ustar = orc.helmholtz_solve(-rhs / cdiff, -1.0 / cdiff, lx, ly, lz, bc, dzc, dzf)
+    back = ustar - cdiff * orc.apply_laplacian(ustar, lx, ly, lz, bc, dzc, dzf)
+    assert np.max(np.abs(back - rhs)) < 1e-12
