@@ -37,7 +37,7 @@ typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the li
 /* Return codes of the int-valued entry points. */
 #define CANS_OK                    0
 #define CANS_ERR_INVALID_ARG       1   /* null pointer, n < 2, non-positive length/spacing/dt, bad bc letter, one-sided 'P' */
-#define CANS_ERR_UNSUPPORTED_BC    2   /* reserved (no longer returned: every boundary pair is implemented) */
+#define CANS_ERR_UNSUPPORTED_BC    2   /* face-located unknown along a direction the Helmholtz plan does not implement */
 #define CANS_ERR_UNSUPPORTED_SIZE  3   /* nx or ny not in the instantiated transform sizes, or nz too large */
 #define CANS_ERR_ALLOC             4   /* device or host allocation failed */
 #define CANS_ERR_CUDA              5   /* a CUDA runtime call or kernel launch failed */
@@ -70,6 +70,30 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz,
                                             double lx, double ly, double lz,
                                             const char bc[3][2],
                                             const double* dzc, const double* dzf);
+
+/*
+ * cans_helmholtz_plan_create / cans_helmholtz_solve -- the Helmholtz solves of the implicit-diffusion step (SURVEY 8f row
+ * f4): eq. 3b, u* - (gamma nu dt / 2) L u* = rhs, "solved with the same type of direct solver".  Divided by
+ * -(gamma nu dt / 2) it reads (L + alpha I) Phi = f with alpha = -2/(gamma nu dt) < 0 and f = alpha * rhs: the same three
+ * passes as cans_poisson_solve with every tridiagonal system shifted by alpha (never singular).
+ *
+ *   bc       here the ghost rule of the UNKNOWN (a velocity component), not of the pressure: 'D' = zero on the boundary face
+ *            (no-slip wall for a tangential component), 'N' = zero normal derivative (free slip / outflow), 'P' periodic.
+ *   stagger  -1: the unknown lives at the cell centres in every direction (cans_poisson_plan_create is this case);
+ *            0, 1, 2: it lives on the +x / +y / +z faces (u, v, w of the staggered arrangement).  Along a periodic
+ *            direction the operator is the one for centres.  stagger = 2 with z walls ('D','D'): faces 0..nz-2 are the
+ *            unknowns, the wall nodes below face 0 and at face nz-1 are homogeneous (a moving wall is folded into f by the
+ *            caller) and slot nz-1 of q is returned as it came; stagger = 2 with periodic z: cyclic systems.  Every other
+ *            face-located case (non-periodic x or y: node-based DST-I / DCT-I; z pairs containing 'N') returns NULL with
+ *            CANS_ERR_UNSUPPORTED_BC.
+ *   q        DEVICE, nx*ny*nz doubles: f on entry, Phi on exit.     alpha < 0.
+ * The pivots entering each z segment depend on alpha: the plan rebuilds that table (N/16 doubles, one extra kernel on the
+ * caller's stream) whenever alpha differs from the previous call's; a time loop with the three RK3 values gamma_k should
+ * keep one plan per substep and component, or accept the rebuild.  A stagger = 2 plan serves cans_helmholtz_solve only.
+ */
+cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
+                                              const char bc[3][2], const double* dzc, const double* dzf, int stagger);
+int cans_helmholtz_solve(cans_poisson_plan* plan, double* q, double alpha, void* stream);
 
 /* Free the plan and its device tables.  NULL is ignored.  Outstanding work must have completed. */
 void cans_poisson_plan_destroy(cans_poisson_plan* plan);

@@ -25,7 +25,7 @@ MAX_KERNEL_RECORDS = 16      # CANS_MAX_KERNEL_RECORDS of the header
 
 EXPORTED_SYMBOLS = (
     "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
-    "cans_projection_step", "cans_chkdt",
+    "cans_projection_step", "cans_chkdt", "cans_helmholtz_plan_create", "cans_helmholtz_solve",
     "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
@@ -68,6 +68,10 @@ def _load() -> ctypes.CDLL:
     lib.cans_plan_launches_per_solve.argtypes = [vp]
     lib.cans_plan_launches_per_projection.restype = i32
     lib.cans_plan_launches_per_projection.argtypes = [vp]
+    lib.cans_helmholtz_plan_create.restype = vp
+    lib.cans_helmholtz_plan_create.argtypes = lib.cans_poisson_plan_create.argtypes + [i32]
+    lib.cans_helmholtz_solve.restype = i32
+    lib.cans_helmholtz_solve.argtypes = [vp, vp, ctypes.c_double, vp]
     lib.cans_projection_step.restype = i32
     lib.cans_projection_step.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_double, vp, vp]
     lib.cans_chkdt.restype = i32
@@ -126,7 +130,8 @@ class PoissonPlan:
     """cans_poisson_plan_create / _destroy.  Fields are torch CUDA float64 tensors of shape (nz, ny, nx)."""
 
     def __init__(self, nx: int, ny: int, nz: int, lx: float, ly: float, lz: float, bc,
-                 dzc: Optional[Sequence[float]] = None, dzf: Optional[Sequence[float]] = None):
+                 dzc: Optional[Sequence[float]] = None, dzf: Optional[Sequence[float]] = None,
+                 stagger: Optional[int] = None):
         self.shape = (nz, ny, nx)
         self._h = None
         dzc_t = dzf_t = None
@@ -141,7 +146,10 @@ class PoissonPlan:
             if dzf_t.numel() != nz:
                 raise ValueError("dzf must have nz entries")
             pf = dzf_t.data_ptr()
-        h = _lib.cans_poisson_plan_create(nx, ny, nz, float(lx), float(ly), float(lz), _bc_bytes(bc), pc, pf)
+        if stagger is None:
+            h = _lib.cans_poisson_plan_create(nx, ny, nz, float(lx), float(ly), float(lz), _bc_bytes(bc), pc, pf)
+        else:       # cans_helmholtz_plan_create: the unknown lives on the faces of direction `stagger` (-1: centres)
+            h = _lib.cans_helmholtz_plan_create(nx, ny, nz, float(lx), float(ly), float(lz), _bc_bytes(bc), pc, pf, int(stagger))
         if not h:
             raise CansError(_lib.cans_last_status(), last_error())
         self._h = h
@@ -161,6 +169,10 @@ class PoissonPlan:
     def poisson_solve(self, p: torch.Tensor, stream=None):
         """cans_poisson_solve: p (f on entry) is overwritten with Phi."""
         _check(_lib.cans_poisson_solve(self._h, _dev_ptr(p, self.shape), _stream_ptr(stream)))
+
+    def helmholtz_solve(self, q: torch.Tensor, alpha: float, stream=None):
+        """cans_helmholtz_solve: q (f on entry) is overwritten with Phi, (L + alpha I) Phi = f, alpha < 0 (eq. 3b)."""
+        _check(_lib.cans_helmholtz_solve(self._h, _dev_ptr(q, self.shape), float(alpha), _stream_ptr(stream)))
 
     def projection(self, u, v, w, p, dt: float, stream=None):
         """cans_projection: u, v, w corrected in place, p overwritten with Phi."""

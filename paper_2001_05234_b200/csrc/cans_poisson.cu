@@ -179,6 +179,9 @@ struct cans_poisson_plan {
     char bc[3][2];
     int kind_x, kind_y;
     int singular;
+    int stagger;              // -1: cell-centred unknown; 0, 1, 2: the unknown lives on the faces of that direction (eq. 3b)
+    int nz_solve;             // rows of the tridiagonal systems (nz, or nz - 1 for a face-located unknown between walls)
+    double alpha_tables;      // Helmholtz shift the pivot tables rstart / r00 were built for
     int cyclic;               // z periodic: cyclic tridiagonal systems (z_pass.cuh)
     double a0w, cw;           // their wrap couplings
     int nseg, nzp;
@@ -249,8 +252,10 @@ static cudaError_t upload(cans_poisson_plan* pl, const std::vector<double>& h, T
 // layout of the scheduler state (unsigned ints)
 enum { SCHED_Z_TICKET = 0, SCHED_WORDS = 8 };
 
-static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
+static ZArgs make_zargs(const cans_poisson_plan* pl, double* p, double alpha = 0.0) {
     ZArgs z;
+    z.alpha = alpha;
+    z.nz_solve = pl->nz_solve;
     z.nx = pl->nx; z.ny = pl->ny; z.nz = pl->nz;
     z.nseg = pl->nseg;
     z.ncols = (long)pl->nx * pl->ny;
@@ -259,7 +264,7 @@ static ZArgs make_zargs(const cans_poisson_plan* pl, double* p) {
     z.az = pl->az; z.bz = pl->bz; z.cz = pl->cz; z.gz = pl->gz;
     z.rstart = pl->rstart;
     z.scale = 1.0 / ((double)pl->nx * (double)pl->ny);
-    z.singular = pl->singular;
+    z.singular = pl->singular && alpha == 0.0;
     z.r00 = pl->r00;
     z.dzf = pl->dzf;
     z.inv_lz = pl->inv_lz;
@@ -335,6 +340,11 @@ void cans_poisson_plan_destroy(cans_poisson_plan* plan) {
 
 cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
                                             const char bc[3][2], const double* dzc, const double* dzf) {
+    return cans_helmholtz_plan_create(nx, ny, nz, lx, ly, lz, bc, dzc, dzf, -1);
+}
+
+cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
+                                              const char bc[3][2], const double* dzc, const double* dzf, int stagger) {
     g_status = CANS_OK;
     g_err.clear();
     if (!bc) { fail(CANS_ERR_INVALID_ARG, "bc is NULL"); return nullptr; }
@@ -351,6 +361,15 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     int kx, ky;
     if (kind_of(bc[0][0], bc[0][1], &kx) != CANS_OK || kind_of(bc[1][0], bc[1][1], &ky) != CANS_OK) {
         fail(CANS_ERR_INVALID_ARG, "unknown boundary pair");
+        return nullptr;
+    }
+    if (stagger < -1 || stagger > 2) { fail(CANS_ERR_INVALID_ARG, "stagger must be -1, 0, 1 or 2"); return nullptr; }
+    if ((stagger == 0 || stagger == 1) && bc[stagger][0] != 'P') {
+        fail(CANS_ERR_UNSUPPORTED_BC, "an unknown on the faces of a non-periodic x or y direction needs the node-based DST-I / DCT-I transforms (not implemented)");
+        return nullptr;
+    }
+    if (stagger == 2 && !((bc[2][0] == 'P') || (bc[2][0] == 'D' && bc[2][1] == 'D'))) {
+        fail(CANS_ERR_UNSUPPORTED_BC, "an unknown on the z faces is implemented between walls ('D','D') and for periodic z");
         return nullptr;
     }
     FftRadices fx, fy;
@@ -383,13 +402,16 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     pl->tmap_field = nullptr;
     pl->singular = (kx == KIND_PP || kx == KIND_NN) && (ky == KIND_PP || ky == KIND_NN) && bc[2][0] != 'D' && bc[2][1] != 'D';
     pl->cyclic = bc[2][0] == 'P';
+    pl->stagger = stagger;
+    pl->nz_solve = (stagger == 2 && bc[2][0] == 'D') ? nz - 1 : nz;
+    pl->alpha_tables = 0.0;
     pl->device = 0;
     cudaGetDevice(&pl->device);
     pl->num_sms = 148;
     cudaDeviceGetAttribute(&pl->num_sms, cudaDevAttrMultiProcessorCount, pl->device);
 
     const double dx = lx / nx, dy = ly / ny;
-    ZRows zr = make_z_rows(nz, pl->nzp, hdzc.data(), hdzf.data(), bc[2][0], bc[2][1]);
+    ZRows zr = make_z_rows(nz, pl->nzp, hdzc.data(), hdzf.data(), bc[2][0], bc[2][1], stagger == 2);
     pl->inv_lz = 1.0 / zr.lz_sum;
     pl->a0w = zr.a0w; pl->cw = zr.cw;
     std::vector<double> rdzc(nz);
@@ -439,7 +461,8 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     }
     if (e == cudaSuccess) {
         ZArgs z = make_zargs(pl, nullptr);
-        e = z_setup_launch(z, pl->rstart, pl->r00);
+        e = z_setup_launch(z, pl->rstart, pl->r00, 0);
+        if (e == cudaSuccess) e = cudaDeviceSynchronize();
     }
     const int rc = CANS_OK;
     if (e == cudaSuccess) e = z_solve_configure(nseg, pl->cyclic, pl->num_sms, &pl->z_grid, &pl->z_smem);
@@ -456,8 +479,16 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz, double lx, d
     return pl;
 }
 
-static int launch_z(cans_poisson_plan* pl, double* p, cudaStream_t st) {
-    ZArgs z = make_zargs(pl, p);
+static int launch_z(cans_poisson_plan* pl, double* p, double alpha, cudaStream_t st) {
+    ZArgs z = make_zargs(pl, p, alpha);
+    if (alpha != pl->alpha_tables) {
+        // the segment-start pivots depend on the shift: rebuild the table on this stream (one sweep per column, no field
+        // data: ~N/16 doubles written) before the solve that uses it
+        LaunchScope scope(pl, st, "z_setup");
+        cudaError_t e = z_setup_launch(z, pl->rstart, pl->r00, st);
+        if (e != cudaSuccess) return fail_cuda(e, "z pivot table launch");
+        pl->alpha_tables = alpha;
+    }
     LaunchScope scope(pl, st, "z_solve");
     cudaError_t e = z_solve_launch(z, pl->z_grid, pl->z_smem, &pl->tmap_z, st);
     if (e != cudaSuccess) return fail_cuda(e, "z solve launch");
@@ -486,7 +517,8 @@ static int ensure_tensor_maps(cans_poisson_plan* pl, double* p) {
 
 // the whole path shared by both entry points; `divargs` selects the fused-divergence load (a1),
 // `grad` the velocity correction (a7)
-static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st) {
+static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, const GradArgs* grad, cudaStream_t st,
+                    double alpha = 0.0) {
     int rc;
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev != pl->device)
@@ -500,7 +532,7 @@ static int run_core(cans_poisson_plan* pl, double* p, const XYArgs* divargs, con
     else rc = launch_xy_any(pl, pl->nx, OP_X_FWD, ax, st);                          // a2
     if (rc) return rc;
     if ((rc = launch_xy_any(pl, pl->ny, OP_Y_FWD, ay, st))) return rc;              // a3
-    if ((rc = launch_z(pl, p, st))) return rc;                                      // a4
+    if ((rc = launch_z(pl, p, alpha, st))) return rc;                               // a4
     if ((rc = launch_xy_any(pl, pl->ny, OP_Y_INV, ay, st))) return rc;              // a5
     if ((rc = launch_xy_any(pl, pl->nx, OP_X_INV, ax, st))) return rc;              // a6
     if (grad) return launch_grad(pl, *grad, st);                                    // a7
@@ -519,7 +551,16 @@ int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream) {
     g_status = CANS_OK;
     if (!plan || !p) return fail(CANS_ERR_INVALID_ARG, "plan and p must be non-NULL");
     if ((reinterpret_cast<size_t>(p) & 15) != 0) return fail(CANS_ERR_INVALID_ARG, "p must be 16-byte aligned");
+    if (plan->stagger == 2) return fail(CANS_ERR_INVALID_ARG, "a plan for an unknown on the z faces solves cans_helmholtz_solve only");
     return run_core(plan, p, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+int cans_helmholtz_solve(cans_poisson_plan* plan, double* q, double alpha, void* stream) {
+    g_status = CANS_OK;
+    if (!plan || !q) return fail(CANS_ERR_INVALID_ARG, "plan and q must be non-NULL");
+    if ((reinterpret_cast<size_t>(q) & 15) != 0) return fail(CANS_ERR_INVALID_ARG, "q must be 16-byte aligned");
+    if (!(alpha < 0.0)) return fail(CANS_ERR_INVALID_ARG, "alpha must be < 0 (eq. 3b: alpha = -2/(gamma nu dt))");
+    return run_core(plan, q, nullptr, nullptr, (cudaStream_t)stream, alpha);
 }
 
 static int chkdt_enqueue(cans_poisson_plan* plan, const double* u, const double* v, const double* w, double* dti, cudaStream_t st);
@@ -569,6 +610,7 @@ int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* 
                          double* dti, void* stream) {
     g_status = CANS_OK;
     if (!plan || !u || !v || !w || !p) return fail(CANS_ERR_INVALID_ARG, "plan, u, v, w, p must be non-NULL");
+    if (plan->stagger == 2) return fail(CANS_ERR_INVALID_ARG, "a plan for an unknown on the z faces solves cans_helmholtz_solve only");
     if (p_acc && ((reinterpret_cast<size_t>(p_acc) & 15) != 0 || p_acc == p))
         return fail(CANS_ERR_INVALID_ARG, "p_acc must be 16-byte aligned and distinct from p");
     if (!(dt > 0.0)) return fail(CANS_ERR_INVALID_ARG, "dt must be > 0");

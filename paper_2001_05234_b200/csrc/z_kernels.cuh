@@ -20,7 +20,8 @@ cudaError_t z_solve_configure(int nseg, int cyclic, int num_sms, int* grid_out, 
 cudaError_t z_make_tensor_map(CUtensorMap* tmap, const double* p, long ncols, int nz, int nseg);
 // enqueue the solve (a.ticket must point at a zeroed counter; tmap from z_make_tensor_map for a.p)
 cudaError_t z_solve_launch(const ZArgs& a, int grid, size_t smem, const CUtensorMap* tmap, cudaStream_t st);
-// plan time: fill rstart / r00 (synchronous)
-cudaError_t z_setup_launch(const ZArgs& a, double* rstart, double* r00);
+// fill rstart / r00 for the shift a.alpha (enqueued on st: at plan time for alpha = 0, again whenever a Helmholtz solve
+// changes the shift)
+cudaError_t z_setup_launch(const ZArgs& a, double* rstart, double* r00, cudaStream_t st);
 
 }  // namespace cans

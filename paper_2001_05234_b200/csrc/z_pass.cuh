@@ -54,6 +54,9 @@ struct ZArgs {
     const double* dzf;        // [nz]
     double inv_lz;            // 1 / sum(dzf)
     unsigned int* ticket;     // tile ticket counter (zeroed before the launch)
+    double alpha;             // Helmholtz shift added to every eigenvalue (eq. 3b): (L + alpha I) Phi = f; 0 for eq. 5
+    int nz_solve;             // rows [0, nz_solve) form the tridiagonal system; rows [nz_solve, nz) are passed through
+                              // (scaled): the wall slot of a face-located unknown (nz_solve = nz - 1), else nz_solve = nz
     int cyclic;               // 1: z is periodic (az[0] = cz[nz-1] = 0 in the tables, the wrap couplings are below)
     double a0w, cw;           // a_0 = 1/(dzf_0 dzc_0) and c_{nz-1} = 1/(dzf_{nz-1} dzc_nz) of the cyclic system
     int nbox, box_rows;       // TMA tiling of a column tile: nbox boxes of box_rows rows (set by z_solve_launch)
@@ -206,7 +209,8 @@ struct ZPass {
     // phase 3: scan from the bottom -> true x below the segment; propagate; DEST 0: store to the field (open system),
     // 1: store to the shared-memory buffer qbuf (cyclic: the correction vector q), 2: keep in st.d (cyclic: y)
     template <int DEST>
-    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, double* qbuf = nullptr) {
+    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, double* qbuf = nullptr,
+                               const double* buf = nullptr) {
         const int nzp = a.nseg * MROWS;
         const double* scz = sm + 2 * nzp;
         const double2* s_scan = reinterpret_cast<const double2*>(sm + 4 * nzp + 2 * TC * a.nseg);   // backward pairs
@@ -231,7 +235,8 @@ struct ZPass {
 #pragma unroll
                 for (int r = 0; r < MROWS; ++r) {
                     const int k = k0 + r;
-                    if (k < a.nz) a.p[(size_t)k * plane + st.col] = st.d[r];
+                    // (the tile buffer still holds this tile: its buffer is not refilled before the next iteration)
+                    if (k < a.nz) a.p[(size_t)k * plane + st.col] = (k < a.nz_solve) ? st.d[r] : buf[(size_t)k * TC + c] * a.scale;
                 }
             } else if (DEST == 1) {
 #pragma unroll
@@ -276,7 +281,7 @@ template <int MROWS>
 CANS_HD void z_setup_column(const ZArgs& a, double* rstart_out, double* r00_out, long col) {
     const int i = (int)(col % a.nx);
     const int j = (int)(col / a.nx);
-    const double lam = a.lamx[i] + a.lamy[j];
+    const double lam = a.lamx[i] + a.lamy[j] + a.alpha;
     double rp = 0.0;
     const int nzp = a.nseg * MROWS;
     for (int k = 0; k < nzp; ++k) {

@@ -79,7 +79,7 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
         ZState<MROWS> st;
         if (CYC) {
             // the correction vector q of this tile's modes (needs no field data) while the tile is still in flight
-            Z::template phase1<1>(a, zsm, nullptr, st, cur, rs, l1 + l2, tid);
+            Z::template phase1<1>(a, zsm, nullptr, st, cur, rs, l1 + l2 + a.alpha, tid);
             __syncthreads();
             Z::phase2a(a, zsm, st, tid);
             Z::phase2b(a, zsm, st, tid);
@@ -88,8 +88,8 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
         }
         mbar_wait(&s_bar[b], (phases >> b) & 1u);   // the current tile has landed (the next may still fly)
         phases ^= 1u << b;
-        if (CYC) Z::template phase1<2>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2, tid);
-        else Z::template phase1<0>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2, tid);
+        if (CYC) Z::template phase1<2>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2 + a.alpha, tid);
+        else Z::template phase1<0>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2 + a.alpha, tid);
         __syncthreads();
         // every thread has read s_next (before the barrier above): thread 0 may now draw the ticket after next
         if (tid == 0 && nxt < a.ntiles) s_next = (long)atomicAdd(a.ticket, 1u);
@@ -100,9 +100,9 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
             Z::template phase3<2>(a, zsm, st, tid);
             Z::cyclic_publish(a, zsm, st, tid);
             __syncthreads();
-            Z::cyclic_store(a, zsm, st, l1 + l2, tid, qbuf);
+            Z::cyclic_store(a, zsm, st, l1 + l2 + a.alpha, tid, qbuf);
         } else {
-            Z::template phase3<0>(a, zsm, st, tid);
+            Z::template phase3<0>(a, zsm, st, tid, nullptr, bufs + (size_t)b * tile_sz);
         }
         if (nxt >= a.ntiles) break;
         cur = nxt;
@@ -180,11 +180,9 @@ cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, const CUten
     return cudaGetLastError();
 }
 
-cudaError_t z_setup_launch(const ZArgs& a, double* rstart, double* r00) {
-    z_setup_kernel<Z_MROWS><<<(unsigned)((a.ncols + 127) / 128), 128>>>(a, rstart, r00);
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) e = cudaDeviceSynchronize();
-    return e;
+cudaError_t z_setup_launch(const ZArgs& a, double* rstart, double* r00, cudaStream_t st) {
+    z_setup_kernel<Z_MROWS><<<(unsigned)((a.ncols + 127) / 128), 128, 0, st>>>(a, rstart, r00);
+    return cudaGetLastError();
 }
 
 }  // namespace cans

@@ -63,6 +63,18 @@ def test_plan_create_rejects_bad_arguments_without_a_gpu(binding, kwargs, status
     assert binding.last_error() != ""
 
 
+@pytest.mark.parametrize("bc,stagger,status", [
+    ((("N", "N"), ("P", "P"), ("D", "D")), 0, 2),      # faces along a non-periodic x: DST-I / DCT-I family, not implemented
+    ((("P", "P"), ("D", "N"), ("D", "D")), 1, 2),
+    ((("P", "P"), ("P", "P"), ("N", "N")), 2, 2),      # faces along z: walls or periodic only
+    ((("P", "P"), ("P", "P"), ("D", "D")), 3, 1),
+])
+def test_helmholtz_plan_rejects_unsupported_staggering_without_a_gpu(binding, bc, stagger, status):
+    with pytest.raises(binding.CansError) as ei:
+        binding.PoissonPlan(32, 32, 32, 1.0, 1.0, 1.0, bc, stagger=stagger)
+    assert ei.value.status == status
+
+
 def test_host_tables_match_their_definitions():
     """plan_tables.hpp is host logic: compile it with g++ and check twiddles / eigenvalue tables against
     closed forms (cos/sin of exact rational angles; sum of eigenvalues = trace of the stencil matrix)."""

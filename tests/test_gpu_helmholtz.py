@@ -1,0 +1,115 @@
+"""GPU parity of the Helmholtz variant (eq. 3b) against the CPU oracle."""
+import itertools
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import cans_oracle as orc
+from paper_2001_05234_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+REL_L2 = 1e-11
+MAX_ABS = 1e-10
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2001_05234_b200 import binding
+    return binding
+
+
+def check(got, ref, what):
+    rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
+    assert rel <= REL_L2, f"{what}: rel-L2 {rel:.3e}"
+    # f = O(1) and |alpha| >= 0.3: |Phi| <= |f| / |alpha| stays O(1) or below, the absolute bar applies to Phi directly
+    assert np.max(np.abs(got - ref)) <= MAX_ABS, f"{what}: max-abs {np.max(np.abs(got - ref)):.3e}"
+
+
+def grid(nz, lz, stretch, periodic):
+    if stretch is None:
+        return None, None
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, stretch)
+    dzc, dzf = dzc_t.numpy().copy(), dzf_t.numpy().copy()
+    if periodic:
+        dzc[0] = dzc[-1] = 0.5 * (dzf[0] + dzf[-1])
+    return dzc, dzf
+
+
+PAIRS = ["PP", "NN", "DD", "ND", "DN"]
+
+
+@pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 32, 33, 1.6), (128, 96, 20, None), (512, 768, 6, 1.8), (32, 16, 300, 1.6)])
+def test_cell_centred_helmholtz_every_boundary_combination(B, nx, ny, nz, stretch):
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    combos = list(itertools.product(PAIRS, PAIRS, PAIRS))
+    if nx * ny * nz > 100000:
+        combos = combos[::7]
+    rng = np.random.default_rng(nx + nz)
+    for n, (px, py, pz) in enumerate(combos):
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        dzc, dzf = grid(nz, lz, stretch, pz == "PP")
+        alpha = (-0.37, -2.3e7, -4.0e3)[n % 3]          # -2/(gamma nu dt): weak shift ... channel-DNS magnitude
+        f = rng.uniform(-1, 1, (nz, ny, nx))
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        q = torch.from_numpy(f).cuda()
+        plan.helmholtz_solve(q, alpha)
+        torch.cuda.synchronize()
+        plan.close()
+        check(q.cpu().numpy(), orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc, dzf), f"{px}/{py}/{pz} alpha={alpha}")
+
+
+@pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 32, 33, 1.6), (1024, 64, 9, None), (32, 48, 512, 1.6), (32, 16, 257, 2.0)])
+def test_face_located_unknowns(B, nx, ny, nz, stretch):
+    """The three velocity components of the channel configuration: u (faces in x), v (faces in y) with no-slip walls in z
+    ('D','D', cell-centred in z), w on the z faces between the walls; and w in a triperiodic box."""
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    rng = np.random.default_rng(5 * nx + nz)
+    alpha = -1.7e5
+    cases = [(0, ("PP", "PP", "DD")), (1, ("PP", "PP", "DD")), (2, ("PP", "PP", "DD")), (2, ("NN", "DN", "DD")),
+             (2, ("PP", "PP", "PP")), (2, ("DD", "PP", "PP")), (-1, ("PP", "PP", "DD"))]
+    for stagger, (px, py, pz) in cases:
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        dzc, dzf = grid(nz, lz, stretch, pz == "PP")
+        f = rng.uniform(-1, 1, (nz, ny, nx))
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf, stagger=stagger)
+        q = torch.from_numpy(f).cuda()
+        plan.helmholtz_solve(q, alpha)
+        torch.cuda.synchronize()
+        got = q.cpu().numpy()
+        ref = orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc, dzf, stagger=None if stagger < 0 else stagger)
+        check(got, ref, f"stagger {stagger} {px}/{py}/{pz}")
+        if stagger == 2 and pz == "DD":
+            assert np.max(np.abs(got[-1] - f[-1])) <= 1e-13          # the wall slot returns as it came (transform round trip)
+            with pytest.raises(B.CansError) as ei:
+                plan.poisson_solve(q)
+            assert ei.value.status == B.CANS_ERR_INVALID_ARG
+        plan.close()
+
+
+def test_shift_changes_rebuild_the_pivot_table(B):
+    """One plan, alternating shifts and the plain Poisson solve: every call must see the pivots of its own alpha."""
+    nx, ny, nz = 96, 64, 40
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    bc = (("P", "P"), ("P", "P"), ("N", "N"))
+    dzc, dzf = grid(nz, lz, 1.6, False)
+    rng = np.random.default_rng(1)
+    f = rng.uniform(-1, 1, (nz, ny, nx))
+    f0 = f - np.sum(f * dzf[:, None, None]) / (np.sum(dzf) * nx * ny)
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    refs = {}
+    for alpha in (-10.0, 0.0, -3.0e6, -10.0, -10.0, 0.0):
+        q = torch.from_numpy(f0 if alpha == 0.0 else f).cuda()
+        if alpha == 0.0:
+            plan.poisson_solve(q)
+            ref = refs.setdefault(alpha, orc.poisson_solve(f0, lx, ly, lz, bc, dzc, dzf))
+        else:
+            plan.helmholtz_solve(q, alpha)
+            ref = refs.setdefault(alpha, orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc, dzf))
+        torch.cuda.synchronize()
+        check(q.cpu().numpy(), ref, f"alpha={alpha}")
+    with pytest.raises(B.CansError) as ei:
+        plan.helmholtz_solve(q, 0.0)
+    assert ei.value.status == B.CANS_ERR_INVALID_ARG
+    plan.close()
