@@ -38,6 +38,10 @@ KERNEL_BYTES_PER_CELL = {
     "y_inv": 16.0,
     "x_inv": 16.0,
     "grad_correct": 56.0,  # read Phi (8) + u, v, w (24), write u, v, w (24)
+    "grad_correct_pacc": 72.0,   # the same kernel also doing eq. 2d: + read and write p_acc (16)
+    "chkdt": 24.0,         # read u, v, w once
+    "face_correct": 0.0,   # O(N^(2/3)) boundary planes
+    "z_setup": 0.5,        # writes the N/16 segment-start pivots
 }
 STEP_MIN_BYTES_PER_CELL = {"projection": 112.0, "poisson": 48.0}   # structural minimum, SURVEY.md 8(d)
 
@@ -196,9 +200,12 @@ def time_poisson_config(binding, workloads, torch, name, steps=10, warmup=3):
             "gcells_per_s": cells / med / 1e6, "min_bytes": 48.0 * cells}
 
 
+PAIRS = ("PP", "NN", "DD", "ND", "DN")
+
+
 def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
     """Every supported boundary-condition combination on the C5 grid (BASELINE.json: "for every supported
-    boundary-condition combination"): Poisson solve and projection step for {PP,NN,DD}^2 x {NN,DN,ND,DD}
+    boundary-condition combination"): Poisson solve and projection step for all 5 x 5 x 5 pairs {PP,NN,DD,ND,DN}^3
     (lower 'D' sides with a registered face plane).  Median ms per call, CUDA events."""
     w = workloads.make_workload("C5", device="cuda", with_fields=False)
     nx, ny, nz = w.n
@@ -217,9 +224,9 @@ def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
         ms = sorted(a.elapsed_time(b) for a, b in ev)
         return ms[len(ms) // 2]
 
-    for px in ("PP", "NN", "DD"):
-        for py in ("PP", "NN", "DD"):
-            for pz in ("NN", "DN", "ND", "DD"):
+    for px in PAIRS:
+        for py in PAIRS:
+            for pz in PAIRS:
                 bc = (tuple(px), tuple(py), tuple(pz))
                 plan = binding.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, w.dzc, w.dzf)
                 key = f"{px}/{py}/{pz}"
@@ -238,9 +245,74 @@ def bc_sweep(binding, workloads, torch, steps=5, warmup=2):
                     lambda: plan.projection(bufs[0], bufs[1], bufs[2], bufs[3], 1e-4), reset)
                 plan.close()
     pv, jv = list(out["poisson_ms"].values()), list(out["projection_ms"].values())
+    out["combinations"] = len(pv)
     out["poisson_ms_min_max"] = [min(pv), max(pv)]
     out["projection_ms_min_max"] = [min(jv), max(jv)]
+    # the paper's own GPU transform set (DFT, DCT-II/III, DST-II/III) separately from the mixed pairs
+    core = [k for k in out["projection_ms"] if all(p in ("PP", "NN", "DD") for p in k.split("/")[:2])]
+    out["projection_ms_min_max_without_mixed_xy"] = [min(out["projection_ms"][k] for k in core),
+                                                     max(out["projection_ms"][k] for k in core)]
     return out
+
+
+def time_step_variants(binding, torch, plan, w, fields, steps=5, warmup=2):
+    """The calls around the projection in a time loop, on the C5 workload: cans_projection_step with eq. 2d fused into the
+    correction kernel and the chkdt reduction; cans_helmholtz_solve (eq. 3b) with a channel-DNS shift.  Median ms."""
+    u0, v0, w0, u, v, ww, p = fields
+    pacc = torch.zeros_like(p)
+    dti = torch.zeros((1,), dtype=torch.float64, device="cuda")
+
+    def med(fn, reset):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for _ in range(warmup):
+            reset(); fn()
+        for a, b in ev:
+            reset(); a.record(); fn(); b.record()
+        torch.cuda.synchronize()
+        ms = sorted(a.elapsed_time(b) for a, b in ev)
+        return ms[len(ms) // 2]
+
+    def restore():
+        u.copy_(u0); v.copy_(v0); ww.copy_(w0)
+
+    out = {}
+    out["projection_step_pacc_chkdt_ms"] = med(lambda: plan.projection_step(u, v, ww, p, w.dt, p_acc=pacc, dti=dti), restore)
+    out["projection_step_pacc_ms"] = med(lambda: plan.projection_step(u, v, ww, p, w.dt, p_acc=pacc), restore)
+    out["chkdt_ms"] = med(lambda: plan.chkdt(u, v, ww, dti), lambda: None)
+    out["chkdt_gbs"] = 24.0 * w.cells / (out["chkdt_ms"] * 1e-3) / 1e9
+    alpha = -2.0 / (0.5 * 1.77e-4 * 1e-3)          # -2/(gamma nu dt): gamma ~ 1/2, nu = 1/5640, dt = 1e-3
+    out["helmholtz_solve_ms"] = med(lambda: plan.helmholtz_solve(p, alpha), lambda: p.copy_(u0))
+    plan.poisson_solve(p)                           # back to the alpha = 0 pivot table
+    torch.cuda.synchronize()
+    out["helmholtz_alpha"] = alpha
+    del pacc
+    return out
+
+
+def time_paper_grid(binding, workloads, torch, steps=3, warmup=2):
+    """Context line: the paper's own grid 1536 x 768 x 576, projection step, same bc / stretching as C5.
+    nx = 1536 runs the 3-pass shared-memory transforms (no warp-level kernel for that length)."""
+    nx, ny, nz = 1536, 768, 576
+    w = workloads.make_workload("C5", device="cuda", with_fields=False, n_override=(nx, ny, nz))
+    plan = binding.plan_for(w)
+    f = torch.rand((nz, ny, nx), dtype=torch.float64, device="cuda")
+    bufs = [torch.empty_like(f) for _ in range(4)]
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for i in range(warmup + steps):
+        for b in bufs[:3]:
+            b.copy_(f)
+        if i >= warmup:
+            ev[i - warmup][0].record()
+        plan.projection(bufs[0], bufs[1], bufs[2], bufs[3], 1e-4)
+        if i >= warmup:
+            ev[i - warmup][1].record()
+    torch.cuda.synchronize()
+    ms = sorted(a.elapsed_time(b) for a, b in ev)
+    plan.close()
+    med = ms[len(ms) // 2]
+    cells = nx * ny * nz
+    return {"grid": f"{nx}x{ny}x{nz}", "cells": cells, "projection_ms": med, "gcells_per_s": cells / med / 1e6,
+            "note": "paper: 0.1404 s per RK3 step (3 projections + momentum) on 16 V100 (P:L280); context only"}
 
 
 def max_over_ranks(total_ms, world, device):
@@ -344,7 +416,10 @@ def run_ours(args):
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": dom_gbs, "peak": peak_gbs, "unit": "GB/s",
                 "frac": dom_gbs / peak_gbs, "traffic": traffic, "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": kavg[dom]}
+                "algorithmic_bytes_per_launch": dom_bytes, "kernel_ms": kavg[dom],
+                "note": "the kernel with the largest share of the step against ITS OWN algorithmic bytes; the SURVEY 8(d) "
+                        "quantity (112 B/cell over the whole step) is roofline_step.  traffic = dram__bytes_read+write of "
+                        "that kernel from the committed ncu --set full capture (profiles/traffic.json), not measured in this run"}
     step_gbs = STEP_MIN_BYTES_PER_CELL["projection"] * cells / (ms_per_step * 1e-3) / 1e9
     kernels = {k: {"ms": kavg[k], "share": kavg[k] / sum(kavg.values()),
                    "achieved_gbs": KERNEL_BYTES_PER_CELL[k] * cells / (kavg[k] * 1e-3) / 1e9} for k in kavg}
@@ -366,8 +441,25 @@ def run_ours(args):
             t_e2e += time.perf_counter() - t0
         e2e = {"value": cells * n_e2e / t_e2e / 1e9, "unit": UNIT, "h2d_bytes_per_step": 3 * 8 * cells,
                "d2h_bytes_per_step": 4 * 8 * cells, "steps": n_e2e, "ms_per_step": 1e3 * t_e2e / n_e2e,
-               "api": "cans_projection_host (pinned host buffers)"}
+               "api": "cans_projection_host (pinned host buffers)",
+               "note": "PCIe-bound: 22.5 GB cross the host link per step, the kernels are 2-3 % of it"}
         del hu, hv, hw, hp, hu0
+
+    # ---- measured denominators: FP64 FMA rate, HBM rate of the y / z tile access patterns (bare TMA copies) ----
+    probes = None
+    variants = None
+    paper_grid = None
+    if not args.no_extra:
+        fma = binding.probe_fp64_fma()
+        zc = plan.probe_tile_copy(p, 0)
+        yc = plan.probe_tile_copy(p, 1)
+        probes = {"fp64_fma_per_s": fma, "fp64_tflops": 2.0 * fma / 1e12,
+                  "z_tile_copy_gbs": 16.0 * cells / (zc * 1e-3) / 1e9, "z_tile_copy_ms": zc,
+                  "y_tile_copy_gbs": 16.0 * cells / (yc * 1e-3) / 1e9, "y_tile_copy_ms": yc,
+                  "note": "bare TMA in/out copy of the field with the z-solve tiles (16 columns x 512 rows: 128-byte row "
+                          "segments) and the y-transform tiles (16 doubles x 768 rows): the HBM ceiling of those access "
+                          "patterns, to be read next to the z_solve / y_fwd / y_inv achieved_gbs"}
+        variants = time_step_variants(binding, torch, plan, w, (u0, v0, w0, u, v, ww, p))
 
     # ---- Poisson-only timings of the other configs (context; parity-test cases, not bench lines) ----
     poisson = []
@@ -380,6 +472,10 @@ def run_ours(args):
             r["frac_of_peak"] = r["min_bytes"] / (r["ms_median"] * 1e-3) / 1e9 / peak_gbs
             poisson.append(r)
         sweep = bc_sweep(binding, workloads, torch)
+        w.fields.clear()
+        del u0, v0, w0
+        torch.cuda.empty_cache()
+        paper_grid = time_paper_grid(binding, workloads, torch)
 
     # ---- CPU baseline: the oracle on a bounded sample, host cores of this box ----
     cpu_baseline = None
@@ -387,6 +483,7 @@ def run_ours(args):
         nz_sample = 256
         ccells, times = time_oracle_sample(nz_sample, 1)
         cpu_baseline = {"value": ccells / times[0] / 1e9, "unit": UNIT, "cores": cpu_threads(), "kind": "oracle",
+                        "method": "numpy + BLAS matmul, naive O(n^2) transforms (the parity oracle as it stands; cores = BLAS threads)",
                         "sample": f"oracle.projection on a 1024x768x{nz_sample} slab of C5 (same domain, bc, "
                                   f"tanh recipe), {ccells} cells, {times[0]:.1f} s wall"}
 
@@ -405,8 +502,11 @@ def run_ours(args):
         "e2e": e2e,
         "gpu_launches": plan.launches_per_projection * args.steps,
         "clocks": clocks,
+        "probes": probes,
+        "step_variants": variants,
         "poisson_configs": poisson,
         "bc_sweep": sweep,
+        "paper_grid": paper_grid,
         "paper_context": "PAPER.md Table 1 (P:L274-284): 0.1404 s per full RK3 time step (3 projections + momentum), "
                          "1536x768x576, 16x V100 DGX-2 -- whole time step on other hardware, not this metric",
     }

@@ -188,6 +188,18 @@ int cans_plan_set_profiling(cans_poisson_plan* plan, int enable);
 int cans_plan_kernel_times(cans_poisson_plan* plan, float* ms, int capacity);
 const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
 
+/*
+ * Measurement probes for bench.py -- the denominators kernel numbers are read against.  Both synchronise the stream.
+ *   cans_probe_fp64_fma   FP64 FMA instructions per second of the current device (independent chains on every SM): the
+ *                         measured peak of the plain FP64 pipe.
+ *   cans_probe_tile_copy  duration (ms) of a bare in-place TMA copy -- tile in, tile out, no arithmetic, data unchanged --
+ *                         of the field p (DEVICE, nx*ny*nz doubles) with exactly the tiles of the z solve (which = 0:
+ *                         16 / 32 / 8 columns x nz rows) or of the TMA-fed y transforms (which = 1: 16 doubles x ny rows,
+ *                         ny = 512, 768 only): the HBM ceiling of that access pattern.  2*8*N bytes move per call.
+ */
+int cans_probe_fp64_fma(double* fma_per_s, void* stream);
+int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* ms, void* stream);
+
 /* "x.y" version string of the library. */
 const char* cans_version(void);
 

@@ -26,6 +26,7 @@ MAX_KERNEL_RECORDS = 16      # CANS_MAX_KERNEL_RECORDS of the header
 EXPORTED_SYMBOLS = (
     "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
     "cans_projection_step", "cans_chkdt", "cans_helmholtz_plan_create", "cans_helmholtz_solve",
+    "cans_probe_fp64_fma", "cans_probe_tile_copy",
     "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
     "cans_plan_launches_per_projection", "cans_version",
@@ -72,6 +73,10 @@ def _load() -> ctypes.CDLL:
     lib.cans_helmholtz_plan_create.argtypes = lib.cans_poisson_plan_create.argtypes + [i32]
     lib.cans_helmholtz_solve.restype = i32
     lib.cans_helmholtz_solve.argtypes = [vp, vp, ctypes.c_double, vp]
+    lib.cans_probe_fp64_fma.restype = i32
+    lib.cans_probe_fp64_fma.argtypes = [ctypes.POINTER(ctypes.c_double), vp]
+    lib.cans_probe_tile_copy.restype = i32
+    lib.cans_probe_tile_copy.argtypes = [vp, vp, i32, ctypes.POINTER(ctypes.c_float), vp]
     lib.cans_projection_step.restype = i32
     lib.cans_projection_step.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_double, vp, vp]
     lib.cans_chkdt.restype = i32
@@ -124,6 +129,13 @@ def _stream_ptr(stream) -> int:
     if stream is None:
         stream = torch.cuda.current_stream()
     return stream.cuda_stream
+
+
+def probe_fp64_fma(stream=None) -> float:
+    """cans_probe_fp64_fma: measured FP64 FMA instructions per second of the current device."""
+    out = ctypes.c_double(0.0)
+    _check(_lib.cans_probe_fp64_fma(ctypes.byref(out), _stream_ptr(stream)))
+    return float(out.value)
 
 
 class PoissonPlan:
@@ -216,6 +228,12 @@ class PoissonPlan:
         _check(_lib.cans_projection_host(self._h, _host_ptr(u, self.shape), _host_ptr(v, self.shape),
                                          _host_ptr(w, self.shape), _host_ptr(p, self.shape), float(dt),
                                          _stream_ptr(stream)))
+
+    def probe_tile_copy(self, p: torch.Tensor, which: int, stream=None) -> float:
+        """cans_probe_tile_copy: ms of a bare TMA copy of p with the z-solve (0) or y-transform (1) tiles."""
+        ms = ctypes.c_float(0.0)
+        _check(_lib.cans_probe_tile_copy(self._h, _dev_ptr(p, self.shape), int(which), ctypes.byref(ms), _stream_ptr(stream)))
+        return float(ms.value)
 
     def set_profiling(self, enable: bool):
         _check(_lib.cans_plan_set_profiling(self._h, 1 if enable else 0))

@@ -30,6 +30,7 @@
 #include "xw_kernels.cuh"
 #include "yw_kernels.cuh"
 #include "yt_kernels.cuh"
+#include "probes.cuh"
 
 namespace cans {
 
@@ -96,10 +97,11 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
 // chkdt (Listing 1): see chkdt_pass.cuh.  One thread per pair of x-adjacent cells, marching up CHK_KC planes.
 constexpr int CHK_KC = 32;
 
-__global__ void __launch_bounds__(256) chkdt_kernel(const ChkArgs a) {
+__global__ void __launch_bounds__(256, 3) chkdt_kernel(const ChkArgs a) {
     const int hx = a.nx / 2;
-    const size_t cols = (size_t)hx * a.ny;
+    const size_t cols = (size_t)hx * a.ny;                 // a multiple of 32: a warp is valid as a whole
     const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
     double m = 0.0;
     if (c < cols) {
         const int i = 2 * (int)(c % hx);
@@ -108,14 +110,24 @@ __global__ void __launch_bounds__(256) chkdt_kernel(const ChkArgs a) {
         const int k1 = (k0 + CHK_KC < a.nz) ? k0 + CHK_KC : a.nz;
         const double qx = 0.25 * a.rdx, qy = 0.25 * a.rdy;
         // carried rows: u(i-1..i+1, j, k); v(i..i+2, j-1 and j, k); w(i..i+2, j, k-1); w(i, i+1; j+1, k-1)
-        Row3 uj = chk_row_u(a, i, j, k0);
-        Row3 vm = chk_row_v(a, i, j - 1, k0), vj = chk_row_v(a, i, j, k0);
-        Row3 wlj = chk_row_w(a, i, j, k0 - 1), wlp = chk_row_w(a, i, j + 1, k0 - 1);
+        Row3 uj, vm, vj, wlj, wlp;
+        {
+            const RowLoad l0 = chk_load_u(a, i, j, k0, lane), l1 = chk_load_v(a, i, j - 1, k0, lane);
+            const RowLoad l2 = chk_load_v(a, i, j, k0, lane), l3 = chk_load_w(a, i, j, k0 - 1, lane);
+            const RowLoad l4 = chk_load_w(a, i, j + 1, k0 - 1, lane);
+            uj = chk_left(l0, i, lane);
+            vm = chk_right(l1, i, a.nx, lane); vj = chk_right(l2, i, a.nx, lane);
+            wlj = chk_right(l3, i, a.nx, lane); wlp = chk_right(l4, i, a.nx, lane);
+        }
         for (int k = k0; k < k1; ++k) {
-            const Row3 up = chk_row_u(a, i, j + 1, k);            // u(i-1..i+1, j+1, k)
-            const Row3 un = chk_row_u(a, i, j, k + 1);            // u(i-1..i+1, j,   k+1)
-            const Row3 vmn = chk_row_v(a, i, j - 1, k + 1), vjn = chk_row_v(a, i, j, k + 1);
-            const Row3 wj = chk_row_w(a, i, j, k), wp = chk_row_w(a, i, j + 1, k);
+            // all six rows of this step in flight before the first is consumed
+            const RowLoad lup = chk_load_u(a, i, j + 1, k, lane);        // u(i-1..i+1, j+1, k)
+            const RowLoad lun = chk_load_u(a, i, j, k + 1, lane);        // u(i-1..i+1, j,   k+1)
+            const RowLoad lvm = chk_load_v(a, i, j - 1, k + 1, lane), lvj = chk_load_v(a, i, j, k + 1, lane);
+            const RowLoad lwj = chk_load_w(a, i, j, k, lane), lwp = chk_load_w(a, i, j + 1, k, lane);
+            const Row3 up = chk_left(lup, i, lane), un = chk_left(lun, i, lane);
+            const Row3 vmn = chk_right(lvm, i, a.nx, lane), vjn = chk_right(lvj, i, a.nx, lane);
+            const Row3 wj = chk_right(lwj, i, a.nx, lane), wp = chk_right(lwp, i, a.nx, lane);
             const double rzf = a.rdzf[k], rzc = a.rdzc[k], qz = 0.25 * rzf;
             // cell i (values .a / .b of the v, w rows; .b of the u rows) and cell i+1 (.b / .c; .c)
             const double dtix0 = fabs(uj.b) * a.rdx + fabs(vj.a + vm.a + vj.b + vm.b) * qy + fabs(wj.a + wlj.a + wj.b + wlj.b) * qz;
@@ -673,6 +685,45 @@ int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* 
         rc = chkdt_enqueue(plan, u, v, w, dti, (cudaStream_t)stream);
         if (rc) return rc;
     }
+    return CANS_OK;
+}
+
+int cans_probe_fp64_fma(double* fma_per_s, void* stream) {
+    g_status = CANS_OK;
+    if (!fma_per_s) return fail(CANS_ERR_INVALID_ARG, "fma_per_s is NULL");
+    int dev = 0, sms = 148;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaError_t e = probe_fp64_fma(sms, fma_per_s, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(e, "FP64 FMA probe");
+    return CANS_OK;
+}
+
+int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* ms, void* stream) {
+    g_status = CANS_OK;
+    if (!plan || !p || !ms) return fail(CANS_ERR_INVALID_ARG, "NULL argument");
+    if ((reinterpret_cast<size_t>(p) & 15) != 0) return fail(CANS_ERR_INVALID_ARG, "p must be 16-byte aligned");
+    int rc = ensure_tensor_maps(plan, p);
+    if (rc) return rc;
+    TileCopyShape sh;
+    const CUtensorMap* tmap;
+    if (which == 0) {            // z solve: tiles of z_tc_for(nseg) columns x nz rows of the (nz, nx*ny) view
+        const int tc = z_tc_for(plan->nseg);
+        int d = 256 / Z_MROWS;
+        while (plan->nseg % d) --d;
+        sh.ntiles = ((long)plan->nx * plan->ny + tc - 1) / tc; sh.m0 = sh.ntiles; sh.s0 = tc; sh.s1 = 0;
+        sh.box_rows = d * Z_MROWS; sh.nbox = plan->nseg / d; sh.box_cols = tc;
+        tmap = &plan->tmap_z;
+    } else if (which == 1) {     // TMA-fed y transforms: tiles of 16 doubles x ny rows of one k-plane
+        if (!plan->use_yt) return fail(CANS_ERR_UNSUPPORTED_SIZE, "this ny does not run the TMA-fed y transforms");
+        sh.m0 = plan->nx / 2 / YT_COLS; sh.ntiles = sh.m0 * plan->nz; sh.s0 = 2 * YT_COLS; sh.s1 = plan->ny;
+        sh.box_rows = YT_BOX_ROWS; sh.nbox = plan->ny / YT_BOX_ROWS; sh.box_cols = 2 * YT_COLS;
+        tmap = &plan->tmap_y;
+    } else {
+        return fail(CANS_ERR_INVALID_ARG, "which must be 0 (z tiles) or 1 (y tiles)");
+    }
+    cudaError_t e = probe_tile_copy(tmap, sh, plan->num_sms, ms, (cudaStream_t)stream);
+    if (e != cudaSuccess) return fail_cuda(e, "tile copy probe");
     return CANS_OK;
 }
 

@@ -30,48 +30,75 @@ struct ChkArgs {
 struct Row3 { double a, b, c; };
 
 #if defined(__CUDACC__)
-// u(i-1, i, i+1) of row jj, plane kk (i even, i+1 < nx)
-CANS_D Row3 chk_row_u(const ChkArgs& a, int i, int jj, int kk) {
-    Row3 r = {0.0, 0.0, 0.0};
-    if (jj >= a.ny) { if (!a.wrap_y) return r; jj = 0; }
-    if (kk >= a.nz) { if (!a.wrap_z) return r; kk = 0; }
+// A row is fetched in two steps so that a thread has all its loads in flight before it consumes any of them (a warp
+// issues in order: a shuffle right behind its load would serialise the loads).  Step 1 (chk_load_*): the pair (x0, x0+1)
+// as one 16-byte load, plus -- only at a row end or a warp edge -- the outer value, loaded or synthesised by the boundary
+// rule.  Step 2 (chk_left / chk_right): the outer value from the neighbouring lane's pair by shuffle (every lane of the
+// warp takes part: cols is a multiple of 32), replaced by the edge value where step 1 fetched one.
+struct RowLoad { double2 t; double edge; };
+
+// u(i-1 | i, i+1) of row jj, plane kk
+CANS_D RowLoad chk_load_u(const ChkArgs& a, int i, int jj, int kk, int lane) {
+    bool in = true;
+    if (jj >= a.ny) { in = a.wrap_y != 0; jj = 0; }
+    if (kk >= a.nz) { in = in && a.wrap_z != 0; kk = 0; }
     const size_t ro = ((size_t)kk * a.ny + jj) * a.nx;
-    const double2 t = *reinterpret_cast<const double2*>(a.u + ro + i);
-    r.b = t.x; r.c = t.y;
-    if (i > 0) r.a = a.u[ro + i - 1];
-    else if (a.wrap_x) r.a = a.u[ro + a.nx - 1];
-    else if (a.fx) r.a = a.fx[(size_t)kk * a.ny + jj];
+    RowLoad r;
+    r.t = in ? *reinterpret_cast<const double2*>(a.u + ro + i) : make_double2(0.0, 0.0);
+    r.edge = 0.0;
+    if (in && (i == 0 || lane == 0)) {
+        if (i > 0) r.edge = a.u[ro + i - 1];
+        else if (a.wrap_x) r.edge = a.u[ro + a.nx - 1];
+        else if (a.fx) r.edge = a.fx[(size_t)kk * a.ny + jj];
+    }
     return r;
 }
-// v(i, i+1, i+2) of row jj (may be -1), plane kk
-CANS_D Row3 chk_row_v(const ChkArgs& a, int i, int jj, int kk) {
-    Row3 r = {0.0, 0.0, 0.0};
-    if (kk >= a.nz) { if (!a.wrap_z) return r; kk = 0; }
-    const double* row;
-    if (jj >= 0) row = a.v + ((size_t)kk * a.ny + jj) * a.nx;
-    else if (a.wrap_y) row = a.v + ((size_t)kk * a.ny + a.ny - 1) * a.nx;
-    else if (a.fy) row = a.fy + (size_t)kk * a.nx;
-    else return r;
-    const double2 t = *reinterpret_cast<const double2*>(row + i);
-    r.a = t.x; r.b = t.y;
-    if (i + 2 < a.nx) r.c = row[i + 2];
-    else if (a.wrap_x) r.c = row[0];
+CANS_D Row3 chk_left(const RowLoad& l, int i, int lane) {
+    double left = __shfl_up_sync(0xffffffffu, l.t.y, 1);
+    if (i == 0 || lane == 0) left = l.edge;
+    Row3 r = {left, l.t.x, l.t.y};
     return r;
 }
-// w(i, i+1, i+2) of row jj (may be ny), plane kk (may be -1)
-CANS_D Row3 chk_row_w(const ChkArgs& a, int i, int jj, int kk) {
-    Row3 r = {0.0, 0.0, 0.0};
-    if (jj >= a.ny) { if (!a.wrap_y) return r; jj = 0; }
-    const double* row;
-    if (kk >= 0) row = a.w + ((size_t)kk * a.ny + jj) * a.nx;
-    else if (a.wrap_z) row = a.w + ((size_t)(a.nz - 1) * a.ny + jj) * a.nx;
-    else if (a.fz) row = a.fz + (size_t)jj * a.nx;
-    else return r;
-    const double2 t = *reinterpret_cast<const double2*>(row + i);
-    r.a = t.x; r.b = t.y;
-    if (i + 2 < a.nx) r.c = row[i + 2];
-    else if (a.wrap_x) r.c = row[0];
+// v or w (i, i+1 | i+2) of a row given by its base pointer (NULL: the row is outside and reads as 0)
+CANS_D RowLoad chk_load_row(const double* row, int i, int nx, int wrap_x, int lane) {
+    RowLoad r;
+    r.t = row ? *reinterpret_cast<const double2*>(row + i) : make_double2(0.0, 0.0);
+    r.edge = 0.0;
+    if (row && (i + 2 >= nx || lane == 31)) {
+        if (i + 2 < nx) r.edge = row[i + 2];
+        else if (wrap_x) r.edge = row[0];
+    }
     return r;
+}
+CANS_D Row3 chk_right(const RowLoad& l, int i, int nx, int lane) {
+    double right = __shfl_down_sync(0xffffffffu, l.t.x, 1);
+    if (i + 2 >= nx || lane == 31) right = l.edge;
+    Row3 r = {l.t.x, l.t.y, right};
+    return r;
+}
+// v(i, i+1 | i+2) of row jj (may be -1), plane kk
+CANS_D RowLoad chk_load_v(const ChkArgs& a, int i, int jj, int kk, int lane) {
+    const double* row = nullptr;
+    bool in = true;
+    if (kk >= a.nz) { in = a.wrap_z != 0; kk = 0; }
+    if (in) {
+        if (jj >= 0) row = a.v + ((size_t)kk * a.ny + jj) * a.nx;
+        else if (a.wrap_y) row = a.v + ((size_t)kk * a.ny + a.ny - 1) * a.nx;
+        else if (a.fy) row = a.fy + (size_t)kk * a.nx;
+    }
+    return chk_load_row(row, i, a.nx, a.wrap_x, lane);
+}
+// w(i, i+1 | i+2) of row jj (may be ny), plane kk (may be -1)
+CANS_D RowLoad chk_load_w(const ChkArgs& a, int i, int jj, int kk, int lane) {
+    const double* row = nullptr;
+    bool in = true;
+    if (jj >= a.ny) { in = a.wrap_y != 0; jj = 0; }
+    if (in) {
+        if (kk >= 0) row = a.w + ((size_t)kk * a.ny + jj) * a.nx;
+        else if (a.wrap_z) row = a.w + ((size_t)(a.nz - 1) * a.ny + jj) * a.nx;
+        else if (a.fz) row = a.fz + (size_t)jj * a.nx;
+    }
+    return chk_load_row(row, i, a.nx, a.wrap_x, lane);
 }
 #endif
 
