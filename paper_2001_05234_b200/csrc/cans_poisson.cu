@@ -207,6 +207,7 @@ struct cans_poisson_plan {
     // device tables
     double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc, *rstart, *r00;
     cplx *tw_x, *tw_y, *wpost_x, *wpost_y, *wpre_x, *wpre_y;
+    cplx wstep_x[32], wstep_y[32];   // mixed pairs, warp-level kernels: wpre[32 m] (XYArgs::wstep)
     cplx* tw2_x;              // W_nx^(p k1), [nx/32][32]: warp-per-line x kernels (xw_pass.cuh), or NULL
     int use_xw;               // 1: x transforms run the warp-per-line kernels
     cplx* tw2_y;              // the same for ny (yw_pass.cuh), or NULL
@@ -296,6 +297,7 @@ static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
     a.tw = xdir ? pl->tw_x : pl->tw_y;
     a.wpost = xdir ? pl->wpost_x : pl->wpost_y;
     a.wpre = xdir ? pl->wpre_x : pl->wpre_y;
+    std::memcpy(a.wstep, xdir ? pl->wstep_x : pl->wstep_y, sizeof(a.wstep));
     a.p = p;
     return a;
 }
@@ -440,8 +442,13 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     up(kind_mixed(kx) ? make_post_twiddles_mixed(nx) : make_post_twiddles(nx), &pl->wpost_x);
     up(kind_mixed(ky) ? make_post_twiddles_mixed(ny) : make_post_twiddles(ny), &pl->wpost_y);
     pl->wpre_x = pl->wpre_y = nullptr;
-    if (kind_mixed(kx)) up(make_pre_twiddles_mixed(nx), &pl->wpre_x);
-    if (kind_mixed(ky)) up(make_pre_twiddles_mixed(ny), &pl->wpre_y);
+    std::memset(pl->wstep_x, 0, sizeof(pl->wstep_x));
+    std::memset(pl->wstep_y, 0, sizeof(pl->wstep_y));
+    auto steps = [](const std::vector<double>& wpre, int n, cplx* out) {
+        for (int m = 0; m < 32 && 32 * m < n; ++m) out[m] = make_double2(wpre[2 * (32 * m)], wpre[2 * (32 * m) + 1]);
+    };
+    if (kind_mixed(kx)) { const std::vector<double> h = make_pre_twiddles_mixed(nx); steps(h, nx, pl->wstep_x); up(h, &pl->wpre_x); }
+    if (kind_mixed(ky)) { const std::vector<double> h = make_pre_twiddles_mixed(ny); steps(h, ny, pl->wstep_y); up(h, &pl->wpre_y); }
     pl->tw2_x = nullptr;
     pl->use_xw = 0;
     if (xw_supported(nx)) {

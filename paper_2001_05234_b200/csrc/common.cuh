@@ -49,6 +49,16 @@ CANS_HD double2 ld_p2(const double* p) {
 #endif
 }
 
+// 16-byte load of data that is streamed once (u, v, w of the fused divergence): L2 only, so that the small twiddle
+// tables keep their place in L1
+CANS_HD double2 ldg_stream2(const double* p) {
+#if defined(__CUDA_ARCH__)
+    return *reinterpret_cast<const double2*>(p);   // TEST: plain
+#else
+    return *reinterpret_cast<const double2*>(p);
+#endif
+}
+
 // Transform kind of one direction (pressure boundary pair), see DESIGN.md "Transforms".
 // KIND_ND / KIND_DN: the mixed pairs (lower Neumann, upper Dirichlet and the reverse), DCT-IV / DST-IV.
 enum Kind : int { KIND_PP = 0, KIND_NN = 1, KIND_DD = 2, KIND_ND = 3, KIND_DN = 4 };

@@ -74,6 +74,10 @@ struct XWPass {
         if (kind == KIND_PP) return e;
         return (e < H) ? 2 * e : 2 * (N - 1 - e) + 1;
     }
+    // Staging position of natural sample i of a periodic line: lane L stores the pair (2e, 2e+1), a stride of two 16-byte
+    // units that would fold the eight lanes of a quarter warp onto four bank groups; flipping the low bit in every
+    // second group of eight makes the pair stores and the unit-stride reads both conflict free.
+    static CANS_HD int stage_pos(int i) { return i ^ ((i >> 3) & 1); }
 
 #if defined(__CUDACC__)
     // W_N^(lane k1), k1 = 1..R1-1, applied to v (conjugated for the inverse): every 8th root is read from the
@@ -95,41 +99,54 @@ struct XWPass {
     }
 
     // ---- forward: rows (ro, ro + nx) of the field (or the divergence at those rows) -> slots ----
-    template <bool DIV>
+    // KC: class of the boundary pair (0 = PP, 1 = NN / DD, 2 = ND / DN), a compile-time switch so that the periodic kernels
+    // carry none of the permutation / twiddle code; the pair inside a class is the run-time a.kind
+    template <bool DIV, int KC>
     static CANS_D void forward(const XYArgs& a, const cplx* __restrict__ tw, cplx* buf, size_t ro, int j, int k, int lane) {
-        // phase 0: the two rows (or the divergence at them) in natural order -> buf[i] = (a_i, b_i), read from
-        // global memory as coalesced 16-byte loads, UB column pairs per lane in flight at a time
+        constexpr bool pp = KC == 0, mixed = KC == 2;
+        const int kind = pp ? (int)KIND_PP : a.kind;
+        // phase 0: the FFT input elements lane + 32 m of the packed line (row a) + i (row b) in registers.
+        //   * stored periodic rows: 8-byte loads straight from global memory (every load instruction of the warp reads
+        //     256 contiguous bytes), no staging;
+        //   * stored non-periodic rows: 16-byte loads of the sample pairs (2e, 2e+1), e = lane + 32 m; Makhoul's
+        //     permutation sends sample 2e to element e (this lane) and sample 2e+1 to element N-1-e = (31 - lane) +
+        //     32 (R1-1-m), i.e. to the mirrored lane: one shuffle, no staging;
+        //   * fused divergence: computed pair by pair in batches and staged once in the warp's buffer at the
+        //     element's position (periodic: an XOR swizzle makes the pair stores conflict free).
         const size_t plane = (size_t)a.nx * a.ny;
         constexpr int NQ = H / 32;                       // column pairs per lane
-        constexpr int UB = DIV ? 4 : (NQ < 16 ? NQ : 16);
+        constexpr int UB = 4;
         cplx v[R1];
-        const bool direct = !DIV && a.kind == KIND_PP;   // periodic rows of a stored field: no staging needed
-        if (direct) {
-            // lane p takes x[p + 32 m] of both rows straight into registers: 2*R1 independent 8-byte loads,
-            // every load instruction of the warp reads 256 contiguous bytes
+        if (!DIV && pp) {
 #pragma unroll
             for (int m = 0; m < R1; ++m)
                 v[m] = make_double2(__ldcg(a.p + ro + lane + 32 * m), __ldcg(a.p + ro + a.nx + lane + 32 * m));
-        }
-#pragma unroll 1
-        for (int m0 = 0; m0 < (direct ? 0 : NQ); m0 += UB) {
-            double2 fa[UB], fb[UB];
-            if (!DIV) {
+        } else if (!DIV) {
+            double2 fa[NQ], fb[NQ];
 #pragma unroll
-                for (int u = 0; u < UB; ++u) {
-                    const int i0 = 2 * (lane + 32 * (m0 + u));
-                    fa[u] = ld_p2(a.p + ro + i0);
-                    fb[u] = ld_p2(a.p + ro + a.nx + i0);
-                }
-            } else {
+            for (int m = 0; m < NQ; ++m) {
+                fa[m] = ld_p2(a.p + ro + 2 * (lane + 32 * m));
+                fb[m] = ld_p2(a.p + ro + a.nx + 2 * (lane + 32 * m));
+            }
+            const double sgn = kind_neg_odd(kind) ? -1.0 : 1.0;
+#pragma unroll
+            for (int m = 0; m < NQ; ++m) {
+                v[m] = make_double2(fa[m].x, fb[m].x);
+                v[R1 - 1 - m] = make_double2(__shfl_xor_sync(0xffffffffu, sgn * fa[m].y, 31),
+                                             __shfl_xor_sync(0xffffffffu, sgn * fb[m].y, 31));
+            }
+        } else {
+#pragma unroll 1
+            for (int m0 = 0; m0 < NQ; m0 += UB) {
+                double2 fa[UB], fb[UB];
                 double2 ua[UB], ub[UB], v0[UB], v1[UB], v2[UB], wa[UB], wb[UB], wla[UB], wlb[UB];
                 double ula0[UB], ulb0[UB];
                 const double2 zero2 = make_double2(0.0, 0.0);
 #pragma unroll
                 for (int u = 0; u < UB; ++u) {
                     const int i0 = 2 * (lane + 32 * (m0 + u));
-                    ua[u] = *reinterpret_cast<const double2*>(a.u + ro + i0);
-                    ub[u] = *reinterpret_cast<const double2*>(a.u + ro + a.nx + i0);
+                    ua[u] = ldg_stream2(a.u + ro + i0);
+                    ub[u] = ldg_stream2(a.u + ro + a.nx + i0);
                     // left neighbour of the pair: lane - 1 holds it, except for lane 0
                     ula0[u] = 0.0; ulb0[u] = 0.0;
                     if (lane == 0) {
@@ -137,23 +154,23 @@ struct XWPass {
                         else if (a.wrap_x) { ula0[u] = a.u[ro + a.nx - 1]; ulb0[u] = a.u[ro + 2 * (size_t)a.nx - 1]; }
                         else if (a.fx) { ula0[u] = a.fx[(size_t)k * a.ny + j]; ulb0[u] = a.fx[(size_t)k * a.ny + j + 1]; }
                     }
-                    v1[u] = *reinterpret_cast<const double2*>(a.v + ro + i0);
-                    v2[u] = *reinterpret_cast<const double2*>(a.v + ro + a.nx + i0);
-                    if (j > 0) v0[u] = *reinterpret_cast<const double2*>(a.v + ro - a.nx + i0);
-                    else if (a.wrap_y) v0[u] = *reinterpret_cast<const double2*>(a.v + ro + (size_t)(a.ny - 1) * a.nx + i0);
-                    else if (a.fy) v0[u] = *reinterpret_cast<const double2*>(a.fy + (size_t)k * a.nx + i0);
+                    v1[u] = ldg_stream2(a.v + ro + i0);
+                    v2[u] = ldg_stream2(a.v + ro + a.nx + i0);
+                    if (j > 0) v0[u] = ldg_stream2(a.v + ro - a.nx + i0);
+                    else if (a.wrap_y) v0[u] = ldg_stream2(a.v + ro + (size_t)(a.ny - 1) * a.nx + i0);
+                    else if (a.fy) v0[u] = ldg_stream2(a.fy + (size_t)k * a.nx + i0);
                     else v0[u] = zero2;
-                    wa[u] = *reinterpret_cast<const double2*>(a.w + ro + i0);
-                    wb[u] = *reinterpret_cast<const double2*>(a.w + ro + a.nx + i0);
+                    wa[u] = ldg_stream2(a.w + ro + i0);
+                    wb[u] = ldg_stream2(a.w + ro + a.nx + i0);
                     if (k > 0) {
-                        wla[u] = *reinterpret_cast<const double2*>(a.w + ro - plane + i0);
-                        wlb[u] = *reinterpret_cast<const double2*>(a.w + ro - plane + a.nx + i0);
+                        wla[u] = ldg_stream2(a.w + ro - plane + i0);
+                        wlb[u] = ldg_stream2(a.w + ro - plane + a.nx + i0);
                     } else if (a.wrap_z) {
-                        wla[u] = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + i0);
-                        wlb[u] = *reinterpret_cast<const double2*>(a.w + ro + (size_t)(a.nz - 1) * plane + a.nx + i0);
+                        wla[u] = ldg_stream2(a.w + ro + (size_t)(a.nz - 1) * plane + i0);
+                        wlb[u] = ldg_stream2(a.w + ro + (size_t)(a.nz - 1) * plane + a.nx + i0);
                     } else if (a.fz) {
-                        wla[u] = *reinterpret_cast<const double2*>(a.fz + (size_t)j * a.nx + i0);
-                        wlb[u] = *reinterpret_cast<const double2*>(a.fz + (size_t)(j + 1) * a.nx + i0);
+                        wla[u] = ldg_stream2(a.fz + (size_t)j * a.nx + i0);
+                        wlb[u] = ldg_stream2(a.fz + (size_t)(j + 1) * a.nx + i0);
                     } else { wla[u] = zero2; wlb[u] = zero2; }
                 }
                 const double rz = a.rdzf[k];
@@ -168,28 +185,31 @@ struct XWPass {
                     fb[u].x = div_value(ub[u].x - ulb, v2[u].x - v1[u].x, wb[u].x - wlb[u].x, a.rdx, a.rdy, rz, a.rdt);
                     fb[u].y = div_value(ub[u].y - ub[u].x, v2[u].y - v1[u].y, wb[u].y - wlb[u].y, a.rdx, a.rdy, rz, a.rdt);
                 }
-            }
 #pragma unroll
-            for (int u = 0; u < UB; ++u) {
-                const int i0 = 2 * (lane + 32 * (m0 + u));
-                buf[i0] = make_double2(fa[u].x, fb[u].x);
-                buf[i0 + 1] = make_double2(fa[u].y, fb[u].y);
+                for (int u = 0; u < UB; ++u) {
+                    const int e = lane + 32 * (m0 + u);          // samples 2e, 2e+1
+                    const cplx z0 = make_double2(fa[u].x, fb[u].x);
+                    cplx z1 = make_double2(fa[u].y, fb[u].y);
+                    if (pp) {
+                        buf[stage_pos(2 * e)] = z0;
+                        buf[stage_pos(2 * e + 1)] = z1;
+                    } else {
+                        if (kind_neg_odd(kind)) z1 = cneg(z1);
+                        buf[e] = z0;
+                        buf[N - 1 - e] = z1;
+                    }
+                }
             }
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < R1; ++m) v[m] = buf[pp ? stage_pos(lane + 32 * m) : lane + 32 * m];
+            __syncwarp();                               // staged elements fully read: reuse the buffer for the exchange
         }
-        __syncwarp();
-        if (!direct) {
+        if (mixed) {
+            const cplx wl = __ldg(a.wpre + lane);
 #pragma unroll
-            for (int m = 0; m < R1; ++m) {
-                const int i = index_of_elem(lane + 32 * m, a.kind);
-                v[m] = buf[i];
-                if (kind_neg_odd(a.kind) && (i & 1)) v[m] = cneg(v[m]);
-            }
-            if (kind_mixed(a.kind)) {
-#pragma unroll
-                for (int m = 0; m < R1; ++m) v[m] = cmul(v[m], __ldg(a.wpre + lane + 32 * m));
-            }
+            for (int m = 0; m < R1; ++m) v[m] = cmul(v[m], cmul(wl, a.wstep[m]));
         }
-        __syncwarp();                                   // natural-order rows fully read: reuse the buffer for the exchange
         Dft<R1, false>::run(v);
         apply_twiddles<false>(v, tw, lane);
 #pragma unroll
@@ -201,26 +221,31 @@ struct XWPass {
             for (int p = 0; p < 32; ++p) w[p] = buf[lane * XSTRIDE + p];
             Dft<32, false>::run(w);
         }
+        // quarter-wave post-twiddles of this lane's slots: all loads issued here, behind the exchange below
+        cplx wq[NQ];
+        if (!pp) {
+#pragma unroll
+            for (int m = 0; m < NQ; ++m) wq[m] = __ldg(a.wpost + lane + 32 * m);
+        }
         __syncwarp();                                   // exchange buffer fully read: reuse it in natural order
         if (lane < R1) {
 #pragma unroll
             for (int k2 = 0; k2 < 32; ++k2) buf[lane + R1 * k2] = w[k2];
         }
         __syncwarp();
-#pragma unroll 4
-        for (int s = lane; s < H; s += 32) {
+#pragma unroll
+        for (int m = 0; m < NQ; ++m) {
+            const int s = lane + 32 * m;
             double2 oa, ob;
-            if (kind_mixed(a.kind)) {
-                post_forward(buf[s], buf[N - 1 - s], __ldg(a.wpost + s), a.kind, oa.x, oa.y, ob.x, ob.y);
+            if (mixed) {
+                post_forward(buf[s], buf[N - 1 - s], wq[m], kind, oa.x, oa.y, ob.x, ob.y);
             } else if (s == 0) {
                 const cplx Z0 = buf[0], Zh = buf[H];
-                const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
+                const double c = pp ? 1.0 : CANS_SQRT_HALF;
                 oa = make_double2(Z0.x, c * Zh.x);
                 ob = make_double2(Z0.y, c * Zh.y);
             } else {
-                cplx wq = make_double2(1.0, 0.0);
-                if (a.kind != KIND_PP) wq = __ldg(a.wpost + s);
-                post_forward(buf[s], buf[N - s], wq, a.kind, oa.x, oa.y, ob.x, ob.y);
+                post_forward(buf[s], buf[N - s], pp ? make_double2(1.0, 0.0) : wq[m], kind, oa.x, oa.y, ob.x, ob.y);
             }
             *reinterpret_cast<double2*>(a.p + ro + 2 * s) = oa;
             *reinterpret_cast<double2*>(a.p + ro + a.nx + 2 * s) = ob;
@@ -229,32 +254,38 @@ struct XWPass {
     }
 
     // ---- inverse: slots of rows (ro, ro + nx) -> the two real rows ----
+    template <int KC>
     static CANS_D void inverse(const XYArgs& a, const cplx* __restrict__ tw, cplx* buf, size_t ro, int lane) {
+        constexpr bool pp = KC == 0, mixed = KC == 2;
+        const int kind = pp ? (int)KIND_PP : a.kind;
         constexpr int NQ = H / 32;                       // slots per lane, all loaded before the first use
         {
             double2 ia[NQ], ib[NQ];
+            cplx wq[NQ];
 #pragma unroll
             for (int m = 0; m < NQ; ++m) {
                 ia[m] = ld_p2(a.p + ro + 2 * (lane + 32 * m));
                 ib[m] = ld_p2(a.p + ro + a.nx + 2 * (lane + 32 * m));
             }
+            if (!pp) {
+#pragma unroll
+                for (int m = 0; m < NQ; ++m) wq[m] = __ldg(a.wpost + lane + 32 * m);
+            }
 #pragma unroll
             for (int m = 0; m < NQ; ++m) {
                 const int s = lane + 32 * m;
-                if (kind_mixed(a.kind)) {
+                if (mixed) {
                     cplx Zq, Zm;
-                    pre_inverse(ia[m].x, ia[m].y, ib[m].x, ib[m].y, __ldg(a.wpost + s), a.kind, Zq, Zm);
+                    pre_inverse(ia[m].x, ia[m].y, ib[m].x, ib[m].y, wq[m], kind, Zq, Zm);
                     buf[s] = Zq;
                     buf[N - 1 - s] = Zm;
                 } else if (s == 0) {
-                    const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
+                    const double c = pp ? 1.0 : (1.0 / CANS_SQRT_HALF);
                     buf[0] = make_double2(ia[m].x, ib[m].x);
                     buf[H] = make_double2(c * ia[m].y, c * ib[m].y);
                 } else {
-                    cplx wq = make_double2(1.0, 0.0);
-                    if (a.kind != KIND_PP) wq = __ldg(a.wpost + s);
                     cplx Zq, Zm;
-                    pre_inverse(ia[m].x, ia[m].y, ib[m].x, ib[m].y, wq, a.kind, Zq, Zm);
+                    pre_inverse(ia[m].x, ia[m].y, ib[m].x, ib[m].y, pp ? make_double2(1.0, 0.0) : wq[m], kind, Zq, Zm);
                     buf[s] = Zq;
                     buf[N - s] = Zm;
                 }
@@ -278,7 +309,7 @@ struct XWPass {
         for (int k1 = 0; k1 < R1; ++k1) v[k1] = buf[k1 * XSTRIDE + lane];
         apply_twiddles<true>(v, tw, lane);
         Dft<R1, true>::run(v);
-        if (a.kind == KIND_PP) {
+        if (pp) {
             // periodic lines need no permutation: lane p holds x[p + 32 m], so every store instruction of the
             // warp writes 256 contiguous bytes of a row straight from registers
 #pragma unroll
@@ -289,23 +320,21 @@ struct XWPass {
             __syncwarp();
             return;
         }
-        __syncwarp();                                   // exchange buffer fully read: reuse it in natural order
-        if (kind_mixed(a.kind)) {
+        // Non-periodic lines: element e = lane + 32 m is sample 2e (m < R1/2); sample 2e+1 is element N-1-e, held by
+        // the mirrored lane as its v[R1-1-m]: one shuffle, then the pair goes out as a coalesced 16-byte store.
+        if (mixed) {
+            const cplx wl = __ldg(a.wpre + lane);
 #pragma unroll
-            for (int m = 0; m < R1; ++m) v[m] = cmulc(v[m], __ldg(a.wpre + lane + 32 * m));
+            for (int m = 0; m < R1; ++m) v[m] = cmulc(v[m], cmul(wl, a.wstep[m]));
         }
-#pragma unroll
-        for (int m = 0; m < R1; ++m) {
-            const int i = index_of_elem(lane + 32 * m, a.kind);
-            buf[i] = (kind_neg_odd(a.kind) && (i & 1)) ? cneg(v[m]) : v[m];
-        }
-        __syncwarp();
+        const double sgn = kind_neg_odd(kind) ? -1.0 : 1.0;
 #pragma unroll
         for (int m = 0; m < NQ; ++m) {
+            const double z1x = sgn * __shfl_xor_sync(0xffffffffu, v[R1 - 1 - m].x, 31);
+            const double z1y = sgn * __shfl_xor_sync(0xffffffffu, v[R1 - 1 - m].y, 31);
             const int i0 = 2 * (lane + 32 * m);
-            const cplx z0 = buf[i0], z1 = buf[i0 + 1];
-            *reinterpret_cast<double2*>(a.p + ro + i0) = make_double2(z0.x, z1.x);
-            *reinterpret_cast<double2*>(a.p + ro + a.nx + i0) = make_double2(z0.y, z1.y);
+            *reinterpret_cast<double2*>(a.p + ro + i0) = make_double2(v[m].x, z1x);
+            *reinterpret_cast<double2*>(a.p + ro + a.nx + i0) = make_double2(v[m].y, z1y);
         }
         __syncwarp();
     }

@@ -34,6 +34,9 @@ struct XYArgs {
     const cplx* tw;         // pass twiddles, FftPlan::TW_TOTAL entries
     const cplx* wpost;      // NN / DD: exp(-i pi q / (2n)); ND / DN: exp(-i pi (2q+1) / (4n)); q = 0..n/2-1
     const cplx* wpre;       // ND / DN only: exp(-i pi m / n), m = 0..n-1
+    cplx wstep[32];         // ND / DN, warp-level kernels (n = 32 R1): wstep[m] = wpre[32 m] -- the pre-twiddle of element
+                            // lane + 32 m is wpre[lane] * wstep[m]: one table load per lane, the steps come from the
+                            // kernel's parameter bank (uniform reads, no memory latency at the end of the transform)
     double* p;              // field transformed in place
     // fused divergence (x forward only): f = (du*rdx + dv*rdy + dw*rdzf[k]) * rdt
     const double* u;

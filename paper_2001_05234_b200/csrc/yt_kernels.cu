@@ -5,10 +5,10 @@ namespace cans {
 
 extern __shared__ __align__(1024) unsigned char cans_dyn_smem_1k[];
 
-template <int N, int R1, bool INV>
+template <int N, int R1, bool INV, int KC>
 __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx* __restrict__ tw,
                                                       const __grid_constant__ CUtensorMap tmap, int ntx, long ntiles) {
-    typedef YTPass<N, R1> W;
+    typedef YTPass<N, R1, KC> W;
     cplx* bufs = reinterpret_cast<cplx*>(cans_dyn_smem_1k);
     __shared__ __align__(8) unsigned long long s_bar[2];
     const int tid = threadIdx.x;
@@ -53,11 +53,9 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
         cplx* T = bufs + (size_t)b * W::TILE;
         if (INV) {
             W::slots_in(a, T, warp, lane);
-            W::column_inverse(T, warp, tw, lane);
-            W::permute_out(T, warp, a.kind, a.wpre, lane);
+            W::column_inverse(a, T, warp, tw, lane);
         } else {
-            W::permute_in(T, warp, a.kind, a.wpre, lane);
-            W::column_forward(T, warp, tw, lane);
+            W::column_forward(a, T, warp, tw, lane);
             W::slots_out(a, T, warp, lane);
         }
         fence_proxy_async_smem();               // this thread's shared-memory writes -> visible to the TMA unit
@@ -77,20 +75,36 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     if (tid == 0) tma_store_wait_all();
 }
 
-template <int N, int R1>
-static cudaError_t yt_launch_n(int op, const XYArgs& a, const cplx* tw, const CUtensorMap* tmap, int max_ctas, cudaStream_t st) {
-    const size_t smem = 2 * sizeof(cplx) * (size_t)YTPass<N, R1>::TILE;
+template <int N, int R1, int KC>
+static cudaError_t yt_launch_k(int op, const XYArgs& a, const cplx* tw, const CUtensorMap* tmap, int max_ctas, cudaStream_t st) {
+    const size_t smem = 2 * sizeof(cplx) * (size_t)YTPass<N, R1, KC>::TILE;
     if (op == OP_CONFIGURE) {
-        cudaError_t e = cudaFuncSetAttribute(yt_kernel<N, R1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(yt_kernel<N, R1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(yt_kernel<N, R1, false, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(yt_kernel<N, R1, true, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         return e;
     }
     const int ntx = a.nx / 2 / YT_COLS;
     const long ntiles = (long)ntx * a.nk;
     const unsigned grid = (unsigned)(ntiles < max_ctas ? ntiles : max_ctas);
-    if (op == OP_Y_FWD) yt_kernel<N, R1, false><<<grid, YT_NT, smem, st>>>(a, tw, *tmap, ntx, ntiles);
-    else yt_kernel<N, R1, true><<<grid, YT_NT, smem, st>>>(a, tw, *tmap, ntx, ntiles);
+    if (op == OP_Y_FWD) yt_kernel<N, R1, false, KC><<<grid, YT_NT, smem, st>>>(a, tw, *tmap, ntx, ntiles);
+    else yt_kernel<N, R1, true, KC><<<grid, YT_NT, smem, st>>>(a, tw, *tmap, ntx, ntiles);
     return cudaGetLastError();
+}
+
+// one kernel per class of boundary pair (yt_kind_class): the periodic kernels carry no permutation / twiddle code
+template <int N, int R1>
+static cudaError_t yt_launch_n(int op, const XYArgs& a, const cplx* tw, const CUtensorMap* tmap, int max_ctas, cudaStream_t st) {
+    if (op == OP_CONFIGURE) {                            // plan time: every class (the opt-in is per kernel)
+        cudaError_t e = yt_launch_k<N, R1, 0>(op, a, tw, tmap, max_ctas, st);
+        if (e == cudaSuccess) e = yt_launch_k<N, R1, 1>(op, a, tw, tmap, max_ctas, st);
+        if (e == cudaSuccess) e = yt_launch_k<N, R1, 2>(op, a, tw, tmap, max_ctas, st);
+        return e;
+    }
+    switch (yt_kind_class(a.kind)) {
+        case 0: return yt_launch_k<N, R1, 0>(op, a, tw, tmap, max_ctas, st);
+        case 1: return yt_launch_k<N, R1, 1>(op, a, tw, tmap, max_ctas, st);
+        default: return yt_launch_k<N, R1, 2>(op, a, tw, tmap, max_ctas, st);
+    }
 }
 
 // the field as a 2-D tensor: nx doubles per row, ny*nz rows; boxes of 16 doubles x 256 rows, 128-byte swizzle

@@ -23,9 +23,14 @@ constexpr int YT_NT = YT_COLS * 32;
 constexpr int YT_BOX_ROWS = 256;
 inline bool yt_supported(int n) { return n == 512 || n == 768; }
 
-template <int N_, int R1_>
+// KC: class of the boundary pair, a compile-time switch so that the periodic kernels carry none of the registers of the
+// permutation / twiddle paths: 0 = PP, 1 = NN / DD, 2 = ND / DN (the pair inside a class is the run-time `kind`)
+constexpr int yt_kind_class(int kind) { return kind == KIND_PP ? 0 : (kind >= KIND_ND ? 2 : 1); }
+
+template <int N_, int R1_, int KC>
 struct YTPass {
     static constexpr int N = N_, R1 = R1_, H = N_ / 2;
+    static constexpr bool IS_PP = KC == 0, IS_MIXED = KC == 2;
     static_assert(R1_ * 32 == N_ && N_ % YT_BOX_ROWS == 0, "N = R1 * 32, whole TMA boxes");
     static constexpr int TILE = N * YT_COLS;                         // cplx per buffer
     static constexpr int NBOX = N / YT_BOX_ROWS;
@@ -49,11 +54,67 @@ struct YTPass {
         }
     }
 
-    // natural-order input -> natural-order spectrum, in place in column f (unnormalised)
-    static CANS_D void column_forward(cplx* t, int f, const cplx* __restrict__ tw, int lane) {
-        cplx v[R1];
+    // Row of the tile holding FFT input element e (Makhoul's even/odd permutation for every non-periodic pair; the
+    // identity for PP): e < H -> row 2e, e >= H -> row 2(N-1-e)+1.
+    static CANS_D int row_of_elem(int e, int kind) {
+        if (IS_PP) return e;
+        return (e < H) ? 2 * e : 2 * (N - 1 - e) + 1;
+    }
+    // Lane p owns the FFT input elements p + 32 m.  For the non-periodic pairs elements m and m + R1/2 sit in an even and an
+    // odd row; lanes with bit 2 set touch the odd row first, so that the eight rows of one shared-memory access differ
+    // modulo 8 (conflict free under the swizzle) -- the permutation costs no pass of its own.
+    static CANS_D void load_elems(const XYArgs& a, const cplx* t, int f, int lane, cplx (&v)[R1]) {
+        const int kind = a.kind;
+        if (IS_PP) {
 #pragma unroll
-        for (int m = 0; m < R1; ++m) v[m] = t[at(lane + 32 * m, f)];
+            for (int m = 0; m < R1; ++m) v[m] = t[at(lane + 32 * m, f)];
+            return;
+        }
+        const bool odd_first = (lane & 4) != 0;
+#pragma unroll
+        for (int m = 0; m < R1 / 2; ++m) {
+            const int je = 2 * (lane + 32 * m);                           // element m
+            const int jo = 2 * (N - 1 - (lane + 32 * (m + R1 / 2))) + 1;   // element m + R1/2
+            const cplx x0 = t[at(odd_first ? jo : je, f)];
+            const cplx x1 = t[at(odd_first ? je : jo, f)];
+            v[m] = odd_first ? x1 : x0;
+            const cplx zo = odd_first ? x0 : x1;
+            v[m + R1 / 2] = kind_neg_odd(kind) ? cneg(zo) : zo;
+        }
+        if (IS_MIXED) {
+            const cplx wl = __ldg(a.wpre + lane);
+#pragma unroll
+            for (int m = 0; m < R1; ++m) v[m] = cmul(v[m], cmul(wl, a.wstep[m]));
+        }
+    }
+    static CANS_D void store_elems(const XYArgs& a, cplx* t, int f, int lane, cplx (&v)[R1]) {
+        const int kind = a.kind;
+        if (IS_PP) {
+#pragma unroll
+            for (int m = 0; m < R1; ++m) t[at(lane + 32 * m, f)] = v[m];
+            return;
+        }
+        if (IS_MIXED) {
+            const cplx wl = __ldg(a.wpre + lane);
+#pragma unroll
+            for (int m = 0; m < R1; ++m) v[m] = cmulc(v[m], cmul(wl, a.wstep[m]));
+        }
+        const bool odd_first = (lane & 4) != 0;
+#pragma unroll
+        for (int m = 0; m < R1 / 2; ++m) {
+            const int je = 2 * (lane + 32 * m);
+            const int jo = 2 * (N - 1 - (lane + 32 * (m + R1 / 2))) + 1;
+            const cplx ze = v[m];
+            const cplx zo = kind_neg_odd(kind) ? cneg(v[m + R1 / 2]) : v[m + R1 / 2];
+            t[at(odd_first ? jo : je, f)] = odd_first ? zo : ze;
+            t[at(odd_first ? je : jo, f)] = odd_first ? ze : zo;
+        }
+    }
+
+    // rows as loaded (natural order) -> natural-order spectrum, in place in column f (unnormalised)
+    static CANS_D void column_forward(const XYArgs& a, cplx* t, int f, const cplx* __restrict__ tw, int lane) {
+        cplx v[R1];
+        load_elems(a, t, f, lane, v);
         Dft<R1, false>::run(v);
         apply_twiddles<false>(v, tw, lane);
         __syncwarp();
@@ -73,7 +134,7 @@ struct YTPass {
         }
         __syncwarp();
     }
-    static CANS_D void column_inverse(cplx* t, int f, const cplx* __restrict__ tw, int lane) {
+    static CANS_D void column_inverse(const XYArgs& a, cplx* t, int f, const cplx* __restrict__ tw, int lane) {
         cplx w[32];
         if (lane < R1) {
 #pragma unroll
@@ -92,69 +153,36 @@ struct YTPass {
         apply_twiddles<true>(v, tw, lane);
         Dft<R1, true>::run(v);
         __syncwarp();
-#pragma unroll
-        for (int m = 0; m < R1; ++m) t[at(lane + 32 * m, f)] = v[m];
+        store_elems(a, t, f, lane, v);       // FFT output elements -> rows (the inverse of load_elems)
         __syncwarp();
     }
 
-    // rows j (as loaded) -> FFT input elements e, in place through registers (NN / DD only; PP is the identity)
-    static CANS_D void permute_in(cplx* t, int f, int kind, const cplx* __restrict__ wpre, int lane) {
-        if (kind == KIND_PP) return;
-        cplx v[R1];
-#pragma unroll
-        for (int m = 0; m < R1; ++m) v[m] = t[at(lane + 32 * m, f)];
-        __syncwarp();
-#pragma unroll
-        for (int m = 0; m < R1; ++m) {
-            const int j = lane + 32 * m;
-            const int e = elem_of_index<N>(j, kind);
-            cplx z = (kind_neg_odd(kind) && (j & 1)) ? cneg(v[m]) : v[m];
-            if (kind_mixed(kind)) z = cmul(z, __ldg(wpre + e));
-            t[at(e, f)] = z;
-        }
-        __syncwarp();
-    }
-    // FFT output elements e -> rows j (inverse of permute_in)
-    static CANS_D void permute_out(cplx* t, int f, int kind, const cplx* __restrict__ wpre, int lane) {
-        if (kind == KIND_PP) return;
-        cplx v[R1];
-#pragma unroll
-        for (int m = 0; m < R1; ++m) {
-            const int j = lane + 32 * m;
-            const int e = elem_of_index<N>(j, kind);
-            cplx z = t[at(e, f)];
-            if (kind_mixed(kind)) z = cmulc(z, __ldg(wpre + e));
-            v[m] = (kind_neg_odd(kind) && (j & 1)) ? cneg(z) : z;
-        }
-        __syncwarp();
-#pragma unroll
-        for (int m = 0; m < R1; ++m) t[at(lane + 32 * m, f)] = v[m];
-        __syncwarp();
-    }
     // natural-order spectrum -> slot rows (2s, 2s+1), in place through registers (YPass::store_forward)
     static CANS_D void slots_out(const XYArgs& a, cplx* t, int f, int lane) {
         constexpr int NS = H / 32;
-        cplx zq[NS], zm[NS];
+        cplx zq[NS], zm[NS], wq[NS];
+        if (!IS_PP) {                         // post-twiddles: issued before the shared-memory reads
+#pragma unroll
+            for (int m = 0; m < NS; ++m) wq[m] = __ldg(a.wpost + lane + 32 * m);
+        }
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
             zq[m] = t[at(s, f)];
-            zm[m] = t[at(kind_mixed(a.kind) ? N - 1 - s : (s == 0 ? H : N - s), f)];
+            zm[m] = t[at(IS_MIXED ? N - 1 - s : (s == 0 ? H : N - s), f)];
         }
         __syncwarp();
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
             cplx r0, r1;
-            if (s == 0 && !kind_mixed(a.kind)) {
-                const double c = (a.kind == KIND_PP) ? 1.0 : CANS_SQRT_HALF;
+            if (s == 0 && !IS_MIXED) {
+                const double c = IS_PP ? 1.0 : CANS_SQRT_HALF;
                 r0 = make_double2(zq[m].x, zq[m].y);
                 r1 = make_double2(c * zm[m].x, c * zm[m].y);
             } else {
-                cplx wq = make_double2(1.0, 0.0);
-                if (a.kind != KIND_PP) wq = __ldg(a.wpost + s);
                 double A0, A1, B0, B1;
-                post_forward(zq[m], zm[m], wq, a.kind, A0, A1, B0, B1);
+                post_forward(zq[m], zm[m], IS_PP ? make_double2(1.0, 0.0) : wq[m], IS_PP ? (int)KIND_PP : a.kind, A0, A1, B0, B1);
                 r0 = make_double2(A0, B0);
                 r1 = make_double2(A1, B1);
             }
@@ -169,7 +197,11 @@ struct YTPass {
     // slot rows -> natural-order spectrum, in place through registers (YPass::load_inverse)
     static CANS_D void slots_in(const XYArgs& a, cplx* t, int f, int lane) {
         constexpr int NS = H / 32;
-        cplx r0[NS], r1[NS];
+        cplx r0[NS], r1[NS], wq[NS];
+        if (!IS_PP) {
+#pragma unroll
+            for (int m = 0; m < NS; ++m) wq[m] = __ldg(a.wpost + lane + 32 * m);
+        }
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
@@ -183,17 +215,15 @@ struct YTPass {
 #pragma unroll
         for (int m = 0; m < NS; ++m) {
             const int s = lane + 32 * m;
-            if (s == 0 && !kind_mixed(a.kind)) {
-                const double c = (a.kind == KIND_PP) ? 1.0 : (1.0 / CANS_SQRT_HALF);
+            if (s == 0 && !IS_MIXED) {
+                const double c = IS_PP ? 1.0 : (1.0 / CANS_SQRT_HALF);
                 t[at(0, f)] = make_double2(r0[m].x, r0[m].y);
                 t[at(H, f)] = make_double2(c * r1[m].x, c * r1[m].y);
             } else {
-                cplx wq = make_double2(1.0, 0.0);
-                if (a.kind != KIND_PP) wq = __ldg(a.wpost + s);
                 cplx Zq, Zm;
-                pre_inverse(r0[m].x, r1[m].x, r0[m].y, r1[m].y, wq, a.kind, Zq, Zm);
+                pre_inverse(r0[m].x, r1[m].x, r0[m].y, r1[m].y, IS_PP ? make_double2(1.0, 0.0) : wq[m], IS_PP ? (int)KIND_PP : a.kind, Zq, Zm);
                 t[at(s, f)] = Zq;
-                t[at(kind_mixed(a.kind) ? N - 1 - s : N - s, f)] = Zm;
+                t[at(IS_MIXED ? N - 1 - s : N - s, f)] = Zm;
             }
         }
         __syncwarp();
