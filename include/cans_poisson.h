@@ -49,7 +49,7 @@ typedef struct cans_poisson_plan cans_poisson_plan;   /* opaque, owned by the li
  *   nx, ny, nz   cells per direction (x, y uniform: "uniformly-spaced in two directions").
  *                nx and ny must be one of 16,32,48,64,96,128,192,256,384,512,768,1024,1536,2048
  *                (512, 768 and 1024 run the warp-level 2-pass kernels, the others the 3-pass kernels);
- *                2 <= nz <= 1024 (periodic z: <= 960).
+ *                2 <= nz <= 1024.
  *   lx, ly, lz   domain lengths (> 0); dx = lx/nx, dy = ly/ny.
  *   bc           bc[d][0] / bc[d][1] = PRESSURE boundary condition on the lower / upper face of
  *                direction d (0 = x, 1 = y, 2 = z), homogeneous, imposed at the boundary face:

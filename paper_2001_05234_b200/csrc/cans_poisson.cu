@@ -394,7 +394,7 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     const int nseg = (nz + Z_MROWS - 1) / Z_MROWS;
     if (nseg > 64) { fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the z-solve tiling (max 1024)"); return nullptr; }
     if (z_solve_smem_bytes(nseg, bc[2][0] == 'P') > Z_SMEM_LIMIT) {
-        fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the periodic z solve (three tile buffers in shared memory: max 960)");
+        fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the z-solve tiling (shared memory)");
         return nullptr;
     }
     std::vector<double> hdzc(nz + 1), hdzf(nz);

@@ -27,9 +27,11 @@
 // Periodic z (the triperiodic Taylor-Green case of P:L222): the system is cyclic, row 0 couples to
 // x_{nz-1} through a_0 and row nz-1 to x_0 through c_{nz-1}.  Sherman-Morrison on the same partitioned Thomas: with
 // gamma = -(b_0 + lam), the open matrix T' = T - u v^T (u = (gamma, 0, .., 0, c_{nz-1}), v = (1, 0, .., 0, a_0/gamma))
-// has b'_0 = 2 (b_0 + lam) and b'_{nz-1} = b_{nz-1} + lam + c_{nz-1} a_0 / (b_0 + lam); per tile the kernel solves
-// T' q = u (no field data needed: it runs while the tile is still in flight, result kept in a third shared-memory
-// buffer), then T' y = d with the same pivots, and stores x = y - q (y_0 + v_n y_{nz-1}) / (1 + q_0 + v_n q_{nz-1}).
+// has b'_0 = 2 (b_0 + lam) and b'_{nz-1} = b_{nz-1} + lam + c_{nz-1} a_0 / (b_0 + lam).  T' q = u and T' y = d share the
+// pivots AND the propagation factors of both sweeps, so q rides along in the same three phases: its forward values cost
+// one FMA per row, its rows live in the tile's own staging buffer (free once the right-hand side is in registers), and
+// x = y - q (y_0 + v_n y_{nz-1}) / (1 + q_0 + v_n q_{nz-1}) is formed in the final store loop (one more CTA barrier
+// than the open system, for the four edge values of each column).
 #pragma once
 #include "common.cuh"
 
@@ -93,19 +95,24 @@ struct ZState {
     double d[MROWS];
     double r[MROWS];
     double start;     // true d'_{k0-1}, later true x_{k0+MROWS}
+    double startq;    // the same for the correction vector q of a cyclic system
     long col;
     bool active;
 };
 
-// shared memory (doubles): tables az,bz,cz,gz [4][nzp]; scan arrays end[TC*P], fac[TC*P] of the forward sweep and a
-// second pair for the backward sweep (so that no barrier is needed between reading one and writing the other);
-// (y_0, y_{nz-1}) per column of the cyclic solve [2*TC]; two tile buffers [nzp][TC]; cyclic: a third one for q
+// shared memory (doubles): tables az,bz,cz,gz [4][nzp]; (end, factor) pairs of the forward sweep [TC*P] and a second
+// array for the backward sweep (so that no barrier is needed between reading one and writing the other); the same two
+// arrays of segment ends for q [TC*P] each; (y_0, q_0, y_{nz-1}, q_{nz-1}) per column of a cyclic solve [4*TC]; two tile
+// buffers [nzp][TC]
 template <int MROWS, int TC>
 struct ZPass {
-    static CANS_HD size_t edge_offset(int nseg) { return (size_t)4 * nseg * MROWS + (size_t)4 * TC * nseg; }
-    static CANS_HD size_t table_doubles(int nseg) { return edge_offset(nseg) + 2 * TC; }
+    static CANS_HD size_t scan_offset(int nseg) { return (size_t)4 * nseg * MROWS; }
+    static CANS_HD size_t scanq_offset(int nseg) { return scan_offset(nseg) + (size_t)4 * TC * nseg; }
+    static CANS_HD size_t edge_offset(int nseg) { return scanq_offset(nseg) + (size_t)2 * TC * nseg; }
+    // (rounded up to 1 KB so that the tile buffers the TMA unit fills start on a 1 KB boundary)
+    static CANS_HD size_t table_doubles(int nseg) { return (edge_offset(nseg) + 4 * TC + 127) / 128 * 128; }
     static CANS_HD size_t tile_doubles(int nseg) { return (size_t)nseg * MROWS * TC; }
-    static CANS_HD size_t smem_doubles(int nseg, int cyclic) { return table_doubles(nseg) + (2 + (cyclic ? 1 : 0)) * tile_doubles(nseg); }
+    static CANS_HD size_t smem_doubles(int nseg) { return table_doubles(nseg) + 2 * tile_doubles(nseg); }
 
     static CANS_HD void load_tables(const ZArgs& a, double* sm, int tid, int nthreads) {
         const int nzp = a.nseg * MROWS;
@@ -117,17 +124,32 @@ struct ZPass {
         }
     }
 
-    // phase 1: take the segment from the tile buffer, pivots, local forward sweep from a zero start;
-    // publish (end, factor).  MODE 0: open system.  Cyclic system: MODE 1 = right-hand side u with the pivots of T'
-    // (no tile data), MODE 2 = the tile's right-hand side with the pivots MODE 1 left in st.r.
-    template <int MODE>
+    // The two rows in which the open matrix T' and the right-hand side u of the correction system differ from the plain
+    // tridiagonal rows, as seen by the thread of segment s: row 0 (diagonal doubled, u_0 = gamma = -(b_0 + lam)) and row
+    // nz-1 (diagonal + c_{nz-1} a_0 / (b_0 + lam), u_{nz-1} = c_{nz-1}).
+    struct CyclicRows {
+        double diag0 = 0.0, rhs0 = 0.0, diagn = 0.0;
+        int rl = -1;
+    };
+    static CANS_HD CyclicRows cyclic_rows(const ZArgs& a, double b0, double lam, int s) {
+        CyclicRows cr;
+        const double bl0 = b0 + lam;
+        if (s == 0) { cr.diag0 = bl0; cr.rhs0 = -bl0; }
+        if (s == (a.nz - 1) / MROWS) { cr.rl = (a.nz - 1) - s * MROWS; cr.diagn = a.cw * a.a0w / bl0; }
+        return cr;
+    }
+
+    // phase 1: take the segment from the tile buffer, pivots, local forward sweep from a zero start; publish (end, factor)
+    // -- and, for a cyclic system, the end of q's local forward sweep
+    template <bool CYC>
     static CANS_HD void phase1(const ZArgs& a, double* sm, const double* buf, ZState<MROWS>& st, long tile,
                                double rstart_val, double lam, int tid) {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
         const double* sbz = sm + nzp;
         const double* sgz = sm + 3 * nzp;
-        double2* s_scan = reinterpret_cast<double2*>(sm + 4 * nzp);      // forward (end, factor) pairs
+        double2* s_scan = reinterpret_cast<double2*>(sm + scan_offset(a.nseg));      // forward (end, factor) pairs
+        double* s_scanq = sm + scanq_offset(a.nseg);
         const int c = tid % TC;
         const int s = tid / TC;
         const long col = tile * TC + c;
@@ -138,82 +160,112 @@ struct ZPass {
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
                 const int k = k0 + r;
-                if (MODE == 1) st.d[r] = (k == 0) ? -(sbz[0] + lam) : ((k == a.nz - 1) ? a.cw : 0.0);
-                else st.d[r] = (k < a.nz) ? buf[(size_t)k * TC + c] * a.scale : 0.0;
+                st.d[r] = (k < a.nz) ? buf[(size_t)k * TC + c] * a.scale : 0.0;
             }
             double rp = rstart_val;
-            double dp = 0.0, fac = 1.0;
+            double dp = 0.0, fac = 1.0, dq = 0.0;
+            // cyclic system: only rows 0 and nz-1 differ from the open one -- row 0 belongs to segment 0 (r = 0 at compile
+            // time), row nz-1 to local row rl of the last segment (rl = -1 elsewhere)
+            const CyclicRows cr = CYC ? cyclic_rows(a, sbz[0], lam, s) : CyclicRows();
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
                 const int k = k0 + r;
-                if (MODE == 0) rp = z_pivot(sbz[k], lam, sgz[k], rp);
-                else if (MODE == 1) rp = z_pivot_bl(z_cyclic_diag(a, k, sbz[k], sbz[0], lam), sgz[k], rp);
-                else rp = st.r[r];
+                double bl = sbz[k] + lam;
+                if (CYC) {
+                    if (r == 0) bl += cr.diag0;
+                    if (r == cr.rl) bl += cr.diagn;
+                }
+                rp = z_pivot_bl(bl, sgz[k], rp);
                 st.r[r] = rp;
                 const double e = saz[k] * rp;
                 dp = st.d[r] * rp - e * dp;
                 st.d[r] = dp;
                 fac *= -e;
+                if (CYC) {
+                    dq = -e * dq;
+                    if (r == 0) dq = cr.rhs0 * rp;            // (e = 0 in row 0 of segment 0; rhs0 = 0 elsewhere keeps dq = -e dq)
+                    if (r == cr.rl) dq = fma(a.cw, rp, dq);
+                }
             }
             s_scan[s * TC + c] = make_double2(dp, fac);
+            if (CYC) s_scanq[s * TC + c] = dq;
         } else {
             s_scan[s * TC + c] = make_double2(0.0, 0.0);
+            if (CYC) s_scanq[s * TC + c] = 0.0;
         }
     }
 
     // phase 2: scan the segment ends -> true start; propagate; local backward sweep from a zero start; publish
+    template <bool CYC>
     static CANS_HD void phase2a(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
-        const int nzp = a.nseg * MROWS;
-        const double2* s_scan = reinterpret_cast<const double2*>(sm + 4 * nzp);
+        const double2* s_scan = reinterpret_cast<const double2*>(sm + scan_offset(a.nseg));
+        const double* s_scanq = sm + scanq_offset(a.nseg);
         const int c = tid % TC;
         const int s = tid / TC;
-        double D = 0.0;                     // true d' at the end of segment s'-1
+        double D = 0.0, Dq = 0.0;           // true d' (and q's) at the end of segment s'-1
 #pragma unroll 4
         for (int q = 0; q < s; ++q) {
             const double2 ef = s_scan[q * TC + c];      // one 16-byte load per segment
             D = ef.x + ef.y * D;
+            if (CYC) Dq = s_scanq[q * TC + c] + ef.y * Dq;
         }
         st.start = D;
+        st.startq = Dq;
     }
-    // (2b publishes into the backward pair of scan arrays, so 2a and 2b need no barrier between them)
-    static CANS_HD void phase2b(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid) {
+    // (2b publishes into the backward arrays, so 2a and 2b need no barrier between them).  Cyclic: q's true forward values
+    // are rebuilt row by row from its true start and parked in qbuf, then swept backwards in place.
+    template <bool CYC>
+    static CANS_HD void phase2b(const ZArgs& a, double* sm, ZState<MROWS>& st, double lam, int tid, double* qbuf) {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
         const double* scz = sm + 2 * nzp;
-        double2* s_scan = reinterpret_cast<double2*>(sm + 4 * nzp + 2 * TC * a.nseg);   // backward pairs
+        double2* s_scan = reinterpret_cast<double2*>(sm + scan_offset(a.nseg)) + TC * a.nseg;   // backward pairs
+        double* s_scanq = sm + scanq_offset(a.nseg) + TC * a.nseg;
         const int c = tid % TC;
         const int s = tid / TC;
         const int k0 = s * MROWS;
         if (st.col < a.ncols) {
             double fac = 1.0;
             const double D = st.start;
+            double dq = st.startq;
+            const CyclicRows cr = CYC ? cyclic_rows(a, sm[nzp], lam, s) : CyclicRows();
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) {
-                fac *= -(saz[k0 + r] * st.r[r]);
+                const double e = saz[k0 + r] * st.r[r];
+                fac *= -e;
                 st.d[r] += fac * D;
+                if (CYC) {
+                    dq = -e * dq;
+                    if (r == 0) dq = fma(cr.rhs0, st.r[r], dq);
+                    if (r == cr.rl) dq = fma(a.cw, st.r[r], dq);
+                    qbuf[(size_t)(k0 + r) * TC + c] = dq;
+                }
             }
-            double xs = 0.0, g = 1.0;
+            double xs = 0.0, g = 1.0, xq = 0.0;
 #pragma unroll
             for (int r = MROWS - 1; r >= 0; --r) {
                 const double cp = scz[k0 + r] * st.r[r];
                 xs = st.d[r] - cp * xs;
                 st.d[r] = xs;
                 g *= -cp;
+                if (CYC) {
+                    xq = qbuf[(size_t)(k0 + r) * TC + c] - cp * xq;
+                    qbuf[(size_t)(k0 + r) * TC + c] = xq;
+                }
             }
             s_scan[s * TC + c] = make_double2(xs, g);     // x^0 at the top row of the segment, its factor
+            if (CYC) s_scanq[s * TC + c] = xq;
         } else {
             s_scan[s * TC + c] = make_double2(0.0, 0.0);
+            if (CYC) s_scanq[s * TC + c] = 0.0;
         }
     }
 
-    // phase 3: scan from the bottom -> true x below the segment; propagate; DEST 0: store to the field (open system),
-    // 1: store to the shared-memory buffer qbuf (cyclic: the correction vector q), 2: keep in st.d (cyclic: y)
-    template <int DEST>
-    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, double* qbuf = nullptr,
-                               const double* buf = nullptr) {
+    // phase 3 of the open system: scan from the bottom -> true x below the segment; propagate; store to the field
+    static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, const double* buf) {
         const int nzp = a.nseg * MROWS;
         const double* scz = sm + 2 * nzp;
-        const double2* s_scan = reinterpret_cast<const double2*>(sm + 4 * nzp + 2 * TC * a.nseg);   // backward pairs
+        const double2* s_scan = reinterpret_cast<const double2*>(sm + scan_offset(a.nseg)) + TC * a.nseg;   // backward pairs
         const int c = tid % TC;
         const int s = tid / TC;
         const int k0 = s * MROWS;
@@ -223,7 +275,7 @@ struct ZPass {
             const double2 ef = s_scan[q * TC + c];
             X = ef.x + ef.y * X;
         }
-        if (DEST == 0 ? st.active : (st.col < a.ncols)) {
+        if (st.active) {
             const size_t plane = (size_t)a.ncols;
             double g = 1.0;
 #pragma unroll
@@ -231,47 +283,67 @@ struct ZPass {
                 g *= -(scz[k0 + r] * st.r[r]);
                 st.d[r] += g * X;
             }
-            if (DEST == 0) {
 #pragma unroll
-                for (int r = 0; r < MROWS; ++r) {
-                    const int k = k0 + r;
-                    // (the tile buffer still holds this tile: its buffer is not refilled before the next iteration)
-                    if (k < a.nz) a.p[(size_t)k * plane + st.col] = (k < a.nz_solve) ? st.d[r] : buf[(size_t)k * TC + c] * a.scale;
-                }
-            } else if (DEST == 1) {
-#pragma unroll
-                for (int r = 0; r < MROWS; ++r) qbuf[(size_t)(k0 + r) * TC + c] = st.d[r];
+            for (int r = 0; r < MROWS; ++r) {
+                const int k = k0 + r;
+                // (the tile buffer still holds this tile: its buffer is not refilled before the next iteration)
+                if (k < a.nz) a.p[(size_t)k * plane + st.col] = (k < a.nz_solve) ? st.d[r] : buf[(size_t)k * TC + c] * a.scale;
             }
         }
     }
 
-    // cyclic system, after phase3<2>: publish y_0 and y_{nz-1} of the column ...
-    static CANS_HD void cyclic_publish(const ZArgs& a, double* sm, const ZState<MROWS>& st, int tid) {
+    // phase 3 of a cyclic system, first half: the backward scans of y and q; the threads holding rows 0 and nz-1 publish
+    // the true (y_0, q_0) and (y_{nz-1}, q_{nz-1}) of their column
+    static CANS_HD void cyclic_scan(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, const double* qbuf) {
+        const double2* s_scan = reinterpret_cast<const double2*>(sm + scan_offset(a.nseg)) + TC * a.nseg;
+        const double* s_scanq = sm + scanq_offset(a.nseg) + TC * a.nseg;
         double* edge = sm + edge_offset(a.nseg);
         const int c = tid % TC;
         const int s = tid / TC;
-        if (s == 0) edge[2 * c] = st.d[0];
-        if (s == (a.nz - 1) / MROWS) {
-            double yn = 0.0;
+        double X = 0.0, Xq = 0.0;
+#pragma unroll 4
+        for (int q = a.nseg - 1; q > s; --q) {
+            const double2 ef = s_scan[q * TC + c];
+            X = ef.x + ef.y * X;
+            Xq = s_scanq[q * TC + c] + ef.y * Xq;
+        }
+        st.start = X;
+        st.startq = Xq;
+        if (st.col < a.ncols) {
+            if (s == 0) {                                   // row 0: local value + (factor of the whole segment) * X
+                const double g = s_scan[c].y;
+                edge[4 * c] = st.d[0] + g * X;
+                edge[4 * c + 1] = qbuf[c] + g * Xq;
+            }
+            if (s == (a.nz - 1) / MROWS) {                  // row nz-1: last segment, nothing above it: local = true
+                double yn = 0.0;
 #pragma unroll
-            for (int r = 0; r < MROWS; ++r) if (s * MROWS + r == a.nz - 1) yn = st.d[r];
-            edge[2 * c + 1] = yn;
+                for (int r = 0; r < MROWS; ++r) if (s * MROWS + r == a.nz - 1) yn = st.d[r];
+                edge[4 * c + 2] = yn;
+                edge[4 * c + 3] = qbuf[(size_t)(a.nz - 1) * TC + c];
+            }
         }
     }
-    // ... and (behind a barrier) combine: x = y - q (y_0 + v y_n) / (1 + q_0 + v q_n), v = a_0 / gamma
+    // ... second half (behind a barrier): x = y - q (y_0 + v y_n) / (1 + q_0 + v q_n), v = a_0 / gamma, with the
+    // propagation of both backward sweeps folded into one term
     static CANS_HD void cyclic_store(const ZArgs& a, double* sm, const ZState<MROWS>& st, double lam, int tid, const double* qbuf) {
         if (!st.active) return;
         const double* edge = sm + edge_offset(a.nseg);
         const int nzp = a.nseg * MROWS;
+        const double* scz = sm + 2 * nzp;
         const int c = tid % TC;
         const int k0 = (tid / TC) * MROWS;
         const double v = a.a0w / -(sm[nzp] + lam);                     // sm[nzp] = bz[0]
-        const double fact = (edge[2 * c] + v * edge[2 * c + 1]) / (1.0 + qbuf[c] + v * qbuf[(size_t)(a.nz - 1) * TC + c]);
+        const double fact = (edge[4 * c] + v * edge[4 * c + 2]) / (1.0 + edge[4 * c + 1] + v * edge[4 * c + 3]);
+        const double Xc = st.start - st.startq * fact;
         const size_t plane = (size_t)a.ncols;
+        double g = 1.0;
 #pragma unroll
-        for (int r = 0; r < MROWS; ++r) {
+        for (int r = MROWS - 1; r >= 0; --r) {
             const int k = k0 + r;
-            if (k < a.nz) a.p[(size_t)k * plane + st.col] = st.d[r] - qbuf[(size_t)k * TC + c] * fact;
+            g *= -(scz[k] * st.r[r]);
+            const double x = (st.d[r] - qbuf[(size_t)k * TC + c] * fact) + g * Xc;
+            if (k < a.nz) a.p[(size_t)k * plane + st.col] = x;
         }
     }
 };

@@ -6,15 +6,16 @@ namespace cans {
 
 template <int MROWS, int TC, bool CYC>
 __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __grid_constant__ CUtensorMap tmap) {
-    extern __shared__ __align__(128) double zsm[];
+    extern __shared__ __align__(1024) double zsm[];
     typedef ZPass<MROWS, TC> Z;
     __shared__ long s_next;
     __shared__ __align__(8) unsigned long long s_bar[2];
-    const int tid = threadIdx.x;
+    int tid = threadIdx.x;
+    asm volatile("" : "+r"(tid));              // opaque: keeps the thread index in a register (the compiler otherwise re-reads
+                                             // the special register ~14 times per warp and tile, a long-latency S2R each)
     const int nthreads = blockDim.x;
     double* bufs = zsm + Z::table_doubles(a.nseg);
     const size_t tile_sz = Z::tile_doubles(a.nseg);
-    double* qbuf = bufs + 2 * tile_sz;          // cyclic systems only
 
     if (a.singular && blockIdx.x == 0) {
         // the singular (0,0) column, staged in shared memory, solved by one thread (reading S3)
@@ -70,39 +71,36 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
     tile_scalars(cur, rs, l1, l2);
     __syncthreads();                           // the first s_next is visible
     while (true) {
-        // No barrier here: s_next was rewritten behind the phase-1 barrier of the previous tile and published by
-        // its phase-2 barrier; buffer b^1 was last read in that tile's phase 1, also behind that barrier.
+        // Open system: no barrier here -- s_next was rewritten behind the phase-1 barrier of the previous tile and published
+        // by its phase-2 barrier; buffer b^1 was last read in that tile's phase 1, also behind that barrier.
+        // Cyclic system: buffer b^1 held the previous tile's q until the end of that iteration, so the copy of the next tile
+        // into it is issued behind this tile's phase-1 barrier instead (every thread has left the previous iteration).
         const long nxt = s_next;
-        if (tid == 0 && nxt < a.ntiles) issue_tile(nxt, b ^ 1);
+        if (!CYC && tid == 0 && nxt < a.ntiles) issue_tile(nxt, b ^ 1);
         double rs_n, l1_n, l2_n;
         tile_scalars(nxt, rs_n, l1_n, l2_n);   // consumed in the next iteration
         ZState<MROWS> st;
-        if (CYC) {
-            // the correction vector q of this tile's modes (needs no field data) while the tile is still in flight
-            Z::template phase1<1>(a, zsm, nullptr, st, cur, rs, l1 + l2 + a.alpha, tid);
-            __syncthreads();
-            Z::phase2a(a, zsm, st, tid);
-            Z::phase2b(a, zsm, st, tid);
-            __syncthreads();
-            Z::template phase3<1>(a, zsm, st, tid, qbuf);
-        }
+        // (buffer address and eigenvalue sum are re-formed at every use: at the 128-register cap of a 512-thread CTA each
+        // value kept live across the phases costs a rematerialised S2R or a spill elsewhere)
         mbar_wait(&s_bar[b], (phases >> b) & 1u);   // the current tile has landed (the next may still fly)
         phases ^= 1u << b;
-        if (CYC) Z::template phase1<2>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2 + a.alpha, tid);
-        else Z::template phase1<0>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2 + a.alpha, tid);
+        Z::template phase1<CYC>(a, zsm, bufs + (size_t)b * tile_sz, st, cur, rs, l1 + l2 + a.alpha, tid);
         __syncthreads();
         // every thread has read s_next (before the barrier above): thread 0 may now draw the ticket after next
-        if (tid == 0 && nxt < a.ntiles) s_next = (long)atomicAdd(a.ticket, 1u);
-        Z::phase2a(a, zsm, st, tid);
-        Z::phase2b(a, zsm, st, tid);
+        if (tid == 0 && nxt < a.ntiles) {
+            if (CYC) issue_tile(nxt, b ^ 1);
+            s_next = (long)atomicAdd(a.ticket, 1u);
+        }
+        Z::template phase2a<CYC>(a, zsm, st, tid);
+        Z::template phase2b<CYC>(a, zsm, st, l1 + l2 + a.alpha, tid, bufs + (size_t)b * tile_sz);    // cyclic: the tile's buffer, now free, holds q
         __syncthreads();
         if (CYC) {
-            Z::template phase3<2>(a, zsm, st, tid);
-            Z::cyclic_publish(a, zsm, st, tid);
+            Z::cyclic_scan(a, zsm, st, tid, bufs + (size_t)b * tile_sz);
             __syncthreads();
-            Z::cyclic_store(a, zsm, st, l1 + l2 + a.alpha, tid, qbuf);
+            Z::cyclic_store(a, zsm, st, l1 + l2 + a.alpha, tid, bufs + (size_t)b * tile_sz);
+            fence_proxy_async_smem();           // this thread's accesses to q are ordered before the TMA refill of the buffer
         } else {
-            Z::template phase3<0>(a, zsm, st, tid, nullptr, bufs + (size_t)b * tile_sz);
+            Z::phase3(a, zsm, st, tid, bufs + (size_t)b * tile_sz);
         }
         if (nxt >= a.ntiles) break;
         cur = nxt;
@@ -119,7 +117,7 @@ __global__ void z_setup_kernel(const ZArgs a, double* rstart, double* r00) {
 
 template <int TC, bool CYC>
 static cudaError_t configure_tc(int nseg, int num_sms, int* grid_out, size_t* smem_out) {
-    size_t smem = sizeof(double) * ZPass<Z_MROWS, TC>::smem_doubles(nseg, CYC ? 1 : 0);
+    size_t smem = sizeof(double) * ZPass<Z_MROWS, TC>::smem_doubles(nseg);
     if (smem > Z_SMEM_LIMIT) return cudaErrorInvalidConfiguration;       // the plan checks z_solve_smem_bytes first
     cudaError_t e = cudaFuncSetAttribute(z_solve_kernel<Z_MROWS, TC, CYC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -135,9 +133,9 @@ static cudaError_t configure_tc(int nseg, int num_sms, int* grid_out, size_t* sm
 
 size_t z_solve_smem_bytes(int nseg, int cyclic) {
     switch (z_tc_for(nseg)) {
-        case 32: return sizeof(double) * ZPass<Z_MROWS, 32>::smem_doubles(nseg, cyclic);
-        case 16: return sizeof(double) * ZPass<Z_MROWS, 16>::smem_doubles(nseg, cyclic);
-        default: return sizeof(double) * ZPass<Z_MROWS, 8>::smem_doubles(nseg, cyclic);
+        case 32: return sizeof(double) * ZPass<Z_MROWS, 32>::smem_doubles(nseg);
+        case 16: return sizeof(double) * ZPass<Z_MROWS, 16>::smem_doubles(nseg);
+        default: return sizeof(double) * ZPass<Z_MROWS, 8>::smem_doubles(nseg);
     }
 }
 

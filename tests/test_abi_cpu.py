@@ -49,7 +49,7 @@ PP_NN = (("P", "P"), ("P", "P"), ("N", "N"))
     (dict(nx=32, ny=32, nz=32, lx=-1.0), 1),
     (dict(nx=32, ny=32, nz=32, bc=(("P", "N"), ("P", "P"), ("N", "N"))), 1),      # one-sided periodic
     (dict(nx=32, ny=32, nz=32, bc=(("X", "X"), ("P", "P"), ("N", "N"))), 1),      # unknown letter
-    (dict(nx=32, ny=32, nz=1000, bc=(("P", "P"), ("P", "P"), ("P", "P"))), 3),    # periodic z: nz <= 960
+    (dict(nx=32, ny=32, nz=1025, bc=(("P", "P"), ("P", "P"), ("P", "P"))), 3),    # nz <= 1024 (periodic z as well)
     (dict(nx=40, ny=32, nz=32), 3),                                                # 40 = 2^3*5
     (dict(nx=32, ny=32, nz=2000), 3),
     (dict(nx=32, ny=32, nz=4, dzf=[0.5, 0.5, -0.5, 0.5], dzc=[0.5] * 5), 1),
