@@ -61,6 +61,7 @@ struct ZArgs {
                               // (scaled): the wall slot of a face-located unknown (nz_solve = nz - 1), else nz_solve = nz
     int cyclic;               // 1: z is periodic (az[0] = cz[nz-1] = 0 in the tables, the wrap couplings are below)
     double a0w, cw;           // a_0 = 1/(dzf_0 dzc_0) and c_{nz-1} = 1/(dzf_{nz-1} dzc_nz) of the cyclic system
+    unsigned long long nx_magic;   // ceil(2^40 / nx): j = (col * nx_magic) >> 40 is col / nx exactly for col < nx*ny <= 2^22
     int nbox, box_rows;       // TMA tiling of a column tile: nbox boxes of box_rows rows (set by z_solve_launch)
 };
 
@@ -139,6 +140,67 @@ struct ZPass {
         return cr;
     }
 
+    // the rows of phase 1 (CYC: cyclic system; LAST: this thread's segment holds row nz-1, at local row cr.rl)
+    template <bool CYC, bool LAST>
+    static CANS_HD void phase1_rows(const ZArgs& a, const double* saz, const double* sbz, const double* sgz, ZState<MROWS>& st,
+                                    int k0, double rstart_val, double lam, const CyclicRows& cr, double& dp_out, double& fac_out,
+                                    double& dq_out) {
+        double rp = rstart_val;
+        double dp = 0.0, fac = 1.0, dq = 0.0;
+#pragma unroll
+        for (int r = 0; r < MROWS; ++r) {
+            const int k = k0 + r;
+            double bl = sbz[k] + lam;
+            if (CYC && r == 0) bl += cr.diag0;
+            if (LAST && r == cr.rl) bl += cr.diagn;
+            rp = z_pivot_bl(bl, sgz[k], rp);
+            st.r[r] = rp;
+            const double e = saz[k] * rp;
+            dp = st.d[r] * rp - e * dp;
+            st.d[r] = dp;
+            fac *= -e;
+            if (CYC) {
+                if (r == 0) dq = cr.rhs0 * rp;             // zero start; rhs0 = gamma in segment 0, 0 elsewhere
+                else dq = -e * dq;
+                if (LAST && r == cr.rl) dq = fma(a.cw, rp, dq);
+            }
+        }
+        dp_out = dp; fac_out = fac; dq_out = dq;
+    }
+    // the rows of phase 2b
+    template <bool CYC, bool LAST>
+    static CANS_HD void phase2b_rows(const ZArgs& a, const double* saz, const double* scz, ZState<MROWS>& st, int k0,
+                                     const CyclicRows& cr, double* qcol, double& xs_out, double& g_out, double& xq_out) {
+        double fac = 1.0;
+        const double D = st.start;
+        double dq = st.startq;
+#pragma unroll
+        for (int r = 0; r < MROWS; ++r) {
+            const double e = saz[k0 + r] * st.r[r];
+            fac *= -e;
+            st.d[r] += fac * D;
+            if (CYC) {
+                dq = -e * dq;
+                if (r == 0) dq = fma(cr.rhs0, st.r[r], dq);
+                if (LAST && r == cr.rl) dq = fma(a.cw, st.r[r], dq);
+                qcol[r * TC] = dq;
+            }
+        }
+        double xs = 0.0, g = 1.0, xq = 0.0;
+#pragma unroll
+        for (int r = MROWS - 1; r >= 0; --r) {
+            const double cp = scz[k0 + r] * st.r[r];
+            xs = st.d[r] - cp * xs;
+            st.d[r] = xs;
+            g *= -cp;
+            if (CYC) {
+                xq = qcol[r * TC] - cp * xq;
+                qcol[r * TC] = xq;
+            }
+        }
+        xs_out = xs; g_out = g; xq_out = xq;
+    }
+
     // phase 1: take the segment from the tile buffer, pivots, local forward sweep from a zero start; publish (end, factor)
     // -- and, for a cyclic system, the end of q's local forward sweep
     template <bool CYC>
@@ -157,35 +219,18 @@ struct ZPass {
         st.active = (col < a.ncols) && !(a.singular && col == 0);
         const int k0 = s * MROWS;
         if (col < a.ncols) {
+            // (rows nz..nzp-1 of the buffer lie outside the tensor: the TMA unit filled them with zeros)
 #pragma unroll
-            for (int r = 0; r < MROWS; ++r) {
-                const int k = k0 + r;
-                st.d[r] = (k < a.nz) ? buf[(size_t)k * TC + c] * a.scale : 0.0;
-            }
-            double rp = rstart_val;
-            double dp = 0.0, fac = 1.0, dq = 0.0;
-            // cyclic system: only rows 0 and nz-1 differ from the open one -- row 0 belongs to segment 0 (r = 0 at compile
-            // time), row nz-1 to local row rl of the last segment (rl = -1 elsewhere)
-            const CyclicRows cr = CYC ? cyclic_rows(a, sbz[0], lam, s) : CyclicRows();
-#pragma unroll
-            for (int r = 0; r < MROWS; ++r) {
-                const int k = k0 + r;
-                double bl = sbz[k] + lam;
-                if (CYC) {
-                    if (r == 0) bl += cr.diag0;
-                    if (r == cr.rl) bl += cr.diagn;
-                }
-                rp = z_pivot_bl(bl, sgz[k], rp);
-                st.r[r] = rp;
-                const double e = saz[k] * rp;
-                dp = st.d[r] * rp - e * dp;
-                st.d[r] = dp;
-                fac *= -e;
-                if (CYC) {
-                    dq = -e * dq;
-                    if (r == 0) dq = cr.rhs0 * rp;            // (e = 0 in row 0 of segment 0; rhs0 = 0 elsewhere keeps dq = -e dq)
-                    if (r == cr.rl) dq = fma(a.cw, rp, dq);
-                }
+            for (int r = 0; r < MROWS; ++r) st.d[r] = buf[(size_t)(k0 + r) * TC + c] * a.scale;
+            double dp, fac, dq;
+            if (!CYC) {
+                phase1_rows<false, false>(a, saz, sbz, sgz, st, k0, rstart_val, lam, CyclicRows(), dp, fac, dq);
+            } else {
+                // cyclic system: only rows 0 and nz-1 differ from the open one -- row 0 belongs to segment 0 (r = 0 at
+                // compile time), row nz-1 to local row rl of the last segment: its threads run their own copy of the loop
+                const CyclicRows cr = cyclic_rows(a, sbz[0], lam, s);
+                if (cr.rl < 0) phase1_rows<true, false>(a, saz, sbz, sgz, st, k0, rstart_val, lam, cr, dp, fac, dq);
+                else phase1_rows<true, true>(a, saz, sbz, sgz, st, k0, rstart_val, lam, cr, dp, fac, dq);
             }
             s_scan[s * TC + c] = make_double2(dp, fac);
             if (CYC) s_scanq[s * TC + c] = dq;
@@ -225,33 +270,14 @@ struct ZPass {
         const int s = tid / TC;
         const int k0 = s * MROWS;
         if (st.col < a.ncols) {
-            double fac = 1.0;
-            const double D = st.start;
-            double dq = st.startq;
-            const CyclicRows cr = CYC ? cyclic_rows(a, sm[nzp], lam, s) : CyclicRows();
-#pragma unroll
-            for (int r = 0; r < MROWS; ++r) {
-                const double e = saz[k0 + r] * st.r[r];
-                fac *= -e;
-                st.d[r] += fac * D;
-                if (CYC) {
-                    dq = -e * dq;
-                    if (r == 0) dq = fma(cr.rhs0, st.r[r], dq);
-                    if (r == cr.rl) dq = fma(a.cw, st.r[r], dq);
-                    qbuf[(size_t)(k0 + r) * TC + c] = dq;
-                }
-            }
-            double xs = 0.0, g = 1.0, xq = 0.0;
-#pragma unroll
-            for (int r = MROWS - 1; r >= 0; --r) {
-                const double cp = scz[k0 + r] * st.r[r];
-                xs = st.d[r] - cp * xs;
-                st.d[r] = xs;
-                g *= -cp;
-                if (CYC) {
-                    xq = qbuf[(size_t)(k0 + r) * TC + c] - cp * xq;
-                    qbuf[(size_t)(k0 + r) * TC + c] = xq;
-                }
+            double xs, g, xq;
+            double* qcol = qbuf + (size_t)k0 * TC + c;      // this thread's rows of q: qcol[r * TC]
+            if (!CYC) {
+                phase2b_rows<false, false>(a, saz, scz, st, k0, CyclicRows(), qcol, xs, g, xq);
+            } else {
+                const CyclicRows cr = cyclic_rows(a, sm[nzp], lam, s);
+                if (cr.rl < 0) phase2b_rows<true, false>(a, saz, scz, st, k0, cr, qcol, xs, g, xq);
+                else phase2b_rows<true, true>(a, saz, scz, st, k0, cr, qcol, xs, g, xq);
             }
             s_scan[s * TC + c] = make_double2(xs, g);     // x^0 at the top row of the segment, its factor
             if (CYC) s_scanq[s * TC + c] = xq;
@@ -283,11 +309,17 @@ struct ZPass {
                 g *= -(scz[k0 + r] * st.r[r]);
                 st.d[r] += g * X;
             }
+            double* out = a.p + (size_t)k0 * plane + st.col;
+            if (k0 + MROWS <= a.nz_solve) {                 // whole segment inside the system (warp-uniform)
 #pragma unroll
-            for (int r = 0; r < MROWS; ++r) {
-                const int k = k0 + r;
-                // (the tile buffer still holds this tile: its buffer is not refilled before the next iteration)
-                if (k < a.nz) a.p[(size_t)k * plane + st.col] = (k < a.nz_solve) ? st.d[r] : buf[(size_t)k * TC + c] * a.scale;
+                for (int r = 0; r < MROWS; ++r) out[(size_t)r * plane] = st.d[r];
+            } else {
+#pragma unroll
+                for (int r = 0; r < MROWS; ++r) {
+                    const int k = k0 + r;
+                    // (the tile buffer still holds this tile: its buffer is not refilled before the next iteration)
+                    if (k < a.nz) out[(size_t)r * plane] = (k < a.nz_solve) ? st.d[r] : buf[(size_t)k * TC + c] * a.scale;
+                }
             }
         }
     }
@@ -326,7 +358,7 @@ struct ZPass {
     }
     // ... second half (behind a barrier): x = y - q (y_0 + v y_n) / (1 + q_0 + v q_n), v = a_0 / gamma, with the
     // propagation of both backward sweeps folded into one term
-    static CANS_HD void cyclic_store(const ZArgs& a, double* sm, const ZState<MROWS>& st, double lam, int tid, const double* qbuf) {
+    static CANS_HD void cyclic_store(const ZArgs& a, double* sm, ZState<MROWS>& st, double lam, int tid, const double* qbuf) {
         if (!st.active) return;
         const double* edge = sm + edge_offset(a.nseg);
         const int nzp = a.nseg * MROWS;
@@ -336,14 +368,21 @@ struct ZPass {
         const double v = a.a0w / -(sm[nzp] + lam);                     // sm[nzp] = bz[0]
         const double fact = (edge[4 * c] + v * edge[4 * c + 2]) / (1.0 + edge[4 * c + 1] + v * edge[4 * c + 3]);
         const double Xc = st.start - st.startq * fact;
-        const size_t plane = (size_t)a.ncols;
+        const double* qcol = qbuf + (size_t)k0 * TC + c;
         double g = 1.0;
 #pragma unroll
         for (int r = MROWS - 1; r >= 0; --r) {
-            const int k = k0 + r;
-            g *= -(scz[k] * st.r[r]);
-            const double x = (st.d[r] - qbuf[(size_t)k * TC + c] * fact) + g * Xc;
-            if (k < a.nz) a.p[(size_t)k * plane + st.col] = x;
+            g *= -(scz[k0 + r] * st.r[r]);
+            st.d[r] = (st.d[r] - qcol[r * TC] * fact) + g * Xc;
+        }
+        const size_t plane = (size_t)a.ncols;
+        double* out = a.p + (size_t)k0 * plane + st.col;
+        if (k0 + MROWS <= a.nz) {                           // whole segment inside the field (warp-uniform)
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) out[(size_t)r * plane] = st.d[r];
+        } else {
+#pragma unroll
+            for (int r = 0; r < MROWS; ++r) if (k0 + r < a.nz) out[(size_t)r * plane] = st.d[r];
         }
     }
 };

@@ -61,10 +61,11 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
         const long col = tile * TC + c;
         rs = 0.0; l1 = 0.0; l2 = 0.0;
         if (tile < a.ntiles && col < a.ncols) {
-            const int ci = (int)col;                  // ncols = nx*ny <= 2048^2 fits an int
+            const unsigned ci = (unsigned)col;        // ncols = nx*ny <= 2048^2 fits 32 bits
             rs = __ldcs(a.rstart + (size_t)s * a.ncols + col);
-            l1 = a.lamx[ci % a.nx];
-            l2 = a.lamy[ci / a.nx];
+            const unsigned j = (unsigned)(((unsigned long long)ci * a.nx_magic) >> 40);     // ci / nx without the division
+            l1 = a.lamx[ci - j * (unsigned)a.nx];
+            l2 = a.lamy[j];
         }
     };
     double rs, l1, l2;
@@ -170,6 +171,7 @@ cudaError_t z_solve_launch(const ZArgs& a_in, int grid, size_t smem, const CUten
     if (g > a.ntiles) g = a.ntiles;
     if (g < 1) g = 1;
     z_boxes(a.nseg, &a.nbox, &a.box_rows);
+    a.nx_magic = ((1ull << 40) + (unsigned long long)a.nx - 1) / (unsigned long long)a.nx;
     const int tc = z_tc_for(a.nseg);
 #define CANS_Z_LAUNCH(TC, CYC) z_solve_kernel<Z_MROWS, TC, CYC><<<(unsigned)g, TC * a.nseg, smem, st>>>(a, *tmap)
     if (a.cyclic) { if (tc == 32) CANS_Z_LAUNCH(32, true); else if (tc == 16) CANS_Z_LAUNCH(16, true); else CANS_Z_LAUNCH(8, true); }
