@@ -101,7 +101,7 @@ struct ZState {
     bool active;
 };
 
-// shared memory (doubles): tables az,bz,cz,gz [4][nzp]; (end, factor) pairs of the forward sweep [TC*P] and a second
+// shared memory (doubles): tables az [nzp], (bz, gz) pairs [2 nzp], cz [nzp]; (end, factor) pairs of the forward sweep [TC*P] and a second
 // array for the backward sweep (so that no barrier is needed between reading one and writing the other); the same two
 // arrays of segment ends for q [TC*P] each; (y_0, q_0, y_{nz-1}, q_{nz-1}) per column of a cyclic solve [4*TC]; two tile
 // buffers [nzp][TC]
@@ -117,11 +117,12 @@ struct ZPass {
 
     static CANS_HD void load_tables(const ZArgs& a, double* sm, int tid, int nthreads) {
         const int nzp = a.nseg * MROWS;
+        // az [nzp] | (bz, gz) pairs [nzp] (phase 1 reads both with one 16-byte load) | cz [nzp]
         for (int i = tid; i < nzp; i += nthreads) {
             sm[i] = a.az[i];
-            sm[nzp + i] = a.bz[i];
-            sm[2 * nzp + i] = a.cz[i];
-            sm[3 * nzp + i] = a.gz[i];
+            sm[nzp + 2 * i] = a.bz[i];
+            sm[nzp + 2 * i + 1] = a.gz[i];
+            sm[3 * nzp + i] = a.cz[i];
         }
     }
 
@@ -142,7 +143,7 @@ struct ZPass {
 
     // the rows of phase 1 (CYC: cyclic system; LAST: this thread's segment holds row nz-1, at local row cr.rl)
     template <bool CYC, bool LAST>
-    static CANS_HD void phase1_rows(const ZArgs& a, const double* saz, const double* sbz, const double* sgz, ZState<MROWS>& st,
+    static CANS_HD void phase1_rows(const ZArgs& a, const double* saz, const double2* sbg, ZState<MROWS>& st,
                                     int k0, double rstart_val, double lam, const CyclicRows& cr, double& dp_out, double& fac_out,
                                     double& dq_out) {
         double rp = rstart_val;
@@ -150,10 +151,11 @@ struct ZPass {
 #pragma unroll
         for (int r = 0; r < MROWS; ++r) {
             const int k = k0 + r;
-            double bl = sbz[k] + lam;
+            const double2 bg = sbg[k];
+            double bl = bg.x + lam;
             if (CYC && r == 0) bl += cr.diag0;
             if (LAST && r == cr.rl) bl += cr.diagn;
-            rp = z_pivot_bl(bl, sgz[k], rp);
+            rp = z_pivot_bl(bl, bg.y, rp);
             st.r[r] = rp;
             const double e = saz[k] * rp;
             dp = st.d[r] * rp - e * dp;
@@ -208,8 +210,7 @@ struct ZPass {
                                double rstart_val, double lam, int tid) {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
-        const double* sbz = sm + nzp;
-        const double* sgz = sm + 3 * nzp;
+        const double2* sbg = reinterpret_cast<const double2*>(sm + nzp);
         double2* s_scan = reinterpret_cast<double2*>(sm + scan_offset(a.nseg));      // forward (end, factor) pairs
         double* s_scanq = sm + scanq_offset(a.nseg);
         const int c = tid % TC;
@@ -224,13 +225,13 @@ struct ZPass {
             for (int r = 0; r < MROWS; ++r) st.d[r] = buf[(size_t)(k0 + r) * TC + c] * a.scale;
             double dp, fac, dq;
             if (!CYC) {
-                phase1_rows<false, false>(a, saz, sbz, sgz, st, k0, rstart_val, lam, CyclicRows(), dp, fac, dq);
+                phase1_rows<false, false>(a, saz, sbg, st, k0, rstart_val, lam, CyclicRows(), dp, fac, dq);
             } else {
                 // cyclic system: only rows 0 and nz-1 differ from the open one -- row 0 belongs to segment 0 (r = 0 at
                 // compile time), row nz-1 to local row rl of the last segment: its threads run their own copy of the loop
-                const CyclicRows cr = cyclic_rows(a, sbz[0], lam, s);
-                if (cr.rl < 0) phase1_rows<true, false>(a, saz, sbz, sgz, st, k0, rstart_val, lam, cr, dp, fac, dq);
-                else phase1_rows<true, true>(a, saz, sbz, sgz, st, k0, rstart_val, lam, cr, dp, fac, dq);
+                const CyclicRows cr = cyclic_rows(a, sbg[0].x, lam, s);
+                if (cr.rl < 0) phase1_rows<true, false>(a, saz, sbg, st, k0, rstart_val, lam, cr, dp, fac, dq);
+                else phase1_rows<true, true>(a, saz, sbg, st, k0, rstart_val, lam, cr, dp, fac, dq);
             }
             s_scan[s * TC + c] = make_double2(dp, fac);
             if (CYC) s_scanq[s * TC + c] = dq;
@@ -263,7 +264,7 @@ struct ZPass {
     static CANS_HD void phase2b(const ZArgs& a, double* sm, ZState<MROWS>& st, double lam, int tid, double* qbuf) {
         const int nzp = a.nseg * MROWS;
         const double* saz = sm;
-        const double* scz = sm + 2 * nzp;
+        const double* scz = sm + 3 * nzp;
         double2* s_scan = reinterpret_cast<double2*>(sm + scan_offset(a.nseg)) + TC * a.nseg;   // backward pairs
         double* s_scanq = sm + scanq_offset(a.nseg) + TC * a.nseg;
         const int c = tid % TC;
@@ -290,7 +291,7 @@ struct ZPass {
     // phase 3 of the open system: scan from the bottom -> true x below the segment; propagate; store to the field
     static CANS_HD void phase3(const ZArgs& a, double* sm, ZState<MROWS>& st, int tid, const double* buf) {
         const int nzp = a.nseg * MROWS;
-        const double* scz = sm + 2 * nzp;
+        const double* scz = sm + 3 * nzp;
         const double2* s_scan = reinterpret_cast<const double2*>(sm + scan_offset(a.nseg)) + TC * a.nseg;   // backward pairs
         const int c = tid % TC;
         const int s = tid / TC;
@@ -362,7 +363,7 @@ struct ZPass {
         if (!st.active) return;
         const double* edge = sm + edge_offset(a.nseg);
         const int nzp = a.nseg * MROWS;
-        const double* scz = sm + 2 * nzp;
+        const double* scz = sm + 3 * nzp;
         const int c = tid % TC;
         const int k0 = (tid / TC) * MROWS;
         const double v = a.a0w / -(sm[nzp] + lam);                     // sm[nzp] = bz[0]
