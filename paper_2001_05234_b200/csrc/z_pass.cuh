@@ -97,6 +97,8 @@ struct ZState {
     double r[MROWS];
     double start;     // true d'_{k0-1}, later true x_{k0+MROWS}
     double startq;    // the same for the correction vector q of a cyclic system
+    double exe, exf, exq;   // composition of the warp's earlier (forward) / later (backward) segments of this column:
+                            // value -> exe + exf * value (exq: the end term of q), see group_scan
     long col;
     bool active;
 };
@@ -124,6 +126,45 @@ struct ZPass {
             sm[nzp + 2 * i + 1] = a.gz[i];
             sm[3 * nzp + i] = a.cz[i];
         }
+    }
+
+    // Segment scans.  The true start of a segment is the composition of the affine maps x -> end + factor * x of all the
+    // segments before it (forward sweep) or above it (backward sweep).  A warp holds G = 32 / TC consecutive segments of
+    // its columns (lanes c + TC * sg): it composes those by shuffles, publishes ONE aggregate per group and keeps each
+    // lane's in-group prefix in registers, so the serial scan behind the barrier walks groups, not segments -- half
+    // (TC = 16) or a quarter (TC = 8) of the 16-byte shared-memory reads and of the dependent steps.
+    static constexpr int G = 32 / TC;
+    // does the warp of segment s hold the segment of row nz-1 ?  (warp-uniform)
+    static CANS_HD bool last_group(const ZArgs& a, int s) { return s / G == ((a.nz - 1) / MROWS) / G; }
+    static CANS_HD int ngroups(int nseg) { return (nseg + G - 1) / G; }
+    // DOWN = false: compose with the earlier segments (lanes below); true: with the later ones (lanes above).
+    // In: this segment's (e, f, q).  Out: (e, f, q) = aggregate of the group as seen from its last (first) lane;
+    // (xe, xf, xq) = composition of the in-group segments before (after) this lane, identity if none.
+    template <bool CYC, bool DOWN>
+    static CANS_HD void group_scan(int tid, int s, int nseg, double& e, double& f, double& q, double& xe, double& xf, double& xq) {
+        xe = 0.0; xf = 1.0; xq = 0.0;
+        if (G == 1) return;
+#if defined(__CUDA_ARCH__)
+        // the lanes of this warp that exist (the last warp of a CTA of TC * nseg threads may be partial)
+        const int left = TC * nseg - (tid & ~31);
+        const unsigned mask = left >= 32 ? 0xffffffffu : ((1u << left) - 1u);
+        const int sg = s % G;
+#pragma unroll
+        for (int off = 1; off < G; off <<= 1) {
+            const double e2 = DOWN ? __shfl_down_sync(mask, e, off * TC) : __shfl_up_sync(mask, e, off * TC);
+            const double f2 = DOWN ? __shfl_down_sync(mask, f, off * TC) : __shfl_up_sync(mask, f, off * TC);
+            double q2 = 0.0;
+            if (CYC) q2 = DOWN ? __shfl_down_sync(mask, q, off * TC) : __shfl_up_sync(mask, q, off * TC);
+            const bool has = DOWN ? (sg + off < G && s + off < nseg) : (sg >= off);
+            if (has) { e = e + f * e2; if (CYC) q = q + f * q2; f = f * f2; }
+        }
+        const double e1 = DOWN ? __shfl_down_sync(mask, e, TC) : __shfl_up_sync(mask, e, TC);
+        const double f1 = DOWN ? __shfl_down_sync(mask, f, TC) : __shfl_up_sync(mask, f, TC);
+        double q1 = 0.0;
+        if (CYC) q1 = DOWN ? __shfl_down_sync(mask, q, TC) : __shfl_up_sync(mask, q, TC);
+        const bool has1 = DOWN ? (sg + 1 < G && s + 1 < nseg) : (sg >= 1);
+        if (has1) { xe = e1; xf = f1; xq = q1; }
+#endif
     }
 
     // The two rows in which the open matrix T' and the right-hand side u of the correction system differ from the plain
@@ -219,25 +260,28 @@ struct ZPass {
         st.col = col;
         st.active = (col < a.ncols) && !(a.singular && col == 0);
         const int k0 = s * MROWS;
+        double dp = 0.0, fac = 0.0, dq = 0.0;
         if (col < a.ncols) {
             // (rows nz..nzp-1 of the buffer lie outside the tensor: the TMA unit filled them with zeros)
 #pragma unroll
             for (int r = 0; r < MROWS; ++r) st.d[r] = buf[(size_t)(k0 + r) * TC + c] * a.scale;
-            double dp, fac, dq;
             if (!CYC) {
                 phase1_rows<false, false>(a, saz, sbg, st, k0, rstart_val, lam, CyclicRows(), dp, fac, dq);
             } else {
                 // cyclic system: only rows 0 and nz-1 differ from the open one -- row 0 belongs to segment 0 (r = 0 at
                 // compile time), row nz-1 to local row rl of the last segment: its threads run their own copy of the loop
                 const CyclicRows cr = cyclic_rows(a, sbg[0].x, lam, s);
-                if (cr.rl < 0) phase1_rows<true, false>(a, saz, sbg, st, k0, rstart_val, lam, cr, dp, fac, dq);
+                // (the choice is made per warp -- the warp holding the last segment runs the general copy in all its lanes,
+                // rl = -1 matching no row -- so that no warp executes both copies)
+                if (!last_group(a, s)) phase1_rows<true, false>(a, saz, sbg, st, k0, rstart_val, lam, cr, dp, fac, dq);
                 else phase1_rows<true, true>(a, saz, sbg, st, k0, rstart_val, lam, cr, dp, fac, dq);
             }
-            s_scan[s * TC + c] = make_double2(dp, fac);
-            if (CYC) s_scanq[s * TC + c] = dq;
-        } else {
-            s_scan[s * TC + c] = make_double2(0.0, 0.0);
-            if (CYC) s_scanq[s * TC + c] = 0.0;
+        }
+        // compose the warp's segments; the last lane of each group publishes its aggregate
+        group_scan<CYC, false>(tid, s, a.nseg, dp, fac, dq, st.exe, st.exf, st.exq);
+        if (s % G == G - 1 || s == a.nseg - 1) {
+            s_scan[(s / G) * TC + c] = make_double2(dp, fac);
+            if (CYC) s_scanq[(s / G) * TC + c] = dq;
         }
     }
 
@@ -248,15 +292,16 @@ struct ZPass {
         const double* s_scanq = sm + scanq_offset(a.nseg);
         const int c = tid % TC;
         const int s = tid / TC;
-        double D = 0.0, Dq = 0.0;           // true d' (and q's) at the end of segment s'-1
+        double D = 0.0, Dq = 0.0;           // true d' (and q's) at the end of the previous group ...
+        const int grp = s / G;
 #pragma unroll 4
-        for (int q = 0; q < s; ++q) {
-            const double2 ef = s_scan[q * TC + c];      // one 16-byte load per segment
-            D = ef.x + ef.y * D;
+        for (int q = 0; q < grp; ++q) {
+            const double2 ef = s_scan[q * TC + c];      // one 16-byte load per group
             if (CYC) Dq = s_scanq[q * TC + c] + ef.y * Dq;
+            D = ef.x + ef.y * D;
         }
-        st.start = D;
-        st.startq = Dq;
+        st.start = st.exe + st.exf * D;     // ... carried through the warp's earlier segments of this group
+        st.startq = st.exq + st.exf * Dq;
     }
     // (2b publishes into the backward arrays, so 2a and 2b need no barrier between them).  Cyclic: q's true forward values
     // are rebuilt row by row from its true start and parked in qbuf, then swept backwards in place.
@@ -270,21 +315,23 @@ struct ZPass {
         const int c = tid % TC;
         const int s = tid / TC;
         const int k0 = s * MROWS;
+        double xs = 0.0, g = 0.0, xq = 0.0;
         if (st.col < a.ncols) {
-            double xs, g, xq;
             double* qcol = qbuf + (size_t)k0 * TC + c;      // this thread's rows of q: qcol[r * TC]
             if (!CYC) {
                 phase2b_rows<false, false>(a, saz, scz, st, k0, CyclicRows(), qcol, xs, g, xq);
             } else {
                 const CyclicRows cr = cyclic_rows(a, sm[nzp], lam, s);
-                if (cr.rl < 0) phase2b_rows<true, false>(a, saz, scz, st, k0, cr, qcol, xs, g, xq);
+                if (!last_group(a, s)) phase2b_rows<true, false>(a, saz, scz, st, k0, cr, qcol, xs, g, xq);
                 else phase2b_rows<true, true>(a, saz, scz, st, k0, cr, qcol, xs, g, xq);
             }
-            s_scan[s * TC + c] = make_double2(xs, g);     // x^0 at the top row of the segment, its factor
-            if (CYC) s_scanq[s * TC + c] = xq;
-        } else {
-            s_scan[s * TC + c] = make_double2(0.0, 0.0);
-            if (CYC) s_scanq[s * TC + c] = 0.0;
+        }
+        // (xs, g): x^0 at the top row of the segment and its factor; compose the warp's segments from the top down, the
+        // first lane of each group publishes its aggregate
+        group_scan<CYC, true>(tid, s, a.nseg, xs, g, xq, st.exe, st.exf, st.exq);
+        if (s % G == 0) {
+            s_scan[(s / G) * TC + c] = make_double2(xs, g);
+            if (CYC) s_scanq[(s / G) * TC + c] = xq;
         }
     }
 
@@ -296,12 +343,13 @@ struct ZPass {
         const int c = tid % TC;
         const int s = tid / TC;
         const int k0 = s * MROWS;
-        double X = 0.0;                     // true x at the top row of segment s'+1
+        double X = 0.0;                     // true x at the top row of the next group ...
 #pragma unroll 4
-        for (int q = a.nseg - 1; q > s; --q) {
+        for (int q = ngroups(a.nseg) - 1; q > s / G; --q) {
             const double2 ef = s_scan[q * TC + c];
             X = ef.x + ef.y * X;
         }
+        X = st.exe + st.exf * X;            // ... carried down through the warp's later segments of this group
         if (st.active) {
             const size_t plane = (size_t)a.ncols;
             double g = 1.0;
@@ -335,16 +383,21 @@ struct ZPass {
         const int s = tid / TC;
         double X = 0.0, Xq = 0.0;
 #pragma unroll 4
-        for (int q = a.nseg - 1; q > s; --q) {
+        for (int q = ngroups(a.nseg) - 1; q > s / G; --q) {
             const double2 ef = s_scan[q * TC + c];
-            X = ef.x + ef.y * X;
             Xq = s_scanq[q * TC + c] + ef.y * Xq;
+            X = ef.x + ef.y * X;
         }
+        Xq = st.exq + st.exf * Xq;
+        X = st.exe + st.exf * X;
         st.start = X;
         st.startq = Xq;
         if (st.col < a.ncols) {
             if (s == 0) {                                   // row 0: local value + (factor of the whole segment) * X
-                const double g = s_scan[c].y;
+                const double* scz0 = sm + 3 * a.nseg * MROWS;
+                double g = 1.0;
+#pragma unroll
+                for (int r = 0; r < MROWS; ++r) g *= -(scz0[r] * st.r[r]);
                 edge[4 * c] = st.d[0] + g * X;
                 edge[4 * c + 1] = qbuf[c] + g * Xq;
             }
