@@ -714,6 +714,7 @@ int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* m
     if (rc) return rc;
     TileCopyShape sh;
     const CUtensorMap* tmap;
+    CUtensorMap tmap_wide;
     if (which == 0) {            // z solve: tiles of z_tc_for(nseg) columns x nz rows of the (nz, nx*ny) view
         const int tc = z_tc_for(plan->nseg);
         int d = 256 / Z_MROWS;
@@ -726,8 +727,16 @@ int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* m
         sh.m0 = plan->nx / 2 / YT_COLS; sh.ntiles = sh.m0 * plan->nz; sh.s0 = 2 * YT_COLS; sh.s1 = plan->ny;
         sh.box_rows = YT_BOX_ROWS; sh.nbox = plan->ny / YT_BOX_ROWS; sh.box_cols = 2 * YT_COLS;
         tmap = &plan->tmap_y;
+    } else if (which == 2) {     // the z view again, row segments twice as wide: tiles of 32 columns x 256 rows (two per column tile)
+        const long ncols = (long)plan->nx * plan->ny;
+        cudaError_t te = make_tensor_map_2d(&tmap_wide, p, (unsigned long long)ncols, (unsigned long long)plan->nz,
+                                            (unsigned long long)ncols * sizeof(double), 32, 256, CU_TENSOR_MAP_SWIZZLE_NONE);
+        if (te != cudaSuccess) return fail_cuda(te, "tensor map encode");
+        sh.m0 = (ncols + 31) / 32; sh.ntiles = sh.m0 * ((plan->nz + 255) / 256); sh.s0 = 32; sh.s1 = 256;
+        sh.box_rows = 256; sh.nbox = 1; sh.box_cols = 32;
+        tmap = &tmap_wide;
     } else {
-        return fail(CANS_ERR_INVALID_ARG, "which must be 0 (z tiles) or 1 (y tiles)");
+        return fail(CANS_ERR_INVALID_ARG, "which must be 0 (z tiles), 1 (y tiles) or 2 (z view, 32-column tiles)");
     }
     cudaError_t e = probe_tile_copy(tmap, sh, plan->num_sms, ms, (cudaStream_t)stream);
     if (e != cudaSuccess) return fail_cuda(e, "tile copy probe");
