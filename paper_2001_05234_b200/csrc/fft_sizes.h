@@ -22,7 +22,7 @@
     X(1024, 16, 8, 8, 4, 256, 4, 256)
 
 #define CANS_FFT_SIZES_D(X) \
-    X(1536, 12, 8, 16, 2, 64, 4, 128)  \
+    X(1536, 12, 8, 16, 2, 384, 4, 256)  \
     X(2048, 16, 8, 16, 2, 256, 4, 256)
 
 #define CANS_FFT_SIZES(X) CANS_FFT_SIZES_A(X) CANS_FFT_SIZES_B(X) CANS_FFT_SIZES_C(X) CANS_FFT_SIZES_D(X)

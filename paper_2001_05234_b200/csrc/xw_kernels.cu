@@ -23,10 +23,11 @@ __global__ void __launch_bounds__(XW_WARPS * 32, 2) xw_kernel(const XYArgs a, co
 
 template <int N, int R1, int KC>
 static cudaError_t xw_launch_k(int op, const XYArgs& a, const cplx* tw, cudaStream_t st) {
-    // at least 80 KB per CTA: two CTAs (8 warps) per SM whatever the register count -- the lean periodic kernels would fit
-    // three, which measured slower (1.25 against 1.00 ms for the x inverse of the 1024 x 768 x 512 grid)
+    // N = 1024: at least 80 KB per CTA, i.e. two CTAs (8 warps) per SM whatever the register count -- the lean periodic
+    // kernels would fit three, which measured slower there (1.25 against 1.00 ms for the x inverse of the 1024 x 768 x 512
+    // grid); the shorter lines do run faster with three (512: 0.17 against 0.20 ms on 512 x 512 x 256)
     size_t smem = sizeof(cplx) * (size_t)XW_WARPS * XWPass<N, R1>::BUF;
-    if (smem < 80 * 1024) smem = 80 * 1024;
+    if (N >= 1024 && smem < 80 * 1024) smem = 80 * 1024;
     if (op == OP_CONFIGURE) {
         cudaError_t e = cudaFuncSetAttribute(xw_kernel<N, R1, 0, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(xw_kernel<N, R1, 1, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
