@@ -8,13 +8,13 @@
     X(32, 4, 1, 8, 16, 64, 8, 32)    \
     X(48, 6, 1, 8, 16, 32, 8, 32)    \
     X(64, 8, 1, 8, 16, 128, 8, 64)   \
-    X(96, 12, 1, 8, 16, 64, 8, 32)   \
-    X(128, 16, 1, 8, 16, 128, 8, 64)
+    X(96, 12, 1, 8, 16, 128, 8, 64)   \
+    X(128, 16, 1, 8, 16, 128, 8, 128)
 
 #define CANS_FFT_SIZES_B(X) \
-    X(192, 12, 1, 16, 16, 64, 8, 64)   \
+    X(192, 12, 1, 16, 16, 128, 8, 128)   \
     X(256, 16, 1, 16, 16, 256, 8, 128) \
-    X(384, 6, 8, 8, 8, 128, 8, 128)    \
+    X(384, 6, 8, 8, 8, 256, 8, 256)    \
     X(512, 8, 8, 8, 8, 256, 8, 256)
 
 #define CANS_FFT_SIZES_C(X) \

@@ -21,7 +21,7 @@
 //     accumulating the propagation factor (prod of -a_k r_k, resp. -c_k r_k); a P-step scan over the
 //     segment ends in shared memory supplies the true start value, which is then propagated;
 //   * results go straight from registers to global memory (coalesced rows).
-// The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_column
+// The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_stage / _sweeps / _store
 // (CTA 0, before it joins the tile loop).
 //
 // Periodic z (the triperiodic Taylor-Green case of P:L222): the system is cyclic, row 0 couples to
@@ -462,26 +462,43 @@ CANS_HD void z_setup_column(const ZArgs& a, double* rstart_out, double* r00_out,
     }
 }
 
-// The singular column (reading S3 / oracle O4): forward sweep on rows 0..nz-2, x[nz-1] = 0,
-// back-substitute, subtract the dzf-weighted mean.  One thread; d is staged in shared memory.
-CANS_HD void z_singular_column(const ZArgs& a, double* sd /* nz doubles */) {
-    const size_t plane = (size_t)a.ncols;
-    const int nz = a.nz;
-    double dp = 0.0;
-    for (int k = 0; k < nz - 1; ++k) {
+// The singular column (reading S3 / oracle O4): forward sweep on rows 0..nz-2, x[nz-1] = 0, back-substitute, subtract the
+// dzf-weighted mean.  The CTA stages t_k = d_k r_k, e_k = a_k r_k, cp_k = c_k r_k and dzf in shared memory in parallel
+// (z_singular_stage), ONE thread runs the two recurrences -- one dependent FMA per row -- and leaves the mean in sd[nz]
+// (z_singular_sweeps), and the CTA writes the column back (z_singular_store).  sd: 4 * nzp + 1 doubles.
+CANS_HD void z_singular_stage(const ZArgs& a, double* sd, int nzp, int tid, int nthreads) {
+    for (int k = tid; k < a.nz; k += nthreads) {
         const double rk = a.r00[k];
-        dp = (sd[k] * a.scale - a.az[k] * dp) * rk;
+        sd[k] = a.p[(size_t)k * a.ncols] * a.scale * rk;
+        sd[nzp + k] = a.az[k] * rk;
+        sd[2 * nzp + k] = a.cz[k] * rk;
+        sd[3 * nzp + k] = a.dzf[k];
+    }
+}
+CANS_HD void z_singular_sweeps(const ZArgs& a, double* sd, int nzp) {
+    const int nz = a.nz;
+    const double* se = sd + nzp;
+    const double* scp = sd + 2 * nzp;
+    const double* sw = sd + 3 * nzp;
+    double dp = 0.0;
+#pragma unroll 8
+    for (int k = 0; k < nz - 1; ++k) {
+        dp = sd[k] - se[k] * dp;
         sd[k] = dp;
     }
     double x = 0.0, acc = 0.0;
     sd[nz - 1] = 0.0;
+#pragma unroll 8
     for (int k = nz - 2; k >= 0; --k) {
-        x = sd[k] - a.cz[k] * a.r00[k] * x;
+        x = sd[k] - scp[k] * x;
         sd[k] = x;
-        acc += x * a.dzf[k];
+        acc += x * sw[k];
     }
-    const double mean = acc * a.inv_lz;
-    for (int k = 0; k < nz; ++k) a.p[(size_t)k * plane] = sd[k] - mean;
+    sd[4 * nzp] = acc * a.inv_lz;
+}
+CANS_HD void z_singular_store(const ZArgs& a, const double* sd, int nzp, int tid, int nthreads) {
+    const double mean = sd[4 * nzp];
+    for (int k = tid; k < a.nz; k += nthreads) a.p[(size_t)k * a.ncols] = sd[k] - mean;
 }
 
 }  // namespace cans

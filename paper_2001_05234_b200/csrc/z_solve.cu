@@ -18,10 +18,13 @@ __global__ void __launch_bounds__(512) z_solve_kernel(const ZArgs a, const __gri
     const size_t tile_sz = Z::tile_doubles(a.nseg);
 
     if (a.singular && blockIdx.x == 0) {
-        // the singular (0,0) column, staged in shared memory, solved by one thread (reading S3)
-        for (int k = tid; k < a.nz; k += nthreads) bufs[k] = a.p[(size_t)k * a.ncols];
+        // the singular (0,0) column (reading S3): staged by the CTA, swept by one thread, written back by the CTA
+        const int nzp = a.nseg * MROWS;
+        z_singular_stage(a, bufs, nzp, tid, nthreads);
         __syncthreads();
-        if (tid == 0) z_singular_column(a, bufs);
+        if (tid == 0) z_singular_sweeps(a, bufs, nzp);
+        __syncthreads();
+        z_singular_store(a, bufs, nzp, tid, nthreads);
         __syncthreads();
     }
     Z::load_tables(a, zsm, tid, nthreads);
