@@ -95,9 +95,63 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
 }
 
 // chkdt (Listing 1): see chkdt_pass.cuh.  One thread per pair of x-adjacent cells, marching up CHK_KC planes.
+// Everything that depends on the boundary rule but not on k -- which row a neighbour row is (inside, wrapped, a lower-face
+// plane, or absent = 0), where the value beyond the thread's pair comes from at a row end or a warp edge -- is resolved
+// ONCE per thread into pointers and strides (ChkStream); the plane loop then only advances pointers.  The step whose k+1
+// plane lies beyond the top of the field is peeled off (it runs the general loaders of chkdt_pass.cuh).
 constexpr int CHK_KC = 32;
 
-__global__ void __launch_bounds__(256, 3) chkdt_kernel(const ChkArgs a) {
+struct ChkStream {
+    const double* p;        // the thread's pair (x0, x0 + 1) of the row at the current plane, or NULL: the row reads as 0
+    const double* e;        // the value beyond the pair where the neighbouring lane cannot supply it, or NULL (0 / not needed)
+};                          // (strides per plane: the field's plane, except for lower-face planes -- kept by the caller)
+// u-type rows need u(i-1): from lane - 1, except at lane 0 / i = 0
+__device__ __forceinline__ ChkStream chk_stream_u(const ChkArgs& a, int i, int jj, int kk, int lane) {
+    ChkStream s = {nullptr, nullptr};
+    if (jj >= a.ny) { if (!a.wrap_y) return s; jj = 0; }
+    const double* row = a.u + ((size_t)kk * a.ny + jj) * a.nx;
+    s.p = row + i;
+    if (i > 0) { if (lane == 0) s.e = row + i - 1; }
+    else if (a.wrap_x) s.e = row + a.nx - 1;
+    else if (a.fx) s.e = a.fx + (size_t)kk * a.ny + jj;       // (stride ny per plane: ChkArgs-dependent, see ue_stride)
+    return s;
+}
+// v / w-type rows need the value at i+2: from lane + 1, except at lane 31 / the row end
+__device__ __forceinline__ ChkStream chk_stream_row(const double* row, int i, int nx, int wrap_x, int lane) {
+    ChkStream s = {nullptr, nullptr};
+    if (!row) return s;
+    s.p = row + i;
+    if (i + 2 < nx) { if (lane == 31) s.e = row + i + 2; }
+    else if (wrap_x) s.e = row;
+    return s;
+}
+__device__ __forceinline__ RowLoad chk_fetch(const ChkStream& s) {
+    RowLoad r;
+    r.t = s.p ? *reinterpret_cast<const double2*>(s.p) : make_double2(0.0, 0.0);
+    r.edge = s.e ? *s.e : 0.0;
+    return r;
+}
+__device__ __forceinline__ void chk_advance(ChkStream& s, long ps, long es) {
+    if (s.p) s.p += ps;
+    if (s.e) s.e += es;
+}
+
+__device__ __forceinline__ double chk_cell_max(const ChkArgs& a, int k, const Row3& uj, const Row3& up, const Row3& un, const Row3& vm,
+                                               const Row3& vj, const Row3& vmn, const Row3& vjn, const Row3& wlj, const Row3& wlp,
+                                               const Row3& wj, const Row3& wp) {
+    const double qx = 0.25 * a.rdx, qy = 0.25 * a.rdy;
+    const double rzf = a.rdzf[k], rzc = a.rdzc[k], qz = 0.25 * rzf;
+    // cell i (values .a / .b of the v, w rows; .b of the u rows) and cell i+1 (.b / .c; .c)
+    const double dtix0 = fabs(uj.b) * a.rdx + fabs(vj.a + vm.a + vj.b + vm.b) * qy + fabs(wj.a + wlj.a + wj.b + wlj.b) * qz;
+    const double dtix1 = fabs(uj.c) * a.rdx + fabs(vj.b + vm.b + vj.c + vm.c) * qy + fabs(wj.b + wlj.b + wj.c + wlj.c) * qz;
+    const double dtiy0 = fabs(uj.b + up.b + up.a + uj.a) * qx + fabs(vj.a) * a.rdy + fabs(wj.a + wp.a + wlp.a + wlj.a) * qz;
+    const double dtiy1 = fabs(uj.c + up.c + up.b + uj.b) * qx + fabs(vj.b) * a.rdy + fabs(wj.b + wp.b + wlp.b + wlj.b) * qz;
+    const double dtiz0 = fabs(uj.b + uj.a + un.a + un.b) * qx + fabs(vj.a + vm.a + vmn.a + vjn.a) * qy + fabs(wj.a) * rzc;
+    const double dtiz1 = fabs(uj.c + uj.b + un.b + un.c) * qx + fabs(vj.b + vm.b + vmn.b + vjn.b) * qy + fabs(wj.b) * rzc;
+    return fmax(fmax(dtix0, dtix1), fmax(fmax(dtiy0, dtiy1), fmax(dtiz0, dtiz1)));
+}
+
+__global__ void __launch_bounds__(256, 2) chkdt_kernel(const ChkArgs a) {
     const int hx = a.nx / 2;
     const size_t cols = (size_t)hx * a.ny;                 // a multiple of 32: a warp is valid as a whole
     const size_t c = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -108,7 +162,7 @@ __global__ void __launch_bounds__(256, 3) chkdt_kernel(const ChkArgs a) {
         const int j = (int)(c / hx);
         const int k0 = (int)blockIdx.y * CHK_KC;
         const int k1 = (k0 + CHK_KC < a.nz) ? k0 + CHK_KC : a.nz;
-        const double qx = 0.25 * a.rdx, qy = 0.25 * a.rdy;
+        const long plane = (long)a.nx * a.ny;
         // carried rows: u(i-1..i+1, j, k); v(i..i+2, j-1 and j, k); w(i..i+2, j, k-1); w(i, i+1; j+1, k-1)
         Row3 uj, vm, vj, wlj, wlp;
         {
@@ -119,24 +173,81 @@ __global__ void __launch_bounds__(256, 3) chkdt_kernel(const ChkArgs a) {
             vm = chk_right(l1, i, a.nx, lane); vj = chk_right(l2, i, a.nx, lane);
             wlj = chk_right(l3, i, a.nx, lane); wlp = chk_right(l4, i, a.nx, lane);
         }
-        for (int k = k0; k < k1; ++k) {
-            // all six rows of this step in flight before the first is consumed
-            const RowLoad lup = chk_load_u(a, i, j + 1, k, lane);        // u(i-1..i+1, j+1, k)
-            const RowLoad lun = chk_load_u(a, i, j, k + 1, lane);        // u(i-1..i+1, j,   k+1)
+        // the six rows fetched per step, positioned at the first step: u(j+1, k), u(j, k+1), v(j-1, k+1), v(j, k+1), w(j, k), w(j+1, k)
+        const int kfast = (k1 < a.nz) ? k1 : a.nz - 1;     // steps [k0, kfast) have their k+1 plane inside the field
+        // Fast path (warp-uniform): every neighbour row of this warp is a stored row (inside or wrapped) and every value
+        // beyond a lane's pair is a stored value -- one running offset and four per-thread deltas address everything.
+        const int i_first = i - 2 * lane;
+        const bool fast = (a.wrap_y || (j > 0 && j + 1 < a.ny)) && (a.wrap_x || (i_first > 0 && i_first + 64 < a.nx));
+        if (fast) {
+            const long d_up = (j + 1 < a.ny) ? (long)a.nx : -(long)(a.ny - 1) * a.nx;      // row j+1 (or row 0)
+            const long d_vm = (j > 0) ? -(long)a.nx : (long)(a.ny - 1) * a.nx;             // row j-1 (or row ny-1)
+            const long dl = (i > 0) ? -1 : (long)a.nx - 1;                                  // u(i-1), for lane 0
+            const long dr = (i + 2 < a.nx) ? 2 : 2 - (long)a.nx;                            // value at i+2, for lane 31
+            size_t o = ((size_t)k0 * a.ny + j) * a.nx + i;
+            const bool l0 = lane == 0, l31 = lane == 31;
+#pragma unroll 2                                    // (two steps per trip: the carried rows rotate by renaming, not by moves)
+            for (int k = k0; k < kfast; ++k, o += plane) {
+                RowLoad lup, lun, lvm, lvj, lwj, lwp;
+                lup.t = *reinterpret_cast<const double2*>(a.u + o + d_up);
+                lun.t = *reinterpret_cast<const double2*>(a.u + o + plane);
+                lvm.t = *reinterpret_cast<const double2*>(a.v + o + plane + d_vm);
+                lvj.t = *reinterpret_cast<const double2*>(a.v + o + plane);
+                lwj.t = *reinterpret_cast<const double2*>(a.w + o);
+                lwp.t = *reinterpret_cast<const double2*>(a.w + o + d_up);
+                lup.edge = lun.edge = lvm.edge = lvj.edge = lwj.edge = lwp.edge = 0.0;
+                if (l0) { lup.edge = a.u[o + d_up + dl]; lun.edge = a.u[o + plane + dl]; }
+                if (l31) {
+                    lvm.edge = a.v[o + plane + d_vm + dr]; lvj.edge = a.v[o + plane + dr];
+                    lwj.edge = a.w[o + dr]; lwp.edge = a.w[o + d_up + dr];
+                }
+                const Row3 up = chk_left(lup, 1, lane), un = chk_left(lun, 1, lane);          // (edge taken at lane 0 / 31 only)
+                const Row3 vmn = chk_right(lvm, 0, a.nx, lane), vjn = chk_right(lvj, 0, a.nx, lane);
+                const Row3 wj = chk_right(lwj, 0, a.nx, lane), wp = chk_right(lwp, 0, a.nx, lane);
+                m = fmax(m, chk_cell_max(a, k, uj, up, un, vm, vj, vmn, vjn, wlj, wlp, wj, wp));
+                uj = un; vm = vmn; vj = vjn; wlj = wj; wlp = wp;
+            }
+        } else {
+            ChkStream s_up, s_un, s_vmn, s_vjn, s_wj, s_wp;
+            long vstride = plane;                               // v(j-1) is the lower-face plane fy (stride nx) at j = 0 of a wall
+            const long ue_stride = (i == 0 && !a.wrap_x && a.fx) ? a.ny : plane;    // u(i-1) from the lower-face plane fx
+            if (k0 < kfast) {
+                s_up = chk_stream_u(a, i, j + 1, k0, lane);
+                s_un = chk_stream_u(a, i, j, k0 + 1, lane);
+                const double* vrow = nullptr;
+                if (j > 0) vrow = a.v + ((size_t)(k0 + 1) * a.ny + j - 1) * a.nx;
+                else if (a.wrap_y) vrow = a.v + ((size_t)(k0 + 1) * a.ny + a.ny - 1) * a.nx;
+                else if (a.fy) { vrow = a.fy + (size_t)(k0 + 1) * a.nx; vstride = a.nx; }
+                s_vmn = chk_stream_row(vrow, i, a.nx, a.wrap_x, lane);
+                s_vjn = chk_stream_row(a.v + ((size_t)(k0 + 1) * a.ny + j) * a.nx, i, a.nx, a.wrap_x, lane);
+                s_wj = chk_stream_row(a.w + ((size_t)k0 * a.ny + j) * a.nx, i, a.nx, a.wrap_x, lane);
+                const double* wrow = nullptr;
+                if (j + 1 < a.ny) wrow = a.w + ((size_t)k0 * a.ny + j + 1) * a.nx;
+                else if (a.wrap_y) wrow = a.w + (size_t)k0 * a.ny * a.nx;
+                s_wp = chk_stream_row(wrow, i, a.nx, a.wrap_x, lane);
+            }
+            for (int k = k0; k < kfast; ++k) {
+                // all six rows of this step in flight before the first is consumed
+                const RowLoad lup = chk_fetch(s_up), lun = chk_fetch(s_un), lvm = chk_fetch(s_vmn), lvj = chk_fetch(s_vjn);
+                const RowLoad lwj = chk_fetch(s_wj), lwp = chk_fetch(s_wp);
+                chk_advance(s_up, plane, ue_stride); chk_advance(s_un, plane, ue_stride); chk_advance(s_vmn, vstride, vstride);
+                chk_advance(s_vjn, plane, plane); chk_advance(s_wj, plane, plane); chk_advance(s_wp, plane, plane);
+                const Row3 up = chk_left(lup, i, lane), un = chk_left(lun, i, lane);
+                const Row3 vmn = chk_right(lvm, i, a.nx, lane), vjn = chk_right(lvj, i, a.nx, lane);
+                const Row3 wj = chk_right(lwj, i, a.nx, lane), wp = chk_right(lwp, i, a.nx, lane);
+                m = fmax(m, chk_cell_max(a, k, uj, up, un, vm, vj, vmn, vjn, wlj, wlp, wj, wp));
+                uj = un; vm = vmn; vj = vjn; wlj = wj; wlp = wp;
+            }
+        }
+        for (int k = kfast; k < k1; ++k) {                 // (at most) the top plane: its k+1 rows wrap or read as 0
+            const RowLoad lup = chk_load_u(a, i, j + 1, k, lane);
+            const RowLoad lun = chk_load_u(a, i, j, k + 1, lane);
             const RowLoad lvm = chk_load_v(a, i, j - 1, k + 1, lane), lvj = chk_load_v(a, i, j, k + 1, lane);
             const RowLoad lwj = chk_load_w(a, i, j, k, lane), lwp = chk_load_w(a, i, j + 1, k, lane);
             const Row3 up = chk_left(lup, i, lane), un = chk_left(lun, i, lane);
             const Row3 vmn = chk_right(lvm, i, a.nx, lane), vjn = chk_right(lvj, i, a.nx, lane);
             const Row3 wj = chk_right(lwj, i, a.nx, lane), wp = chk_right(lwp, i, a.nx, lane);
-            const double rzf = a.rdzf[k], rzc = a.rdzc[k], qz = 0.25 * rzf;
-            // cell i (values .a / .b of the v, w rows; .b of the u rows) and cell i+1 (.b / .c; .c)
-            const double dtix0 = fabs(uj.b) * a.rdx + fabs(vj.a + vm.a + vj.b + vm.b) * qy + fabs(wj.a + wlj.a + wj.b + wlj.b) * qz;
-            const double dtix1 = fabs(uj.c) * a.rdx + fabs(vj.b + vm.b + vj.c + vm.c) * qy + fabs(wj.b + wlj.b + wj.c + wlj.c) * qz;
-            const double dtiy0 = fabs(uj.b + up.b + up.a + uj.a) * qx + fabs(vj.a) * a.rdy + fabs(wj.a + wp.a + wlp.a + wlj.a) * qz;
-            const double dtiy1 = fabs(uj.c + up.c + up.b + uj.b) * qx + fabs(vj.b) * a.rdy + fabs(wj.b + wp.b + wlp.b + wlj.b) * qz;
-            const double dtiz0 = fabs(uj.b + uj.a + un.a + un.b) * qx + fabs(vj.a + vm.a + vmn.a + vjn.a) * qy + fabs(wj.a) * rzc;
-            const double dtiz1 = fabs(uj.c + uj.b + un.b + un.c) * qx + fabs(vj.b + vm.b + vmn.b + vjn.b) * qy + fabs(wj.b) * rzc;
-            m = fmax(m, fmax(fmax(dtix0, dtix1), fmax(fmax(dtiy0, dtiy1), fmax(dtiz0, dtiz1))));
+            m = fmax(m, chk_cell_max(a, k, uj, up, un, vm, vj, vmn, vjn, wlj, wlp, wj, wp));
             uj = un; vm = vmn; vj = vjn; wlj = wj; wlp = wp;
         }
     }

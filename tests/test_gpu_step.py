@@ -54,6 +54,56 @@ def test_chkdt_matches_the_oracle_for_every_boundary_combination(B, nx, ny, nz):
         plan.close()
 
 
+@pytest.mark.parametrize("bcs", ["PP/PP/PP", "NN/NN/NN", "DD/DD/DD", "ND/DN/NN", "PP/NN/DD", "DN/PP/ND"])
+def test_chkdt_localised_maxima_at_every_kind_of_boundary(B, bcs):
+    """The reduction returns one number: to see a wrong stencil at a boundary, the maximum is planted there.  Small noise
+    everywhere plus O(1) values in the 3 x 3 x 3 neighbourhood of one cell -- the corners, edge and face centres of the box, a
+    warp edge in x (i = 63 | 64) and an interior cell -- each compared with the oracle."""
+    nx, ny, nz = 128, 32, 35            # nz > 32: the marching chunks meet inside the column
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    px, py, pz = bcs.split("/")
+    bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+    rng = np.random.default_rng(5)
+    faces = _faces(rng, bc, (nz, ny, nx), inflow=tuple(d for d in range(3) if bc[d][0] == "N"))
+    for f in faces.values():
+        f *= 1e-3
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    fd = {d: torch.from_numpy(f.copy()).cuda() for d, f in faces.items()}
+    for d, t in fd.items():
+        plan.set_lower_face(d, t)
+    dti = torch.zeros((1,), dtype=torch.float64, device="cuda")
+    spots = [(i, j, k) for i in (0, nx - 1) for j in (0, ny - 1) for k in (0, nz - 1)]
+    spots += [(nx // 2, 0, 0), (0, ny // 2, nz - 1), (nx - 1, ny - 1, nz // 2), (63, 7, 31), (64, 8, 32), (nx // 2, ny // 2, nz // 2),
+              (nx // 2, ny // 2, 0), (nx // 2, ny // 2, nz - 1), (0, ny // 2, nz // 2), (nx - 1, ny // 2, nz // 2),
+              (nx // 2, 0, nz // 2), (nx // 2, ny - 1, nz // 2)]
+    base = [1e-3 * rng.standard_normal((nz, ny, nx)) for _ in range(3)]
+    for (i, j, k) in spots:
+        fields = [b.copy() for b in base]
+        for f in fields:
+            for dk in (-1, 0, 1):
+                for dj in (-1, 0, 1):
+                    for di in (-1, 0, 1):
+                        kk, jj, ii = k + dk, j + dj, i + di
+                        if 0 <= kk < nz and 0 <= jj < ny and 0 <= ii < nx:
+                            f[kk, jj, ii] = rng.uniform(0.5, 1.5) * rng.choice((-1.0, 1.0))
+        # the boundary planes next to the spot carry O(1) values too
+        fl = {d: f.copy() for d, f in faces.items()}
+        for d, f in fl.items():
+            near = (i, j, k)[d] <= 1
+            if near:
+                f += rng.uniform(0.5, 1.5, size=f.shape) * (np.abs(rng.standard_normal(f.shape)) < 0.3)
+        for d, t in fd.items():
+            t.copy_(torch.from_numpy(fl[d]))
+        u, v, w = fields
+        plan.chkdt(*(torch.from_numpy(a).cuda() for a in (u, v, w)), dti)
+        torch.cuda.synchronize()
+        want = orc.chkdt(u, v, w, lx, ly, lz, bc, dzc, dzf, fl)
+        assert abs(float(dti[0]) - want) <= 1e-13 * want, (bcs, (i, j, k), float(dti[0]), want)
+    plan.close()
+
+
 def test_chkdt_special_values_and_errors(B):
     nx, ny, nz = 32, 16, 8
     bc = (("P", "P"), ("P", "P"), ("N", "N"))
