@@ -828,10 +828,8 @@ int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* m
     CUtensorMap tmap_wide;
     if (which == 0) {            // z solve: tiles of z_tc_for(nseg) columns x nz rows of the (nz, nx*ny) view
         const int tc = z_tc_for(plan->nseg);
-        int d = 256 / Z_MROWS;
-        while (plan->nseg % d) --d;
         sh.ntiles = ((long)plan->nx * plan->ny + tc - 1) / tc; sh.m0 = sh.ntiles; sh.s0 = tc; sh.s1 = 0;
-        sh.box_rows = d * Z_MROWS; sh.nbox = plan->nseg / d; sh.box_cols = tc;
+        z_boxes(plan->nseg, &sh.nbox, &sh.box_rows); sh.box_cols = tc;
         tmap = &plan->tmap_z;
     } else if (which == 1) {     // TMA-fed y transforms: tiles of 16 doubles x ny rows of one k-plane
         if (!plan->use_yt) return fail(CANS_ERR_UNSUPPORTED_SIZE, "this ny does not run the TMA-fed y transforms");

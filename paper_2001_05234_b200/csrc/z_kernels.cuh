@@ -16,6 +16,8 @@ size_t z_solve_smem_bytes(int nseg, int cyclic);
 constexpr size_t Z_SMEM_LIMIT = 227u * 1024u;
 // plan time: opt in to the dynamic shared memory of the solve kernel and compute the persistent grid
 cudaError_t z_solve_configure(int nseg, int cyclic, int num_sms, int* grid_out, size_t* smem_out);   // cudaErrorInvalidConfiguration: the tile buffers do not fit
+// TMA boxes covering the padded column exactly: nbox boxes of box_rows (<= 256) rows
+void z_boxes(int nseg, int* nbox, int* box_rows);
 // tensor map of the (nz, nx*ny) view of the field p, boxes of z_tc_for(nseg) columns
 cudaError_t z_make_tensor_map(CUtensorMap* tmap, const double* p, long ncols, int nz, int nseg);
 // enqueue the solve (a.ticket must point at a zeroed counter; tmap from z_make_tensor_map for a.p)

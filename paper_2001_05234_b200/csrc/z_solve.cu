@@ -151,13 +151,15 @@ cudaError_t z_solve_configure(int nseg, int cyclic, int num_sms, int* grid_out, 
     }
 }
 
-// TMA tiling of a column tile: the padded column length nseg*MROWS is covered exactly by nbox boxes of box_rows
-// (<= 256) rows, box_rows = MROWS * (largest divisor of nseg that is <= 256/MROWS)
-static void z_boxes(int nseg, int* nbox, int* box_rows) {
-    int d = 256 / Z_MROWS;
-    while (nseg % d) --d;
-    *box_rows = d * Z_MROWS;
-    *nbox = nseg / d;
+// TMA tiling of a column tile: the padded column length nzp = nseg*MROWS is covered exactly by nbox boxes of box_rows rows,
+// box_rows = the largest divisor of nzp that is <= 256 (any divisor, not only whole segments: a prime segment count -- nz =
+// 577..592 gives nseg = 37 -- still gets boxes of 148 rows, not 37 boxes of 16)
+void z_boxes(int nseg, int* nbox, int* box_rows) {
+    const int nzp = nseg * Z_MROWS;
+    int br = nzp < 256 ? nzp : 256;
+    while (nzp % br) --br;
+    *box_rows = br;
+    *nbox = nzp / br;
 }
 
 cudaError_t z_make_tensor_map(CUtensorMap* tmap, const double* p, long ncols, int nz, int nseg) {

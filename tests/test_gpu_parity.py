@@ -358,9 +358,10 @@ def test_lower_face_argument_checks(B):
     plan.close()
 
 
-@pytest.mark.parametrize("nz", [1024, 1000, 513])
+@pytest.mark.parametrize("nz", [1024, 1000, 590, 513])
 def test_tallest_columns(B, nz):
-    """nz up to the documented maximum (64 z segments, tiles of 8 columns, four TMA boxes per tile) and ragged heights."""
+    """nz up to the documented maximum (64 z segments, tiles of 8 columns, four TMA boxes per tile) and ragged heights;
+    590: a prime number of segments (37), whose padded column is tiled by four boxes of 148 rows."""
     nx, ny = 48, 32
     lx, ly, lz = 1.0, 1.0, 2.0
     dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.8)
