@@ -2,13 +2,13 @@
 // gradient-correction kernels, and the launch sequences of cans_poisson_solve / cans_projection.
 //
 // Hot path (eqs. 2b, 5, 6, 2c), default launch sequence:
-//   a1+a2  xw_kernel<fwd, DIV> / x_pass_kernel   divergence fused into the forward x transform
-//   a3     yw_kernel<fwd>      / y_pass_kernel   forward y transform (strided, tile staged in shared memory)
-//   a4     z_solve_kernel                        Thomas solve per (kx, ky) mode (TMA tiles), singular mode pinned
-//   a5     yw_kernel<inv>      / y_pass_kernel
-//   a6     xw_kernel<inv>      / x_pass_kernel
-//   a7     grad_correct_kernel                   u -= dt G Phi
-// (xw / yw: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
+//   a1+a2  xw_kernel<fwd, DIV> / x_pass_kernel          divergence fused into the forward x transform
+//   a3     yt_kernel<fwd> / yw_kernel / y_pass_kernel   forward y transform (strided; tiles staged in shared memory, by TMA for 512, 768)
+//   a4     z_solve_kernel                               Thomas solve per (kx, ky) mode (TMA tiles), singular mode pinned, cyclic for periodic z
+//   a5     yt_kernel<inv> / yw_kernel / y_pass_kernel
+//   a6     xw_kernel<inv> / x_pass_kernel
+//   a7     grad_correct_kernel (+ face_correct_kernel)  u -= dt G Phi, optionally p_acc += Phi (eq. 2d); then chkdt_kernel on request
+// (xw / yt / yw: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
 //  FFTs for the other lengths.)
 // Every x / y / correction kernel takes a range of k-planes (XYArgs::k0, nk; GradArgs::k0, k1); the entry points launch each
 // once over all planes -- per-batch launches through L2 were measured and are slower (profiles/r02a_plane_batching.md).

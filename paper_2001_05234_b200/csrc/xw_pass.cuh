@@ -5,12 +5,15 @@
 //
 //   * ONE WARP owns a pair of rows from the first load to the last store: no CTA barrier anywhere, warps
 //     drift apart freely, so one warp's loads overlap another warp's butterflies;
-//   * 2-pass Cooley-Tukey in REGISTERS: lane p loads x[p + 32 m] (m < R1) straight from global memory --
-//     2*R1 independent, perfectly coalesced 8-byte loads in flight per lane -- does the R1-point DFT over m,
-//     applies W_N^(p k1), exchanges once through a padded per-warp shared-memory buffer, and lane k1 does
-//     the 32-point DFT over p.  One shared-memory round trip instead of three;
+//   * 2-pass Cooley-Tukey in REGISTERS: lane p holds the FFT input elements p + 32 m (m < R1) -- periodic rows as
+//     2*R1 coalesced 8-byte loads straight from global memory, non-periodic rows as 16-byte sample pairs whose odd
+//     sample goes to the mirrored lane by one shuffle (Makhoul's permutation is a lane mirror), the fused divergence
+//     through one staging pass in the warp's buffer -- does the R1-point DFT over m, applies W_N^(p k1), exchanges once
+//     through a padded per-warp shared-memory buffer, and lane k1 does the 32-point DFT over p.  One shared-memory
+//     round trip instead of three;
 //   * the spectrum is laid out in natural order in the same buffer for the real/imaginary separation
-//     (post_forward / pre_inverse of xy_pass.cuh) and goes to global memory as coalesced 16-byte stores.
+//     (post_forward / pre_inverse of xy_pass.cuh) and goes to global memory as coalesced 16-byte stores;
+//   * one kernel per class of boundary pair (KC: PP; NN / DD; ND / DN), so the periodic kernels carry no twiddle code.
 //
 // Forward:  X[k1 + R1 k2] = sum_p W_32^(p k2) * W_N^(p k1) * sum_m W_R1^(m k1) x[p + 32 m]
 // Inverse:  the same factorisation run backwards with conjugated roots (unnormalised).

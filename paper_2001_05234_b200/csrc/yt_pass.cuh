@@ -6,9 +6,11 @@
 //     SWIZZLE_128B, completion on an mbarrier) and, after the transform, shared -> global -- no thread issues a
 //     global load or store, and the copy of tile n+1 / the write-back of tile n-1 overlap the transform of tile n
 //     (two buffers);
-//   * warp f owns column f of the tile from the first to the last shared-memory access: input permutation,
-//     2-pass register FFT (as yw_pass.cuh) and real/imaginary separation all happen in place with __syncwarp
-//     only; one CTA barrier per tile hands the finished tile to the TMA store.
+//   * warp f owns column f of the tile from the first to the last shared-memory access: the 2-pass register FFT (as
+//     yw_pass.cuh; the permutation of the non-periodic pairs is folded into its first load / last store) and the
+//     real/imaginary separation all happen in place with __syncwarp only; one CTA barrier per tile hands the
+//     finished tile to the TMA store;
+//   * one kernel per class of boundary pair (KC), as in xw_pass.cuh.
 // With the 128-byte swizzle, element (row e, column f) sits at complex index e*8 + (f ^ (e & 7)): the eight lanes of a
 // quarter warp reading one column at eight consecutive (or XOR-permuted) rows hit eight different 16-byte bank
 // groups, so every column access of the FFT is conflict free without padding.

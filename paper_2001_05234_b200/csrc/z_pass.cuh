@@ -18,9 +18,10 @@
 //     (nx*ny*P doubles, 1/MROWS of a field) and recomputed in-register -- bit-identical to the
 //     sequential pivots;
 //   * d' and x are first-order linear recurrences: each segment runs them from a zero start while
-//     accumulating the propagation factor (prod of -a_k r_k, resp. -c_k r_k); a P-step scan over the
-//     segment ends in shared memory supplies the true start value, which is then propagated;
-//   * results go straight from registers to global memory (coalesced rows).
+//     accumulating the propagation factor (prod of -a_k r_k, resp. -c_k r_k); a scan over the segment ends --
+//     composed per warp by shuffles, one aggregate per group of 32/TC segments in shared memory (group_scan) --
+//     supplies the true start value, which is then propagated;
+//   * results go straight from registers to global memory (coalesced rows, a walking pointer, no per-row predicate).
 // The singular kx = ky = 0 column of an all-periodic/Neumann problem is handled by z_singular_stage / _sweeps / _store
 // (CTA 0, before it joins the tile loop).
 //
