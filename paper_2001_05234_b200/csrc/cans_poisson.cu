@@ -3,12 +3,12 @@
 //
 // Hot path (eqs. 2b, 5, 6, 2c), default launch sequence:
 //   a1+a2  xw_kernel<fwd, DIV> / x_pass_kernel          divergence fused into the forward x transform
-//   a3     yt_kernel<fwd> / yw_kernel / y_pass_kernel   forward y transform (strided; tiles staged in shared memory, by TMA for 512, 768)
+//   a3     yt_kernel<fwd> / y_pass_kernel               forward y transform (strided; tiles staged in shared memory, by TMA for 512, 768, 1024)
 //   a4     z_solve_kernel                               Thomas solve per (kx, ky) mode (TMA tiles), singular mode pinned, cyclic for periodic z
-//   a5     yt_kernel<inv> / yw_kernel / y_pass_kernel
+//   a5     yt_kernel<inv> / y_pass_kernel
 //   a6     xw_kernel<inv> / x_pass_kernel
 //   a7     grad_correct_kernel (+ face_correct_kernel)  u -= dt G Phi, optionally p_acc += Phi (eq. 2d); then chkdt_kernel on request
-// (xw / yt / yw: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
+// (xw / yt: warp-level 2-pass register FFTs for lengths 512, 768, 1024; x_pass / y_pass: 3-pass shared-memory
 //  FFTs for the other lengths.)
 // Every x / y / correction kernel takes a range of k-planes (XYArgs::k0, nk; GradArgs::k0, k1); the entry points launch each
 // once over all planes -- per-batch launches through L2 were measured and are slower (profiles/r02a_plane_batching.md).
@@ -28,7 +28,6 @@
 #include "grad_pass.cuh"
 #include "chkdt_pass.cuh"
 #include "xw_kernels.cuh"
-#include "yw_kernels.cuh"
 #include "yt_kernels.cuh"
 #include "probes.cuh"
 
@@ -321,8 +320,7 @@ struct cans_poisson_plan {
     cplx wstep_x[32], wstep_y[32];   // mixed pairs, warp-level kernels: wpre[32 m] (XYArgs::wstep)
     cplx* tw2_x;              // W_nx^(p k1), [nx/32][32]: warp-per-line x kernels (xw_pass.cuh), or NULL
     int use_xw;               // 1: x transforms run the warp-per-line kernels
-    cplx* tw2_y;              // the same for ny (yw_pass.cuh), or NULL
-    int use_yw;
+    cplx* tw2_y;              // the same for ny (yt_pass.cuh), or NULL
     int use_yt;               // 1: y transforms run the persistent TMA-fed kernels (yt_pass.cuh)
     // TMA descriptors of the field the last call worked on: encoded on the host only when the pointer changes
     const double* tmap_field;
@@ -423,7 +421,6 @@ static int launch_xy_any(cans_poisson_plan* pl, int n, int op, const XYArgs& a, 
     bool done = false;
     if (xdir && pl->use_xw) done = xw_launch(n, op, a, pl->tw2_x, st, &err);
     else if (!xdir && pl->use_yt) done = yt_launch(n, op, a, pl->tw2_y, &pl->tmap_y, pl->num_sms, st, &err);
-    else if (!xdir && pl->use_yw) done = yw_launch(n, op, a, pl->tw2_y, st, &err);
     if (!done)
         done = launch_xy_group_a(n, op, a, st, &err) || launch_xy_group_b(n, op, a, st, &err) ||
                launch_xy_group_c(n, op, a, st, &err) || launch_xy_group_d(n, op, a, st, &err);
@@ -444,7 +441,6 @@ static cudaError_t configure_kernels(cans_poisson_plan* pl) {
         if (e != cudaSuccess) return e;
     }
     if (pl->use_xw) { xw_launch(pl->nx, OP_CONFIGURE, dummy, pl->tw2_x, 0, &e); if (e != cudaSuccess) return e; }
-    if (pl->use_yw) { yw_launch(pl->ny, OP_CONFIGURE, dummy, pl->tw2_y, 0, &e); if (e != cudaSuccess) return e; }
     if (pl->use_yt) { yt_launch(pl->ny, OP_CONFIGURE, dummy, pl->tw2_y, nullptr, pl->num_sms, 0, &e); if (e != cudaSuccess) return e; }
     return e;
 }
@@ -567,12 +563,11 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
         pl->use_xw = 1;
     }
     pl->tw2_y = nullptr;
-    pl->use_yw = 0;
-    if (yw_supported(ny) && (nx / 2) % YW_TXC == 0) {
+    pl->use_yt = 0;
+    if (yt_supported(ny) && (nx / 2) % YT_COLS == 0) {
         up(make_two_pass_twiddles(ny), &pl->tw2_y);
-        pl->use_yw = 1;
+        pl->use_yt = 1;
     }
-    pl->use_yt = (pl->use_yw && yt_supported(ny)) ? 1 : 0;
     if (e == cudaSuccess) {
         void* d = nullptr;
         e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
@@ -832,7 +827,7 @@ int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* m
         z_boxes(plan->nseg, &sh.nbox, &sh.box_rows); sh.box_cols = tc;
         tmap = &plan->tmap_z;
     } else if (which == 1) {     // TMA-fed y transforms: tiles of 16 doubles x ny rows of one k-plane
-        if (!plan->use_yt) return fail(CANS_ERR_UNSUPPORTED_SIZE, "this ny does not run the TMA-fed y transforms");
+        if (!plan->use_yt || plan->ny > 768) return fail(CANS_ERR_UNSUPPORTED_SIZE, "the y-tile probe needs two tile buffers: ny = 512, 768");
         sh.m0 = plan->nx / 2 / YT_COLS; sh.ntiles = sh.m0 * plan->nz; sh.s0 = 2 * YT_COLS; sh.s1 = plan->ny;
         sh.box_rows = YT_BOX_ROWS; sh.nbox = plan->ny / YT_BOX_ROWS; sh.box_cols = 2 * YT_COLS;
         tmap = &plan->tmap_y;

@@ -30,8 +30,10 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
 #pragma unroll
         for (int box = 0; box < W::NBOX; ++box) {
             if (!first) {
+                // box b may be refilled once the write-back group of box b has read it: at most NBOX-1-b younger groups pending
                 if (box == 0) tma_store_wait_read_pending<W::NBOX - 1>();
                 else if (box == 1) tma_store_wait_read_pending<(W::NBOX > 2 ? W::NBOX - 2 : 0)>();
+                else if (box == 2) tma_store_wait_read_pending<(W::NBOX > 3 ? W::NBOX - 3 : 0)>();
                 else tma_store_wait_read_pending<0>();
             }
             tma_load_2d(bufs + (size_t)bsel * W::TILE + (size_t)box * YT_BOX_ROWS * YT_COLS, &tmap, 2 * YT_COLS * c,
@@ -43,9 +45,13 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     if (tid == 0) issue_load(t, 0, true);
     unsigned phases = 0u;
     int b = 0;
+    // NBUF = 2: the copy of the next tile into the other buffer is issued before this tile is transformed.  NBUF = 1 (one
+    // tile fills the shared memory: N = 1024): the next tile is copied into the same buffer box by box, each box as soon
+    // as its write-back has read it -- the transform of a tile overlaps nothing but the tail of the previous write-back.
+    constexpr int NBUF = W::NBUF;
     for (; t < ntiles; t += gridDim.x) {
         const long tn = t + gridDim.x;
-        if (tid == 0 && tn < ntiles) {
+        if (NBUF == 2 && tid == 0 && tn < ntiles) {
             issue_load(tn, b ^ 1, false);
         }
         mbar_wait(&s_bar[b], (phases >> b) & 1u);
@@ -69,15 +75,16 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
                 tma_store_2d(&tmap, 2 * YT_COLS * c, k * N + box * YT_BOX_ROWS, T + (size_t)box * YT_BOX_ROWS * YT_COLS);
                 tma_store_commit();             // one bulk group per box
             }
+            if (NBUF == 1 && tn < ntiles) issue_load(tn, 0, false);
         }
-        b ^= 1;
+        if (NBUF == 2) b ^= 1;
     }
     if (tid == 0) tma_store_wait_all();
 }
 
 template <int N, int R1, int KC>
 static cudaError_t yt_launch_k(int op, const XYArgs& a, const cplx* tw, const CUtensorMap* tmap, int max_ctas, cudaStream_t st) {
-    const size_t smem = 2 * sizeof(cplx) * (size_t)YTPass<N, R1, KC>::TILE;
+    const size_t smem = YTPass<N, R1, KC>::NBUF * sizeof(cplx) * (size_t)YTPass<N, R1, KC>::TILE;
     if (op == OP_CONFIGURE) {
         cudaError_t e = cudaFuncSetAttribute(yt_kernel<N, R1, false, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e == cudaSuccess) e = cudaFuncSetAttribute(yt_kernel<N, R1, true, KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -118,6 +125,7 @@ bool yt_launch(int n, int op, const XYArgs& a, const cplx* tw, const CUtensorMap
     switch (n) {
         case 512: *err = yt_launch_n<512, 16>(op, a, tw, tmap, max_ctas, st); return true;
         case 768: *err = yt_launch_n<768, 24>(op, a, tw, tmap, max_ctas, st); return true;
+        case 1024: *err = yt_launch_n<1024, 32>(op, a, tw, tmap, max_ctas, st); return true;
         default: return false;
     }
 }

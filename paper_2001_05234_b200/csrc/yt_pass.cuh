@@ -1,5 +1,5 @@
-// yt_pass.cuh -- TMA-fed y transforms (N = R1 * 32 with two tiles fitting shared memory: 512, 768): F^y of eq. 6
-// and its inverse.  Mathematics and slot layout as YPass / YWPass.
+// yt_pass.cuh -- TMA-fed y transforms (N = R1 * 32: 512, 768 with two tile buffers, 1024 with one): F^y of eq. 6
+// and its inverse.  Mathematics and slot layout as YPass (xy_pass.cuh).
 //
 // A persistent CTA of 8 warps (one per SM) walks over tiles of 8 complex columns x N rows:
 //   * the TMA unit copies the tile global -> shared (cp.async.bulk.tensor.2d, boxes of 16 doubles x 256 rows,
@@ -7,7 +7,7 @@
 //     global load or store, and the copy of tile n+1 / the write-back of tile n-1 overlap the transform of tile n
 //     (two buffers);
 //   * warp f owns column f of the tile from the first to the last shared-memory access: the 2-pass register FFT (as
-//     yw_pass.cuh; the permutation of the non-periodic pairs is folded into its first load / last store) and the
+//     xw_pass.cuh; the permutation of the non-periodic pairs is folded into its first load / last store) and the
 //     real/imaginary separation all happen in place with __syncwarp only; one CTA barrier per tile hands the
 //     finished tile to the TMA store;
 //   * one kernel per class of boundary pair (KC), as in xw_pass.cuh.
@@ -23,7 +23,7 @@ namespace cans {
 constexpr int YT_COLS = 8;                       // complex columns per tile = warps per CTA
 constexpr int YT_NT = YT_COLS * 32;
 constexpr int YT_BOX_ROWS = 256;
-inline bool yt_supported(int n) { return n == 512 || n == 768; }
+inline bool yt_supported(int n) { return n == 512 || n == 768 || n == 1024; }
 
 // KC: class of the boundary pair, a compile-time switch so that the periodic kernels carry none of the registers of the
 // permutation / twiddle paths: 0 = PP, 1 = NN / DD, 2 = ND / DN (the pair inside a class is the run-time `kind`)
@@ -37,6 +37,7 @@ struct YTPass {
     static constexpr int TILE = N * YT_COLS;                         // cplx per buffer
     static constexpr int NBOX = N / YT_BOX_ROWS;
     static constexpr unsigned TILE_BYTES = (unsigned)(TILE * sizeof(cplx));
+    static constexpr int NBUF = (2 * TILE_BYTES <= 200 * 1024) ? 2 : 1;      // tile buffers that fit the shared memory
 
 #if defined(__CUDACC__)
     static CANS_D int at(int e, int f) { return e * YT_COLS + (f ^ (e & 7)); }

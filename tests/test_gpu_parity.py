@@ -243,7 +243,7 @@ def test_repeated_calls_are_bit_identical(B, nx, ny, nz):
 
 @pytest.mark.parametrize("nx,ny,nz", [(512, 512, 9), (768, 1024, 5), (1024, 768, 6)])
 def test_warp_level_transform_kernels_every_kind_pair(B, nx, ny, nz):
-    """Lengths 512 / 768 / 1024 run the warp-level 2-pass kernels (xw_pass.cuh, yw_pass.cuh): every (x, y)
+    """Lengths 512 / 768 / 1024 run the warp-level 2-pass kernels (xw_pass.cuh, yt_pass.cuh): every (x, y)
     boundary-pair combination against the oracle, on a stretched grid, Poisson and (where allowed) projection."""
     lx, ly, lz = 2 * np.pi, np.pi, 2.0
     dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
