@@ -22,13 +22,15 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     // tile t = (plane k, column tile c): boxes of 16 doubles x 256 rows at (16 c, k N + 256 box)
     // FIRST: all boxes at once.  Otherwise box by box, each as soon as the write-back of the same box of the tile
     // that occupied this buffer (one bulk group per box, oldest first) has finished reading shared memory.
-    auto issue_load = [&](long t, int bsel, bool first) {
+    // boxes [box0, box1) of tile t into buffer bsel; the first box of a tile arms the buffer's mbarrier for the whole tile
+    auto issue_load = [&](long t, int bsel, bool first, int box0, int box1) {
         const int kl = (int)(t / ntx);
         const int c = (int)(t - (long)kl * ntx);
         const int k = a.k0 + kl;
-        mbar_expect_tx(&s_bar[bsel], W::TILE_BYTES);
+        if (box0 == 0) mbar_expect_tx(&s_bar[bsel], W::TILE_BYTES);
 #pragma unroll
         for (int box = 0; box < W::NBOX; ++box) {
+            if (box < box0 || box >= box1) continue;
             if (!first) {
                 // box b may be refilled once the write-back group of box b has read it: at most NBOX-1-b younger groups pending
                 if (box == 0) tma_store_wait_read_pending<W::NBOX - 1>();
@@ -42,7 +44,7 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     };
     long t = blockIdx.x;
     if (t >= ntiles) return;
-    if (tid == 0) issue_load(t, 0, true);
+    if (tid == 0) issue_load(t, 0, true, 0, W::NBOX);
     unsigned phases = 0u;
     int b = 0;
     // NBUF = 2: the copy of the next tile into the other buffer is issued before this tile is transformed.  NBUF = 1 (one
@@ -51,17 +53,22 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
     constexpr int NBUF = W::NBUF;
     for (; t < ntiles; t += gridDim.x) {
         const long tn = t + gridDim.x;
-        if (NBUF == 2 && tid == 0 && tn < ntiles) {
-            issue_load(tn, b ^ 1, false);
-        }
+        // The thread that issued the write-back of the previous tile (same buffer b^1) must wait for each box to be read
+        // before refilling it: it asks for the first box now (its write-back group is the oldest) and for the others
+        // between its own two transform phases, when they have drained -- it hardly ever blocks, so its warp does not
+        // keep the other seven waiting at the tile barrier.
+        if (NBUF == 2 && tid == 0 && tn < ntiles) issue_load(tn, b ^ 1, false, 0, 1);
         mbar_wait(&s_bar[b], (phases >> b) & 1u);
         phases ^= 1u << b;
         cplx* T = bufs + (size_t)b * W::TILE;
         if (INV) {
             W::slots_in(a, T, warp, lane);
+            if (NBUF == 2 && tid == 0 && tn < ntiles) issue_load(tn, b ^ 1, false, 1, W::NBOX);
             W::column_inverse(a, T, warp, tw, lane);
         } else {
-            W::column_forward(a, T, warp, tw, lane);
+            W::column_forward(a, T, warp, tw, lane, [&]() {
+                if (NBUF == 2 && tid == 0 && tn < ntiles) issue_load(tn, b ^ 1, false, 1, W::NBOX);
+            });
             W::slots_out(a, T, warp, lane);
         }
         fence_proxy_async_smem();               // this thread's shared-memory writes -> visible to the TMA unit
@@ -75,7 +82,7 @@ __global__ void __launch_bounds__(YT_NT, 1) yt_kernel(const XYArgs a, const cplx
                 tma_store_2d(&tmap, 2 * YT_COLS * c, k * N + box * YT_BOX_ROWS, T + (size_t)box * YT_BOX_ROWS * YT_COLS);
                 tma_store_commit();             // one bulk group per box
             }
-            if (NBUF == 1 && tn < ntiles) issue_load(tn, 0, false);
+            if (NBUF == 1 && tn < ntiles) issue_load(tn, 0, false, 0, W::NBOX);
         }
         if (NBUF == 2) b ^= 1;
     }

@@ -115,7 +115,9 @@ struct YTPass {
     }
 
     // rows as loaded (natural order) -> natural-order spectrum, in place in column f (unnormalised)
-    static CANS_D void column_forward(const XYArgs& a, cplx* t, int f, const cplx* __restrict__ tw, int lane) {
+    // `mid` runs between the two passes (the kernel's elected thread issues TMA work there)
+    template <class Mid>
+    static CANS_D void column_forward(const XYArgs& a, cplx* t, int f, const cplx* __restrict__ tw, int lane, Mid&& mid) {
         cplx v[R1];
         load_elems(a, t, f, lane, v);
         Dft<R1, false>::run(v);
@@ -123,6 +125,7 @@ struct YTPass {
         __syncwarp();
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1) t[at(k1 * 32 + (lane ^ k1), f)] = v[k1];
+        mid();
         __syncwarp();
         cplx w[32];
         if (lane < R1) {
