@@ -273,6 +273,25 @@ def test_warp_level_transform_kernels_every_kind_pair(B, nx, ny, nz):
         plan.close()
 
 
+@pytest.mark.parametrize("ny", [512, 768, 1024])
+def test_y_tile_pipeline_several_tiles_per_cta(B, ny):
+    """The persistent TMA-fed y kernels with 600 tiles on 148 CTAs: every CTA walks 4-5 tiles, so the steady state of the
+    tile pipeline runs -- two buffers for 512 / 768, ONE buffer refilled box by box behind its write-back for 1024."""
+    nx, nz = 32, 300
+    lx, ly, lz = 1.0, 2.0, 1.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.4)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    for n, bc in enumerate(((("P", "P"), ("P", "P"), ("N", "N")), (("N", "N"), ("D", "N"), ("D", "D")))):
+        f = random_rhs(nx, ny, nz, bc, dzf, 7100 + ny + n)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        torch.cuda.synchronize()
+        plan.close()
+        ref = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        check_field(np_of(p), ref, what=f"ny={ny} {bc}")
+
+
 @pytest.mark.parametrize("nx,ny,nz", [(1024, 768, 3), (768, 1024, 3), (512, 512, 17), (256, 128, 18), (48, 96, 33)])
 def test_no_write_outside_the_fields(B, nx, ny, nz):
     """Every field lives inside a larger allocation whose guard zones (before and after, 1 MiB each) hold a
