@@ -60,7 +60,7 @@ def test_cell_centred_helmholtz_every_boundary_combination(B, nx, ny, nz, stretc
         check(q.cpu().numpy(), orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc, dzf), f"{px}/{py}/{pz} alpha={alpha}")
 
 
-@pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 32, 33, 1.6), (1024, 64, 9, None), (32, 48, 512, 1.6), (32, 16, 257, 2.0)])
+@pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 32, 33, 1.6), (1024, 64, 9, None), (32, 48, 512, 1.6), (32, 16, 257, 2.0), (32, 32, 600, 1.6)])
 def test_face_located_unknowns(B, nx, ny, nz, stretch):
     """The three velocity components of the channel configuration: u (faces in x), v (faces in y) with no-slip walls in z
     ('D','D', cell-centred in z), w on the z faces between the walls; and w in a triperiodic box."""

@@ -399,6 +399,28 @@ def test_tallest_columns(B, nz):
     assert ei.value.status == B.CANS_ERR_UNSUPPORTED_SIZE
 
 
+@pytest.mark.parametrize("nz", [576, 1000])
+def test_tall_columns_tile_pipeline(B, nz):
+    """nz > 512 (tiles of 8 columns, up to 64 segments): 6144 columns = 768 tiles on 148 CTAs, so the ticket and the
+    double-buffered tiles reach their steady state.  Singular and regular; a repeated call is bit-identical."""
+    nx, ny = 96, 64
+    lx, ly, lz = 1.0, 1.5, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.7)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    for n, bc in enumerate(((("P", "P"), ("N", "N"), ("N", "N")), (("D", "N"), ("P", "P"), ("N", "D")))):
+        f = random_rhs(nx, ny, nz, bc, dzf, 8200 + nz + n)
+        plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+        p = torch.from_numpy(f).cuda()
+        plan.poisson_solve(p)
+        q = torch.from_numpy(f).cuda()
+        plan.poisson_solve(q)                      # a second call: the ticket is reset, the result repeats bit for bit
+        torch.cuda.synchronize()
+        plan.close()
+        assert torch.equal(p, q)
+        ref = orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf)
+        check_field(np_of(p), ref, what=f"nz={nz} {bc}")
+
+
 # ----------------------------------------------------------------------------------------------
 # the z-solve instantiation bench.py times on C4 / C5: 257 <= nz <= 512 runs z_solve_kernel<16,16> (tiles of 16 columns,
 # up to 32 segments per column, two TMA boxes per tile).  48 x 32 columns = 96 tiles, so a persistent CTA sees several
