@@ -147,6 +147,42 @@ int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* 
 int cans_chkdt(cans_poisson_plan* plan, const double* u, const double* v, const double* w, double* dti, void* stream);
 
 /*
+ * cans_chkdt_static -- cans_chkdt for callers that cannot allocate device memory: no plan, no cudaMalloc / cudaFree and no
+ * allocating library routine anywhere inside it.
+ *
+ * Why it exists.  A plan owns device tables, so creating one allocates and destroying one frees.  Two kinds of caller
+ * cannot do that at the point where they need the time step: a solver whose own arena already fills the board's memory
+ * (the driver has nothing left to give, the plan's cudaMalloc fails), and a time loop that keeps several streams busy
+ * (cudaMalloc and cudaFree wait for the whole device, so every stream in flight stalls behind them).  For them the memory
+ * the kernel needs besides the caller's arrays -- the reciprocal z spacings and one partial maximum per CTA -- is a fixed
+ * array inside the library image: 528 KB on every GPU that loads libcans_poisson.so, held until the process exits.
+ *
+ *   nx, ny, nz, lx, ly, lz, bc   as cans_poisson_plan_create (bc = the pressure pairs that fix the ghost rule of cans_chkdt);
+ *                nx even and (nx/2)*ny a multiple of 32 (every size a plan accepts is), and within the fixed array:
+ *                nz <= CANS_STATIC_MAX_NZ  and  ceil(nx*ny/512) * ceil(nz/32) <= CANS_STATIC_MAX_CTAS
+ *                (about 2^30 cells: 1024 x 768 x 512 and 1536 x 768 x 576 fit).  Anything larger returns
+ *                CANS_ERR_UNSUPPORTED_SIZE with a message that names the limit; nothing is launched.
+ *   dzc, dzf     DEVICE (not host, unlike the plan: a host array would have to be staged), nz+1 / nz doubles with the meaning
+ *                given at cans_poisson_plan_create, or both NULL for the uniform spacing lz/nz.  Read on the stream.
+ *   u, v, w      DEVICE, nx*ny*nz doubles each, 16-byte aligned, read only.
+ *   face_x/y/z   DEVICE lower-face planes with the layout of cans_projection_set_lower_face, or NULL.  Required on a lower
+ *                'D' side (CANS_ERR_NEEDS_FACE), optional on a lower 'N' side (prescribed inflow), must be NULL on 'P'.
+ *   dti          DEVICE, one double, overwritten; the same value cans_chkdt returns, bit for bit.
+ *   stream       cudaStream_t as void*.  Two kernels are enqueued; nothing synchronises.
+ *
+ * The fixed array is shared by every call in the process and keeps the contents of the last one.  Each call rewrites the
+ * spacing tables and zeroes its arrival counter before use, so calls on one stream, or otherwise ordered on the GPU, are
+ * independent of each other; calls that can overlap on the GPU (two streams, two host threads) race and return garbage.
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, once, cached): make that first
+ * call with the device current and outside any stream capture.
+ */
+#define CANS_STATIC_MAX_NZ    1024
+#define CANS_STATIC_MAX_CTAS  65536
+int cans_chkdt_static(int nx, int ny, int nz, double lx, double ly, double lz, const char bc[3][2],
+                      const double* dzc, const double* dzf, const double* u, const double* v, const double* w,
+                      const double* face_x, const double* face_y, const double* face_z, double* dti, void* stream);
+
+/*
  * cans_projection_set_lower_face -- register the boundary-normal velocity on the LOWER face of
  * direction dir (0,1,2): DEVICE plane of (product of the other two extents) doubles, x fastest among the
  * remaining indices (dir 0: j + ny*k; dir 1: i + nx*k; dir 2: i + nx*j), 16-byte aligned, or NULL to

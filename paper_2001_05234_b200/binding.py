@@ -25,7 +25,7 @@ MAX_KERNEL_RECORDS = 16      # CANS_MAX_KERNEL_RECORDS of the header
 
 EXPORTED_SYMBOLS = (
     "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
-    "cans_projection_step", "cans_chkdt", "cans_helmholtz_plan_create", "cans_helmholtz_solve",
+    "cans_projection_step", "cans_chkdt", "cans_chkdt_static", "cans_helmholtz_plan_create", "cans_helmholtz_solve",
     "cans_probe_fp64_fma", "cans_probe_tile_copy",
     "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
@@ -81,6 +81,8 @@ def _load() -> ctypes.CDLL:
     lib.cans_projection_step.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_double, vp, vp]
     lib.cans_chkdt.restype = i32
     lib.cans_chkdt.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.cans_chkdt_static.restype = i32
+    lib.cans_chkdt_static.argtypes = [i32, i32, i32, dbl, dbl, dbl, ctypes.c_char_p] + [vp] * 10
     lib.cans_plan_set_profiling.restype = i32
     lib.cans_plan_set_profiling.argtypes = [vp, i32]
     lib.cans_plan_kernel_times.restype = i32
@@ -136,6 +138,29 @@ def probe_fp64_fma(stream=None) -> float:
     out = ctypes.c_double(0.0)
     _check(_lib.cans_probe_fp64_fma(ctypes.byref(out), _stream_ptr(stream)))
     return float(out.value)
+
+
+STATIC_MAX_NZ = 1024         # CANS_STATIC_MAX_NZ
+STATIC_MAX_CTAS = 65536      # CANS_STATIC_MAX_CTAS
+
+
+def chkdt_static(u, v, w, dti, lx: float, ly: float, lz: float, bc, dzc=None, dzf=None, faces=None, stream=None):
+    """cans_chkdt_static: the chkdt reduction without a plan and without any device allocation inside the library -- for
+    a caller whose own pool already holds all of the GPU's memory, or whose other streams must not stall behind a
+    cudaMalloc / cudaFree.  The scratch is a fixed 528 KB array in the library image, shared by all calls: calls that may
+    overlap on the GPU race.  u, v, w: CUDA float64 tensors (nz, ny, nx); dzc / dzf: CUDA float64 tensors of nz+1 / nz
+    entries or both None (uniform); faces: {direction: lower-face plane tensor} (required on lower 'D' sides);
+    dti: one-element CUDA float64 tensor, overwritten.  Grids beyond the fixed array raise CansError (status 3)."""
+    nz, ny, nx = u.shape
+    shape = (nz, ny, nx)
+    faces = faces or {}
+    want = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+    fptr = [None if faces.get(d) is None else _dev_ptr(faces[d], want[d]) for d in range(3)]
+    _check(_lib.cans_chkdt_static(nx, ny, nz, float(lx), float(ly), float(lz), _bc_bytes(bc),
+                                  None if dzc is None else _dev_ptr(dzc, (nz + 1,)),
+                                  None if dzf is None else _dev_ptr(dzf, (nz,)),
+                                  _dev_ptr(u, shape), _dev_ptr(v, shape), _dev_ptr(w, shape),
+                                  fptr[0], fptr[1], fptr[2], _dev_ptr(dti, (1,)), _stream_ptr(stream)))
 
 
 class PoissonPlan:

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libcans_poisson.so")
-SOURCES = ["xw_kernels.cu", "yt_kernels.cu", "cans_poisson.cu", "z_solve.cu", "probes.cu",
+SOURCES = ["xw_kernels.cu", "yt_kernels.cu", "cans_poisson.cu", "z_solve.cu", "probes.cu", "chkdt_static.cu",
            "xy_group_a.cu", "xy_group_b.cu", "xy_group_c.cu", "xy_group_d.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -30,6 +30,7 @@
 #include "xw_kernels.cuh"
 #include "yt_kernels.cuh"
 #include "probes.cuh"
+#include "errors.hpp"
 
 namespace cans {
 
@@ -44,6 +45,10 @@ static int fail(int code, const std::string& msg) {
 static int fail_cuda(cudaError_t e, const char* where) {
     return fail(CANS_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
 }
+// the same for the other translation units (errors.hpp)
+void report_ok() { g_status = CANS_OK; }
+int report_failure(int code, const char* message) { return fail(code, message); }
+int report_cuda_failure(cudaError_t e, const char* where) { return fail_cuda(e, where); }
 
 // ------------------------------------------------------------------------------------------------
 // a7: velocity correction u -= dt G Phi (eq. 2c).  A thread owns one pair of x-adjacent cells of a row
@@ -133,21 +138,6 @@ __device__ __forceinline__ RowLoad chk_fetch(const ChkStream& s) {
 __device__ __forceinline__ void chk_advance(ChkStream& s, long ps, long es) {
     if (s.p) s.p += ps;
     if (s.e) s.e += es;
-}
-
-__device__ __forceinline__ double chk_cell_max(const ChkArgs& a, int k, const Row3& uj, const Row3& up, const Row3& un, const Row3& vm,
-                                               const Row3& vj, const Row3& vmn, const Row3& vjn, const Row3& wlj, const Row3& wlp,
-                                               const Row3& wj, const Row3& wp) {
-    const double qx = 0.25 * a.rdx, qy = 0.25 * a.rdy;
-    const double rzf = a.rdzf[k], rzc = a.rdzc[k], qz = 0.25 * rzf;
-    // cell i (values .a / .b of the v, w rows; .b of the u rows) and cell i+1 (.b / .c; .c)
-    const double dtix0 = fabs(uj.b) * a.rdx + fabs(vj.a + vm.a + vj.b + vm.b) * qy + fabs(wj.a + wlj.a + wj.b + wlj.b) * qz;
-    const double dtix1 = fabs(uj.c) * a.rdx + fabs(vj.b + vm.b + vj.c + vm.c) * qy + fabs(wj.b + wlj.b + wj.c + wlj.c) * qz;
-    const double dtiy0 = fabs(uj.b + up.b + up.a + uj.a) * qx + fabs(vj.a) * a.rdy + fabs(wj.a + wp.a + wlp.a + wlj.a) * qz;
-    const double dtiy1 = fabs(uj.c + up.c + up.b + uj.b) * qx + fabs(vj.b) * a.rdy + fabs(wj.b + wp.b + wlp.b + wlj.b) * qz;
-    const double dtiz0 = fabs(uj.b + uj.a + un.a + un.b) * qx + fabs(vj.a + vm.a + vmn.a + vjn.a) * qy + fabs(wj.a) * rzc;
-    const double dtiz1 = fabs(uj.c + uj.b + un.b + un.c) * qx + fabs(vj.b + vm.b + vmn.b + vjn.b) * qy + fabs(wj.b) * rzc;
-    return fmax(fmax(dtix0, dtix1), fmax(fmax(dtiy0, dtiy1), fmax(dtiz0, dtiz1)));
 }
 
 __global__ void __launch_bounds__(256, 2) chkdt_kernel(const ChkArgs a) {

@@ -100,6 +100,21 @@ CANS_D RowLoad chk_load_w(const ChkArgs& a, int i, int jj, int kk, int lane) {
     }
     return chk_load_row(row, i, a.nx, a.wrap_x, lane);
 }
+// the six face sums of the pair of cells (i, i+1) of plane k from the eleven rows a thread holds; returns their maximum
+CANS_D double chk_cell_max(const ChkArgs& a, int k, const Row3& uj, const Row3& up, const Row3& un, const Row3& vm,
+                            const Row3& vj, const Row3& vmn, const Row3& vjn, const Row3& wlj, const Row3& wlp,
+                            const Row3& wj, const Row3& wp) {
+    const double qx = 0.25 * a.rdx, qy = 0.25 * a.rdy;
+    const double rzf = a.rdzf[k], rzc = a.rdzc[k], qz = 0.25 * rzf;
+    // cell i (values .a / .b of the v, w rows; .b of the u rows) and cell i+1 (.b / .c; .c)
+    const double dtix0 = fabs(uj.b) * a.rdx + fabs(vj.a + vm.a + vj.b + vm.b) * qy + fabs(wj.a + wlj.a + wj.b + wlj.b) * qz;
+    const double dtix1 = fabs(uj.c) * a.rdx + fabs(vj.b + vm.b + vj.c + vm.c) * qy + fabs(wj.b + wlj.b + wj.c + wlj.c) * qz;
+    const double dtiy0 = fabs(uj.b + up.b + up.a + uj.a) * qx + fabs(vj.a) * a.rdy + fabs(wj.a + wp.a + wlp.a + wlj.a) * qz;
+    const double dtiy1 = fabs(uj.c + up.c + up.b + uj.b) * qx + fabs(vj.b) * a.rdy + fabs(wj.b + wp.b + wlp.b + wlj.b) * qz;
+    const double dtiz0 = fabs(uj.b + uj.a + un.a + un.b) * qx + fabs(vj.a + vm.a + vmn.a + vjn.a) * qy + fabs(wj.a) * rzc;
+    const double dtiz1 = fabs(uj.c + uj.b + un.b + un.c) * qx + fabs(vj.b + vm.b + vmn.b + vjn.b) * qy + fabs(wj.b) * rzc;
+    return fmax(fmax(dtix0, dtix1), fmax(fmax(dtiy0, dtiy1), fmax(dtiz0, dtiz1)));
+}
 #endif
 
 }  // namespace cans
