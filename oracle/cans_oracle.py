@@ -416,13 +416,17 @@ def chkdt_fields(u, v, w, lx, ly, lz, bc, dzc=None, dzf=None, lower_face=None):
 
     def pad3(a, comp):
         a = _pad_velocity(a, 2, px, comp == 0, lower_face.get(0))
-        # the planes registered for y and z have the extent of the unpadded field: pad them with zeros along x
+        # the planes registered for y and z have the extent of the unpadded field: they get the same layers along the
+        # directions already padded -- wrapped where that direction is periodic (the plane is a layer of the same periodic
+        # field, reading S18 "wrapped when periodic"), 0 otherwise (a tangential value beyond a wall)
+        wrap_x, wrap_y = ("wrap" if px == "PP" else "constant"), ("wrap" if py == "PP" else "constant")
         fy, fz = lower_face.get(1), lower_face.get(2)
         if fy is not None:
-            fy = np.pad(np.asarray(fy, dtype=np.float64).reshape(nz, 1, nx), ((0, 0), (0, 0), (1, 1)))
+            fy = np.pad(np.asarray(fy, dtype=np.float64).reshape(nz, 1, nx), ((0, 0), (0, 0), (1, 1)), mode=wrap_x)
         a = _pad_velocity(a, 1, py, comp == 1, fy if comp == 1 else None)
         if fz is not None:
-            fz = np.pad(np.asarray(fz, dtype=np.float64).reshape(1, ny, nx), ((0, 0), (1, 1), (1, 1)))
+            fz = np.pad(np.asarray(fz, dtype=np.float64).reshape(1, ny, nx), ((0, 0), (0, 0), (1, 1)), mode=wrap_x)
+            fz = np.pad(fz, ((0, 0), (1, 1), (0, 0)), mode=wrap_y)
         a = _pad_velocity(a, 0, pz, comp == 2, fz if comp == 2 else None)
         return a                                    # index [k+1, j+1, i+1] = cell (i, j, k)
 

@@ -587,6 +587,34 @@ def test_chkdt_boundaries():
     assert fx[1, 2, nx - 1] == 0.5 / dy and fx[1, 2, 0] == 1.0 / dy and fx[1, 0, 0] == 0.5 / dy
 
 
+def test_chkdt_is_invariant_under_shifts_along_periodic_directions():
+    """A periodic direction has no origin: rolling every field AND every registered lower-face plane along it rolls the
+    three per-face sums and leaves the maximum unchanged.  This holds whatever the other directions are, so it pins how
+    a lower-face plane of a wall direction is continued along a periodic one (reading S18: wrapped) -- a plane padded
+    with zeros there breaks the invariance at the cells next to the wrap."""
+    nz, ny, nx = 5, 6, 8
+    lx, ly, lz = 3.0, 2.5, 2.0
+    rng = np.random.default_rng(17)
+    cases = [((("P", "P"), ("D", "N"), ("N", "D")), (2,)),            # x periodic; planes in y ('D') and z (inflow on 'N')
+             ((("P", "P"), ("P", "P"), ("D", "D")), (2, 1)),          # x, y periodic; plane in z
+             ((("N", "N"), ("P", "P"), ("D", "N")), (1,)),            # y periodic; planes in x (inflow) and z
+             ((("D", "D"), ("N", "D"), ("P", "P")), (0,))]            # z periodic (uniform grid); planes in x and y
+    shapes = {0: (nz, ny, 1), 1: (nz, 1, nx), 2: (1, ny, nx)}
+    for bc, axes in cases:
+        u, v, w = (rng.standard_normal((nz, ny, nx)) for _ in range(3))
+        faces = {d: rng.standard_normal(shapes[d]) for d in range(3) if bc[d][0] != "P"}
+        ref_fields = orc.chkdt_fields(u, v, w, lx, ly, lz, bc, None, None, faces)
+        ref = orc.chkdt(u, v, w, lx, ly, lz, bc, None, None, faces)
+        for axis in axes:                       # numpy axis: 2 = x, 1 = y, 0 = z
+            for s in (1, 3):
+                ur, vr, wr = (np.roll(a, s, axis=axis) for a in (u, v, w))
+                fr = {d: np.roll(f, s, axis=axis) for d, f in faces.items()}       # (extent 1 along its own direction)
+                got_fields = orc.chkdt_fields(ur, vr, wr, lx, ly, lz, bc, None, None, fr)
+                for g, r in zip(got_fields, ref_fields):
+                    assert np.array_equal(g, np.roll(r, s, axis=axis)), (bc, axis, s)
+                assert orc.chkdt(ur, vr, wr, lx, ly, lz, bc, None, None, fr) == ref
+
+
 # ----------------------------------------------------------------------------------------------
 # NEXT row f4: the Helmholtz solve of eq. 3b (P:L73, P:L106), cell-centred and with the unknown on the z faces
 # ----------------------------------------------------------------------------------------------
