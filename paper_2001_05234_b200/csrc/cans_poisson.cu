@@ -166,8 +166,12 @@ __global__ void __launch_bounds__(256, 2) chkdt_kernel(const ChkArgs a) {
         const int kfast = (k1 < a.nz) ? k1 : a.nz - 1;     // steps [k0, kfast) have their k+1 plane inside the field
         // Fast path (warp-uniform): every neighbour row of this warp is a stored row (inside or wrapped) and every value
         // beyond a lane's pair is a stored value -- one running offset and four per-thread deltas address everything.
+        // Only when a warp lies inside one row (nx/2 a multiple of 32): then j and the row ends are the same for all its
+        // lanes, the branch is warp-uniform (it contains shuffles) and lanes 0 / 31 are the only ones whose outer value the
+        // neighbouring lane cannot supply.  Narrower rows take the general loaders, which test i itself.
         const int i_first = i - 2 * lane;
-        const bool fast = (a.wrap_y || (j > 0 && j + 1 < a.ny)) && (a.wrap_x || (i_first > 0 && i_first + 64 < a.nx));
+        const bool fast = (hx % 32 == 0) && (a.wrap_y || (j > 0 && j + 1 < a.ny)) &&
+                          (a.wrap_x || (i_first > 0 && i_first + 64 < a.nx));
         if (fast) {
             const long d_up = (j + 1 < a.ny) ? (long)a.nx : -(long)(a.ny - 1) * a.nx;      // row j+1 (or row 0)
             const long d_vm = (j > 0) ? -(long)a.nx : (long)(a.ny - 1) * a.nx;             // row j-1 (or row ny-1)

@@ -104,6 +104,60 @@ def test_chkdt_localised_maxima_at_every_kind_of_boundary(B, bcs):
     plan.close()
 
 
+@pytest.mark.parametrize("path", ["planned", "static"])
+@pytest.mark.parametrize("nx", [16, 32, 48, 96])
+def test_chkdt_rows_shorter_than_a_warp(B, nx, path):
+    """nx / 2 < 32 or not a multiple of 32: a warp of the chkdt kernels holds several rows (or a row and a part), so a row
+    starts and ends in the middle of a warp.  The value beyond a lane's pair must then come from the boundary rule of the
+    lane's own row, not from the neighbouring lane (which holds another row).  The maximum is planted at the first and last
+    cells of rows that start inside a warp, with periodic x (the wrapped value) and with walls in x, next to periodic and
+    non-periodic y; both the planned kernel and the plan-free one (cans_chkdt_static) are checked against the oracle."""
+    ny, nz = 16, 5
+    hx = nx // 2
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, 1.6)
+    dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    rows = [j for j in range(ny) if (j * hx) % 32 != 0][:3] + [j for j in range(ny) if (j * hx) % 32 != 0][-2:]
+    rows = sorted(set(rows + [0, ny - 1]))
+    spots = [(i, j, k) for i in (0, 1, nx - 2, nx - 1) for j in rows for k in (0, 2, nz - 1)]
+    for bcs in ("PP/PP/PP", "PP/NN/DD", "PP/DN/NN", "NN/PP/PP", "DN/ND/ND"):
+        px, py, pz = bcs.split("/")
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        rng = np.random.default_rng(nx + len(bcs))
+        faces = _faces(rng, bc, (nz, ny, nx), inflow=tuple(d for d in range(3) if bc[d][0] == "N"))
+        for f in faces.values():
+            f *= 1e-3
+        fd = {d: torch.from_numpy(f.copy()).cuda() for d, f in faces.items()}
+        plan = None
+        if path == "planned":
+            plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+            for d, t in fd.items():
+                plan.set_lower_face(d, t)
+        dzc_d, dzf_d = dzc_t.cuda(), dzf_t.cuda()
+        dti = torch.zeros((1,), dtype=torch.float64, device="cuda")
+        base = [1e-3 * rng.standard_normal((nz, ny, nx)) for _ in range(3)]
+        for (i, j, k) in spots:
+            fields = [b.copy() for b in base]
+            for f in fields:         # O(1) values in the cell and its neighbours along x, wrapped where x is periodic
+                for di in (-1, 0, 1):
+                    ii = i + di
+                    if bc[0][0] == "P":
+                        ii %= nx
+                    if 0 <= ii < nx:
+                        f[k, j, ii] = rng.uniform(0.5, 1.5) * rng.choice((-1.0, 1.0))
+            u, v, w = fields
+            ud, vd, wd = (torch.from_numpy(a).cuda() for a in (u, v, w))
+            if plan is not None:
+                plan.chkdt(ud, vd, wd, dti)
+            else:
+                B.chkdt_static(ud, vd, wd, dti, lx, ly, lz, bc, dzc_d, dzf_d, fd)
+            torch.cuda.synchronize()
+            want = orc.chkdt(u, v, w, lx, ly, lz, bc, dzc, dzf, faces)
+            assert abs(float(dti[0]) - want) <= 1e-13 * want, (bcs, (i, j, k), float(dti[0]), want)
+        if plan is not None:
+            plan.close()
+
+
 def test_chkdt_special_values_and_errors(B):
     nx, ny, nz = 32, 16, 8
     bc = (("P", "P"), ("P", "P"), ("N", "N"))
