@@ -20,8 +20,10 @@
  * +y face, w on the +z face.  Out-of-range neighbours are synthesised from `bc`.
  *
  * Threading: calls only enqueue work on `stream` (a cudaStream_t passed as void*) and never
- * synchronise.  A plan is immutable after creation apart from the registered lower-face planes;
- * it may be used by one stream at a time.  No function throws or prints.
+ * synchronise.  A plan is immutable after creation apart from the registered lower-face planes, the cached
+ * tensor maps of the last field and (Helmholtz) the pivot table of the last alpha, which calls rewrite on their
+ * stream: a plan may be used by ONE stream at a time -- for work that overlaps (u, v, w Helmholtz solves next to
+ * a Poisson solve) create one plan per stream.  No function throws or prints.
  */
 #ifndef CANS_POISSON_H
 #define CANS_POISSON_H
@@ -112,7 +114,8 @@ int cans_poisson_solve(cans_poisson_plan* plan, double* p, void* stream);
  * cans_projection -- one pressure-projection step, eqs. 2b-2c:
  *     f = D(u,v,w)/dt ;  L Phi = f ;  (u,v,w) -= dt * G Phi.
  *   u, v, w  DEVICE, corrected in place.
- *   p        DEVICE, overwritten with Phi (entry contents ignored; eq. 2d is the caller's).
+ *   p        DEVICE, overwritten with Phi (entry contents ignored; eq. 2d is the caller's).  u, v, w, p must be four
+ *            distinct arrays (CANS_ERR_INVALID_ARG otherwise).
  *   dt       the whole factor gamma_k*Delta_t of eqs. 2b-2c (> 0).
  * The boundary-normal velocity on a lower 'P' face is the wrapped value, on a lower 'N' face 0
  * (or the plane registered with cans_projection_set_lower_face), on a lower 'D' face the registered plane
@@ -125,7 +128,7 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
 /*
  * cans_projection_step -- cans_projection plus the two bandwidth-only steps a time loop runs after it:
  *   p_acc   DEVICE or NULL: the accumulated pressure; eq. 2d  p_acc += Phi  is done by the correction kernel itself
- *           (the same pass that applies eq. 2c: +16 B/cell instead of a separate 24 B/cell sweep).  Must not alias p.
+ *           (the same pass that applies eq. 2c: +16 B/cell instead of a separate 24 B/cell sweep).  Must not alias p, u, v, w.
  *   dti     DEVICE scalar (one double) or NULL: receives the reduction of Listing 1 (`chkdt`; eq. 4)
  *           over the CORRECTED velocities, see cans_chkdt.
  * Everything else as cans_projection (which is this call with p_acc = dti = NULL).
@@ -199,6 +202,8 @@ int cans_projection_set_lower_face(cans_poisson_plan* plan, int dir, double* fac
  * Host-buffer convenience entry points (used for end-to-end timing): copy the HOST arrays to
  * device buffers owned by the plan (allocated on first use), run the device path on `stream`,
  * copy the results back and synchronise the stream.  Pinned host memory gives full PCIe rate.
+ * Only the four fields travel: lower-face planes registered with cans_projection_set_lower_face stay DEVICE pointers
+ * here too -- they are read, and on 'D' sides corrected, where they are; the caller copies them if it wants them.
  */
 int cans_poisson_solve_host(cans_poisson_plan* plan, double* p_host, void* stream);
 int cans_projection_host(cans_poisson_plan* plan, double* u_host, double* v_host, double* w_host,
@@ -223,21 +228,6 @@ int cans_plan_launches_per_projection(const cans_poisson_plan* plan);
 int cans_plan_set_profiling(cans_poisson_plan* plan, int enable);
 int cans_plan_kernel_times(cans_poisson_plan* plan, float* ms, int capacity);
 const char* cans_plan_kernel_name(const cans_poisson_plan* plan, int idx);
-
-/*
- * Measurement probes for bench.py -- the denominators kernel numbers are read against.  Both synchronise the stream.
- *   cans_probe_fp64_fma   FP64 FMA instructions per second of the current device (independent chains on every SM): the
- *                         measured peak of the plain FP64 pipe.
- *   cans_probe_tile_copy  duration (ms) of a bare in-place TMA copy -- tile in, tile out, no arithmetic, data unchanged --
- *                         of the field p (DEVICE, nx*ny*nz doubles) with exactly the tiles of the z solve (which = 0:
- *                         16 / 32 / 8 columns x nz rows) or of the TMA-fed y transforms (which = 1: 16 doubles x ny rows,
- *                         ny = 512, 768 only): the HBM ceiling of that access pattern.  which = 2: the z view with tiles of
- *                         32 columns x 256 rows -- the same plane-strided rows, twice as wide (every row of a z tile lies
- *                         in another 2 MB page: the rate follows the bytes moved per row).
- *                         2*8*N bytes move per call.
- */
-int cans_probe_fp64_fma(double* fma_per_s, void* stream);
-int cans_probe_tile_copy(cans_poisson_plan* plan, double* p, int which, float* ms, void* stream);
 
 /* "x.y" version string of the library. */
 const char* cans_version(void);

@@ -1,10 +1,11 @@
 """Build libcans_poisson.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
 Usage: ``python -m paper_2001_05234_b200.build [--force]`` or ``build()`` from Python.
-The five translation units compile in parallel; objects go to ``csrc/build/``.
+The translation units compile in parallel; objects go to ``csrc/build/``.
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import shutil
 import subprocess
@@ -30,22 +31,35 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found: the CUDA toolkit is required to build libcans_poisson.so")
 
 
-def _newest_source_mtime() -> float:
-    m = 0.0
+def _source_digest() -> str:
+    """SHA-256 over the names and contents of every file the library is built from (csrc/*, include/*) and the flags."""
+    h = hashlib.sha256(" ".join(NVCC_FLAGS[:-1]).encode())
     for d in (CSRC, os.path.join(ROOT, "include")):
-        for fn in os.listdir(d):
+        for fn in sorted(os.listdir(d)):
             p = os.path.join(d, fn)
             if os.path.isfile(p):
-                m = max(m, os.path.getmtime(p))
-    return m
+                h.update(fn.encode())
+                with open(p, "rb") as fh:
+                    h.update(fh.read())
+    return h.hexdigest()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source_mtime():
+    """Rebuild unless the library exists and was built from exactly these sources (a digest of their contents, kept beside
+    the objects -- modification times say nothing after a checkout)."""
+    digest = _source_digest()
+    stamp = os.path.join(CSRC, "build", "sources.sha256")
+    if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read().strip() == digest:
         return LIB
     nvcc = _nvcc()
     bdir = os.path.join(CSRC, "build")
     os.makedirs(bdir, exist_ok=True)
+    keep = {src.replace(".cu", ".o") for src in SOURCES}
+    for fn in os.listdir(bdir):             # objects and logs of sources that no longer exist
+        if (fn.endswith(".o") and fn not in keep) or (fn.endswith(".o.log") and fn[:-4] not in keep):
+            os.remove(os.path.join(bdir, fn))
+    if os.path.exists(stamp):
+        os.remove(stamp)
 
     def compile_one(src):
         obj = os.path.join(bdir, src.replace(".cu", ".o"))
@@ -63,6 +77,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    with open(stamp, "w") as fh:
+        fh.write(digest + "\n")
     if verbose:
         print("built", LIB)
     return LIB

@@ -14,6 +14,7 @@
 // once over all planes -- per-batch launches through L2 were measured and are slower (profiles/r02a_plane_batching.md).
 #include <cuda_runtime.h>
 
+#include <cmath>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -22,6 +23,7 @@
 #include <vector>
 
 #include "../../include/cans_poisson.h"
+#include "../../include/cans_poisson_probe.h"
 #include "plan_tables.hpp"
 #include "xy_kernels.cuh"
 #include "z_kernels.cuh"
@@ -494,7 +496,7 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     }
     const int nseg = (nz + Z_MROWS - 1) / Z_MROWS;
     if (nseg > 64) { fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the z-solve tiling (max 1024)"); return nullptr; }
-    if (z_solve_smem_bytes(nseg, bc[2][0] == 'P') > Z_SMEM_LIMIT) {
+    if (z_solve_smem_bytes(nseg) > Z_SMEM_LIMIT) {
         fail(CANS_ERR_UNSUPPORTED_SIZE, "nz too large for the z-solve tiling (shared memory)");
         return nullptr;
     }
@@ -503,6 +505,12 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     for (int k = 0; k <= nz; ++k) hdzc[k] = dzc ? dzc[k] : lz / nz;
     for (int k = 0; k < nz; ++k) if (!(hdzf[k] > 0.0)) { fail(CANS_ERR_INVALID_ARG, "dzf must be positive"); return nullptr; }
     for (int k = 0; k <= nz; ++k) if (!(hdzc[k] > 0.0)) { fail(CANS_ERR_INVALID_ARG, "dzc must be positive"); return nullptr; }
+    if (bc[2][0] == 'P' && std::fabs(hdzc[0] - hdzc[nz]) > 1e-12 * (hdzc[0] + hdzc[nz])) {
+        // dzc[0] and dzc[nz] are the same distance (last centre to first centre through the wrap): two values would give a
+        // gradient and a divergence that do not compose to the Laplacian, i.e. a projection that is not divergence free
+        fail(CANS_ERR_INVALID_ARG, "periodic z needs a single-valued wrap spacing: dzc[0] == dzc[nz]");
+        return nullptr;
+    }
 
     cans_poisson_plan* pl = new (std::nothrow) cans_poisson_plan();
     if (!pl) { fail(CANS_ERR_ALLOC, "host allocation failed"); return nullptr; }
@@ -583,13 +591,11 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
         e = z_setup_launch(z, pl->rstart, pl->r00, 0);
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
     }
-    const int rc = CANS_OK;
     if (e == cudaSuccess) e = z_solve_configure(nseg, pl->cyclic, pl->num_sms, &pl->z_grid, &pl->z_smem);
     if (e == cudaSuccess) e = configure_kernels(pl);
-    if (e != cudaSuccess || rc != CANS_OK) {
-        const bool oom = (e == cudaErrorMemoryAllocation);
-        std::string msg = (rc != CANS_OK) ? g_err : std::string("plan creation: ") + cudaGetErrorString(e);
-        const int code = (rc != CANS_OK) ? rc : (oom ? CANS_ERR_ALLOC : CANS_ERR_CUDA);
+    if (e != cudaSuccess) {
+        const std::string msg = std::string("plan creation: ") + cudaGetErrorString(e);
+        const int code = (e == cudaErrorMemoryAllocation) ? CANS_ERR_ALLOC : CANS_ERR_CUDA;
         cans_poisson_plan_destroy(pl);
         cudaGetLastError();
         fail(code, msg);
@@ -730,8 +736,10 @@ int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* 
     g_status = CANS_OK;
     if (!plan || !u || !v || !w || !p) return fail(CANS_ERR_INVALID_ARG, "plan, u, v, w, p must be non-NULL");
     if (plan->stagger == 2) return fail(CANS_ERR_INVALID_ARG, "a plan for an unknown on the z faces solves cans_helmholtz_solve only");
-    if (p_acc && ((reinterpret_cast<size_t>(p_acc) & 15) != 0 || p_acc == p))
-        return fail(CANS_ERR_INVALID_ARG, "p_acc must be 16-byte aligned and distinct from p");
+    if (p_acc && ((reinterpret_cast<size_t>(p_acc) & 15) != 0 || p_acc == p || p_acc == u || p_acc == v || p_acc == w))
+        return fail(CANS_ERR_INVALID_ARG, "p_acc must be 16-byte aligned and distinct from p, u, v, w");
+    if (p == u || p == v || p == w || u == v || u == w || v == w)
+        return fail(CANS_ERR_INVALID_ARG, "u, v, w, p must be four distinct arrays (p is overwritten while u, v, w are still read)");
     if (!(dt > 0.0)) return fail(CANS_ERR_INVALID_ARG, "dt must be > 0");
     if (((reinterpret_cast<size_t>(p) | reinterpret_cast<size_t>(u) | reinterpret_cast<size_t>(v) |
           reinterpret_cast<size_t>(w)) & 15) != 0)

@@ -49,15 +49,9 @@ CANS_HD double2 ld_p2(const double* p) {
 #endif
 }
 
-// 16-byte load of data that is streamed once (u, v, w of the fused divergence): L2 only, so that the small twiddle
-// tables keep their place in L1
-CANS_HD double2 ldg_stream2(const double* p) {
-#if defined(__CUDA_ARCH__)
-    return *reinterpret_cast<const double2*>(p);   // TEST: plain
-#else
-    return *reinterpret_cast<const double2*>(p);
-#endif
-}
+// 16-byte load of data that is streamed once (u, v, w of the fused divergence).  A plain load: the L2-only variants
+// (ld.global.cg / .cs) were measured on the C5 grid and changed nothing, the twiddle tables stay in L1 either way.
+CANS_HD double2 ldg_stream2(const double* p) { return *reinterpret_cast<const double2*>(p); }
 
 // Transform kind of one direction (pressure boundary pair), see DESIGN.md "Transforms".
 // KIND_ND / KIND_DN: the mixed pairs (lower Neumann, upper Dirichlet and the reverse), DCT-IV / DST-IV.

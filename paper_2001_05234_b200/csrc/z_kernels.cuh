@@ -11,8 +11,9 @@ constexpr int Z_MROWS = 16;   // rows per thread in the z solve
 // columns per CTA for a given segment count (threads = TC * nseg <= 512)
 inline int z_tc_for(int nseg) { return nseg <= 16 ? 32 : (nseg <= 32 ? 16 : 8); }
 
-// dynamic shared memory of the solve kernel (the periodic-z kernel keeps a third tile buffer); host arithmetic only
-size_t z_solve_smem_bytes(int nseg, int cyclic);
+// dynamic shared memory of the solve kernel (two tile buffers + tables; the periodic-z kernel parks its correction vector
+// in the tile's own staging buffer and needs no more); host arithmetic only
+size_t z_solve_smem_bytes(int nseg);
 constexpr size_t Z_SMEM_LIMIT = 227u * 1024u;
 // plan time: opt in to the dynamic shared memory of the solve kernel and compute the persistent grid
 cudaError_t z_solve_configure(int nseg, int cyclic, int num_sms, int* grid_out, size_t* smem_out);   // cudaErrorInvalidConfiguration: the tile buffers do not fit

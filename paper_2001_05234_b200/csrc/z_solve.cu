@@ -135,7 +135,7 @@ static cudaError_t configure_tc(int nseg, int num_sms, int* grid_out, size_t* sm
     return cudaSuccess;
 }
 
-size_t z_solve_smem_bytes(int nseg, int cyclic) {
+size_t z_solve_smem_bytes(int nseg) {
     switch (z_tc_for(nseg)) {
         case 32: return sizeof(double) * ZPass<Z_MROWS, 32>::smem_doubles(nseg);
         case 16: return sizeof(double) * ZPass<Z_MROWS, 16>::smem_doubles(nseg);

@@ -22,9 +22,15 @@ def binding():
 
 
 def declared_functions():
-    txt = open(HEADER).read()
-    txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(cans_[a-z0-9_]+)\s*\(", txt)))
+    """Every function declared in include/*.h (the API header and the probe header)."""
+    names = set()
+    inc = os.path.dirname(HEADER)
+    for fn in sorted(os.listdir(inc)):
+        if fn.endswith(".h"):
+            txt = open(os.path.join(inc, fn)).read()
+            txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
+            names.update(re.findall(r"\b(cans_[a-z0-9_]+)\s*\(", txt))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported(binding):
@@ -53,6 +59,8 @@ PP_NN = (("P", "P"), ("P", "P"), ("N", "N"))
     (dict(nx=40, ny=32, nz=32), 3),                                                # 40 = 2^3*5
     (dict(nx=32, ny=32, nz=2000), 3),
     (dict(nx=32, ny=32, nz=4, dzf=[0.5, 0.5, -0.5, 0.5], dzc=[0.5] * 5), 1),
+    # periodic z: the wrap spacing dzc[0] = dzc[nz] must be single-valued
+    (dict(nx=32, ny=32, nz=4, bc=(("P", "P"), ("P", "P"), ("P", "P")), dzf=[0.2, 0.3, 0.3, 0.2], dzc=[0.2, 0.25, 0.3, 0.25, 0.21]), 1),
 ])
 def test_plan_create_rejects_bad_arguments_without_a_gpu(binding, kwargs, status):
     args = dict(nx=32, ny=32, nz=32, lx=1.0, ly=1.0, lz=1.0, bc=PP_NN, dzc=None, dzf=None)

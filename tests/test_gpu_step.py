@@ -178,6 +178,21 @@ def test_chkdt_special_values_and_errors(B):
     pland.close()
 
 
+def test_projection_rejects_aliased_fields(B):
+    """p is overwritten with the divergence while u, v, w are still being read, and p_acc is updated next to them: any two
+    of the arrays being the same memory would silently corrupt the step."""
+    nx, ny, nz = 32, 16, 8
+    plan = B.PoissonPlan(nx, ny, nz, 1.0, 1.0, 1.0, (("P", "P"), ("P", "P"), ("N", "N")))
+    u, v, w, p, pa = (torch.zeros((nz, ny, nx), dtype=torch.float64, device="cuda") for _ in range(5))
+    for args, kw in (((u, v, w, u), {}), ((u, v, w, w), {}), ((u, u, w, p), {}), ((u, v, w, p), {"p_acc": v}), ((u, v, w, p), {"p_acc": p})):
+        with pytest.raises(B.CansError) as ei:
+            plan.projection_step(*args, 1e-3, **kw)
+        assert ei.value.status == B.CANS_ERR_INVALID_ARG
+    plan.projection_step(u, v, w, p, 1e-3, p_acc=pa)          # five distinct arrays are accepted
+    torch.cuda.synchronize()
+    plan.close()
+
+
 @pytest.mark.parametrize("nx,ny,nz,bcs", [(96, 64, 40, ("PP", "PP", "NN")), (512, 32, 9, ("NN", "DN", "ND")),
                                           (48, 768, 6, ("ND", "PP", "PP")), (1024, 32, 4, ("PP", "NN", "DD"))])
 def test_projection_step_fuses_eq_2d_and_returns_chkdt(B, nx, ny, nz, bcs):

@@ -494,6 +494,12 @@ def test_pressure_update_is_a_plain_sum():
     p, phi = rng.standard_normal((3, 4, 5)), rng.standard_normal((3, 4, 5))
     out = orc.pressure_update(p, phi)
     assert np.array_equal(out, p + phi) and out is not p
+    # by hand (eq. 2d): constant fields 2.5 and -0.75 give 1.75 everywhere; a single cell 3 + 4 = 7
+    a, b = np.full((2, 3, 4), 2.5), np.full((2, 3, 4), -0.75)
+    assert np.all(orc.pressure_update(a, b) == 1.75)
+    a[1, 2, 3], b[1, 2, 3] = 3.0, 4.0
+    out = orc.pressure_update(a, b)
+    assert out[1, 2, 3] == 7.0 and out[0, 0, 0] == 1.75 and a[1, 2, 3] == 3.0
 
 
 def test_chkdt_of_uniform_flow():
