@@ -21,7 +21,7 @@
  *
  * Threading: calls only enqueue work on `stream` (a cudaStream_t passed as void*) and never
  * synchronise.  A plan is immutable after creation apart from the registered lower-face planes, the cached
- * tensor maps of the last field and (Helmholtz) the pivot table of the last alpha, which calls rewrite on their
+ * tensor maps of the last field and (Helmholtz) the pivot tables per alpha, which calls rewrite on their
  * stream: a plan may be used by ONE stream at a time -- for work that overlaps (u, v, w Helmholtz solves next to
  * a Poisson solve) create one plan per stream.  No function throws or prints.
  */
@@ -89,10 +89,13 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz,
  *            face-located case (non-periodic x or y: node-based DST-I / DCT-I; z pairs containing 'N') returns NULL with
  *            CANS_ERR_UNSUPPORTED_BC.
  *   q        DEVICE, nx*ny*nz doubles: f on entry, Phi on exit.     alpha < 0.
- * The pivots entering each z segment depend on alpha: the plan rebuilds that table (N/16 doubles, one extra kernel on the
- * caller's stream) whenever alpha differs from the previous call's; a time loop with the three RK3 values gamma_k should
- * keep one plan per substep and component, or accept the rebuild.  A stagger = 2 plan serves cans_helmholtz_solve only.
+ * The pivots entering each z segment depend on alpha: the plan keeps up to CANS_MAX_PIVOT_TABLES tables (N/16 doubles each;
+ * the first, for alpha = 0, from plan creation) and builds one -- one device allocation and one extra kernel on the caller's
+ * stream -- the first time it meets a new alpha.  The three gamma_k of an RK3 loop therefore cost three builds in the whole
+ * run; a further alpha, or a full board, replaces the table used longest ago.  A stagger = 2 plan serves
+ * cans_helmholtz_solve only.
  */
+#define CANS_MAX_PIVOT_TABLES 4
 cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx, double ly, double lz,
                                               const char bc[3][2], const double* dzc, const double* dzf, int stagger);
 int cans_helmholtz_solve(cans_poisson_plan* plan, double* q, double alpha, void* stream);

@@ -299,7 +299,13 @@ struct cans_poisson_plan {
     int singular;
     int stagger;              // -1: cell-centred unknown; 0, 1, 2: the unknown lives on the faces of that direction (eq. 3b)
     int nz_solve;             // rows of the tridiagonal systems (nz, or nz - 1 for a face-located unknown between walls)
-    double alpha_tables;      // Helmholtz shift the pivot tables rstart / r00 were built for
+    // Pivot tables of the z solve (segment-start pivots rstart, singular-column pivots r00), one set per Helmholtz shift
+    // alpha: slot 0 is built at plan creation for alpha = 0, the others on the first solve with a new alpha.  An RK3 loop
+    // has three gamma_k, so four slots hold everything a plan meets; a fifth alpha replaces the slot used longest ago.
+    struct PivotSlot { double alpha; double* rstart; double* r00; unsigned long long last_use; };
+    PivotSlot pivots[CANS_MAX_PIVOT_TABLES];
+    int npivots;              // slots allocated so far
+    unsigned long long pivot_clock;
     int cyclic;               // z periodic: cyclic tridiagonal systems (z_pass.cuh)
     double a0w, cw;           // their wrap couplings
     int nseg, nzp;
@@ -311,7 +317,7 @@ struct cans_poisson_plan {
     size_t sched_bytes;
     std::vector<void*> dev_allocs;
     // device tables
-    double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc, *rstart, *r00;
+    double *lamx, *lamy, *az, *bz, *cz, *gz, *rdzf, *dzf, *rdzc;
     cplx *tw_x, *tw_y, *wpost_x, *wpost_y, *wpre_x, *wpre_y;
     cplx wstep_x[32], wstep_y[32];   // mixed pairs, warp-level kernels: wpre[32 m] (XYArgs::wstep)
     cplx* tw2_x;              // W_nx^(p k1), [nx/32][32]: warp-per-line x kernels (xw_pass.cuh), or NULL
@@ -370,7 +376,7 @@ static cudaError_t upload(cans_poisson_plan* pl, const std::vector<double>& h, T
 // layout of the scheduler state (unsigned ints)
 enum { SCHED_Z_TICKET = 0, SCHED_WORDS = 8 };
 
-static ZArgs make_zargs(const cans_poisson_plan* pl, double* p, double alpha = 0.0) {
+static ZArgs make_zargs(const cans_poisson_plan* pl, double* p, double alpha = 0.0, int slot = 0) {
     ZArgs z;
     z.alpha = alpha;
     z.nz_solve = pl->nz_solve;
@@ -380,10 +386,10 @@ static ZArgs make_zargs(const cans_poisson_plan* pl, double* p, double alpha = 0
     z.p = p;
     z.lamx = pl->lamx; z.lamy = pl->lamy;
     z.az = pl->az; z.bz = pl->bz; z.cz = pl->cz; z.gz = pl->gz;
-    z.rstart = pl->rstart;
+    z.rstart = pl->pivots[slot].rstart;
     z.scale = 1.0 / ((double)pl->nx * (double)pl->ny);
     z.singular = pl->singular && alpha == 0.0;
-    z.r00 = pl->r00;
+    z.r00 = pl->pivots[slot].r00;
     z.dzf = pl->dzf;
     z.inv_lz = pl->inv_lz;
     const int tc = z_tc_for(pl->nseg);
@@ -405,6 +411,20 @@ static XYArgs make_xyargs(const cans_poisson_plan* pl, double* p, bool xdir) {
     std::memcpy(a.wstep, xdir ? pl->wstep_x : pl->wstep_y, sizeof(a.wstep));
     a.p = p;
     return a;
+}
+
+// one more pivot-table slot for the shift alpha (contents are filled by z_setup_launch)
+static cudaError_t alloc_pivot_slot(cans_poisson_plan* pl, double alpha) {
+    void *d0 = nullptr, *d1 = nullptr;
+    cudaError_t e = cudaMalloc(&d0, sizeof(double) * (size_t)pl->nseg * pl->nx * pl->ny);
+    if (e != cudaSuccess) return e;
+    e = cudaMalloc(&d1, sizeof(double) * (size_t)pl->nz);
+    if (e != cudaSuccess) { cudaFree(d0); return e; }
+    pl->dev_allocs.push_back(d0);
+    pl->dev_allocs.push_back(d1);
+    cans_poisson_plan::PivotSlot& sl = pl->pivots[pl->npivots++];
+    sl.alpha = alpha; sl.rstart = (double*)d0; sl.r00 = (double*)d1; sl.last_use = 0;
+    return cudaSuccess;
 }
 
 static const char* const XY_NAMES[5] = {"x_fwd", "x_fwd_div", "x_inv", "y_fwd", "y_inv"};
@@ -527,7 +547,8 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     pl->cyclic = bc[2][0] == 'P';
     pl->stagger = stagger;
     pl->nz_solve = (stagger == 2 && bc[2][0] == 'D') ? nz - 1 : nz;
-    pl->alpha_tables = 0.0;
+    pl->npivots = 0;
+    pl->pivot_clock = 0;
     pl->device = 0;
     cudaGetDevice(&pl->device);
     pl->num_sms = 148;
@@ -570,16 +591,7 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
         up(make_two_pass_twiddles(ny), &pl->tw2_y);
         pl->use_yt = 1;
     }
-    if (e == cudaSuccess) {
-        void* d = nullptr;
-        e = cudaMalloc(&d, sizeof(double) * (size_t)nseg * nx * ny);
-        if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->rstart = (double*)d; }
-    }
-    if (e == cudaSuccess) {
-        void* d = nullptr;
-        e = cudaMalloc(&d, sizeof(double) * (size_t)nz);
-        if (e == cudaSuccess) { pl->dev_allocs.push_back(d); pl->r00 = (double*)d; }
-    }
+    if (e == cudaSuccess) e = alloc_pivot_slot(pl, 0.0);
     if (e == cudaSuccess) {
         pl->sched_bytes = sizeof(unsigned int) * SCHED_WORDS;
         void* d = nullptr;
@@ -588,7 +600,7 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     }
     if (e == cudaSuccess) {
         ZArgs z = make_zargs(pl, nullptr);
-        e = z_setup_launch(z, pl->rstart, pl->r00, 0);
+        e = z_setup_launch(z, pl->pivots[0].rstart, pl->pivots[0].r00, 0);
         if (e == cudaSuccess) e = cudaDeviceSynchronize();
     }
     if (e == cudaSuccess) e = z_solve_configure(nseg, pl->cyclic, pl->num_sms, &pl->z_grid, &pl->z_smem);
@@ -605,14 +617,34 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
 }
 
 static int launch_z(cans_poisson_plan* pl, double* p, double alpha, cudaStream_t st) {
-    ZArgs z = make_zargs(pl, p, alpha);
-    if (alpha != pl->alpha_tables) {
-        // the segment-start pivots depend on the shift: rebuild the table on this stream (one sweep per column, no field
-        // data: ~N/16 doubles written) before the solve that uses it
+    int slot = -1;
+    for (int i = 0; i < pl->npivots; ++i)
+        if (pl->pivots[i].alpha == alpha) slot = i;
+    const bool build = slot < 0;
+    if (build) {
+        // a shift this plan has not met (or has dropped): take a free slot -- the only allocation a solve can make, at most
+        // CANS_MAX_PIVOT_TABLES - 1 times in the life of a plan -- or, when all are taken or the board is full, the slot
+        // used longest ago (never slot 0: the Poisson table)
+        if (pl->npivots < CANS_MAX_PIVOT_TABLES && alloc_pivot_slot(pl, alpha) == cudaSuccess) slot = pl->npivots - 1;
+        else {
+            cudaGetLastError();
+            if (pl->npivots < 2) slot = 0;
+            else {
+                slot = 1;
+                for (int i = 2; i < pl->npivots; ++i)
+                    if (pl->pivots[i].last_use < pl->pivots[slot].last_use) slot = i;
+            }
+            pl->pivots[slot].alpha = alpha;
+        }
+    }
+    pl->pivots[slot].last_use = ++pl->pivot_clock;
+    ZArgs z = make_zargs(pl, p, alpha, slot);
+    if (build) {
+        // the segment-start pivots depend on the shift: fill the table on this stream (one sweep per column, no field
+        // data: ~N/16 doubles written) before the solve that uses it; stream order also protects a replaced slot
         LaunchScope scope(pl, st, "z_setup");
-        cudaError_t e = z_setup_launch(z, pl->rstart, pl->r00, st);
-        if (e != cudaSuccess) return fail_cuda(e, "z pivot table launch");
-        pl->alpha_tables = alpha;
+        cudaError_t e = z_setup_launch(z, pl->pivots[slot].rstart, pl->pivots[slot].r00, st);
+        if (e != cudaSuccess) { pl->pivots[slot].alpha = NAN; return fail_cuda(e, "z pivot table launch"); }
     }
     LaunchScope scope(pl, st, "z_solve");
     cudaError_t e = z_solve_launch(z, pl->z_grid, pl->z_smem, &pl->tmap_z, st);

@@ -113,3 +113,40 @@ def test_shift_changes_rebuild_the_pivot_table(B):
         plan.helmholtz_solve(q, 0.0)
     assert ei.value.status == B.CANS_ERR_INVALID_ARG
     plan.close()
+
+
+def test_pivot_tables_are_kept_per_shift(B):
+    """An RK3 loop alternates three shifts (one per gamma_k) next to the Poisson solve.  The plan keeps one pivot table per
+    shift (CANS_MAX_PIVOT_TABLES = 4): the table kernel `z_setup` runs on the first solve with a new alpha and never again,
+    every solve still sees the pivots of its own alpha, and a fifth alpha replaces the table used longest ago."""
+    nx, ny, nz = 96, 64, 40
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    bc = (("P", "P"), ("P", "P"), ("D", "D"))
+    dzc, dzf = grid(nz, lz, 1.6, False)
+    rng = np.random.default_rng(4)
+    f = rng.uniform(-1, 1, (nz, ny, nx))
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    plan.set_profiling(True)
+    refs = {}
+
+    def solve(alpha):
+        q = torch.from_numpy(f).cuda()
+        if alpha == 0.0:
+            plan.poisson_solve(q)
+            ref = refs.setdefault(alpha, orc.poisson_solve(f, lx, ly, lz, bc, dzc, dzf))
+        else:
+            plan.helmholtz_solve(q, alpha)
+            ref = refs.setdefault(alpha, orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc, dzf))
+        torch.cuda.synchronize()
+        check(q.cpu().numpy(), ref, f"alpha={alpha}")
+        return "z_setup" in [name for name, _ in plan.kernel_times()]
+
+    gammas = (-8.0e5, -1.5e6, -3.0e6)
+    built = [solve(a) for a in gammas]
+    assert built == [True, True, True]                      # first meeting: one table each
+    for _ in range(3):                                      # the loop proper: nothing is rebuilt, the Poisson table included
+        assert [solve(a) for a in gammas + (0.0,)] == [False, False, False, False]
+    assert solve(-10.0) is True                             # a fifth shift: replaces the table of gammas[0] (used longest ago)
+    assert solve(gammas[1]) is False and solve(gammas[2]) is False and solve(0.0) is False
+    assert solve(gammas[0]) is True                         # ... which has to be rebuilt when it comes back
+    plan.close()
