@@ -15,6 +15,7 @@ Source: /root/reference/PAPER.md ("P:L<n>" = line n of that file).
                     P:L98-100                              -> ``poisson_solve``
   * P:L104  "the grid in z can be non-uniform"             -> ``z_coefficients``
   * eq. 2d  P:L64   p^{k+1/2} = p^{k-1/2} + Phi             -> ``pressure_update``
+  * eq. 3e  P:L80   ... + Phi - (gamma nu dt / 2) L Phi     -> ``pressure_update_implicit``
   * eq. 4   P:L87 and Listing 1 P:L142-205 (``chkdt``)     -> ``chkdt_fields``, ``chkdt``
   * eq. 3b  P:L73, P:L106 (implicit diffusion: "solved with the same type of direct solver")
                                                            -> ``z_face_coefficients``, ``helmholtz_solve``
@@ -41,7 +42,7 @@ import numpy as np
 __all__ = [
     "pair_of", "basis", "z_coefficients", "z_matrix_rows", "thomas",
     "apply_laplacian", "poisson_solve", "divergence", "correct_velocity",
-    "projection", "is_singular", "uniform_spacing", "pressure_update", "chkdt_fields", "chkdt",
+    "projection", "is_singular", "uniform_spacing", "pressure_update", "pressure_update_implicit", "chkdt_fields", "chkdt",
     "z_face_coefficients", "helmholtz_solve",
 ]
 
@@ -377,6 +378,13 @@ def projection(u, v, w, dt, lx, ly, lz, bc, dzc=None, dzf=None, lower_face=None)
 def pressure_update(p, phi):
     """p^{k+1/2} = p^{k-1/2} + Phi (eq. 2d, explicit diffusion)."""
     return np.asarray(p, dtype=np.float64) + np.asarray(phi, dtype=np.float64)
+
+
+def pressure_update_implicit(p, phi, coeff, lx, ly, lz, bc, dzc=None, dzf=None):
+    """p^{k+1/2} = p^{k-1/2} + Phi - coeff * L Phi with coeff = gamma_k nu dt / 2 (P:L80-81 eq. 3e, implicit diffusion);
+    L is the Laplacian of eq. 5 with the ghost rules of Phi (``apply_laplacian``)."""
+    phi = np.asarray(phi, dtype=np.float64)
+    return np.asarray(p, dtype=np.float64) + phi - coeff * apply_laplacian(phi, lx, ly, lz, bc, dzc, dzf)
 
 
 def _pad_velocity(vel, axis, pair, normal, face):

@@ -502,6 +502,44 @@ def test_pressure_update_is_a_plain_sum():
     assert out[1, 2, 3] == 7.0 and out[0, 0, 0] == 1.75 and a[1, 2, 3] == 3.0
 
 
+def test_pressure_update_implicit_closed_forms():
+    """eq. 3e: p + Phi - c L Phi, on fields whose Laplacian is known by hand."""
+    nz, ny, nx = 6, 8, 12
+    lx, ly, lz = 3.0, 2.0, 1.5
+    c = 0.37
+    rng = np.random.default_rng(8)
+    p = rng.standard_normal((nz, ny, nx))
+    x = (np.arange(nx) + 0.5) * lx / nx
+    # (1) a discrete eigenmode of the periodic second difference: L Phi = -(4/dx^2) sin^2(pi m / nx) Phi, nothing from y, z
+    #     (Neumann there: a field constant along y and z has zero second differences, ghosts included)
+    m = 2
+    phi = np.broadcast_to(np.cos(2 * np.pi * m * x / lx), (nz, ny, nx)).copy()
+    lam = -4.0 * np.sin(np.pi * m / nx) ** 2 / (lx / nx) ** 2
+    bc = (("P", "P"), ("N", "N"), ("N", "N"))
+    out = orc.pressure_update_implicit(p, phi, c, lx, ly, lz, bc)
+    assert np.allclose(out, p + (1.0 - c * lam) * phi, rtol=0, atol=1e-12)
+    # (2) Phi linear in z on a stretched grid: the flux (Phi_{k+1} - Phi_k) / dzc_{k+1} is the same through every face, so
+    #     L Phi = 0 in the interior; next to a Neumann wall only the inner flux is left: L Phi = -+ slope / dzf
+    dzc, dzf = stretched(nz, lz, 1.7)
+    zc = np.cumsum(dzf) - 0.5 * dzf
+    slope = 1.3
+    phi = np.broadcast_to((slope * zc)[:, None, None], (nz, ny, nx)).copy()
+    out = orc.pressure_update_implicit(p, phi, c, lx, ly, lz, bc, dzc, dzf)
+    want = p + phi
+    want[0] -= c * slope / dzf[0]
+    want[-1] += c * slope / dzf[-1]
+    assert np.allclose(out, want, rtol=0, atol=1e-12)
+    # (3) Dirichlet walls in y, Phi = 1: the anti-mirrored ghost is -1, so L Phi = -2/dy^2 in the two rows next to the walls
+    bcd = (("P", "P"), ("D", "D"), ("N", "N"))
+    out = orc.pressure_update_implicit(p, np.ones_like(p), c, lx, ly, lz, bcd)
+    want = p + 1.0
+    want[:, 0, :] += 2.0 * c / (ly / ny) ** 2
+    want[:, -1, :] += 2.0 * c / (ly / ny) ** 2
+    assert np.allclose(out, want, rtol=0, atol=1e-12)
+    # (4) c = 0 is eq. 2d
+    assert np.array_equal(orc.pressure_update_implicit(p, phi, 0.0, lx, ly, lz, bc, dzc, dzf), orc.pressure_update(p, phi))
+
+
 def test_chkdt_of_uniform_flow():
     """u = a, v = b, w = c everywhere on a triperiodic grid: every face sum is |a|/dx + |b|/dy + |c|/dz."""
     nz, ny, nx = 5, 6, 8
