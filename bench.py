@@ -391,6 +391,7 @@ def time_step_variants(binding, torch, plan, w, fields, steps=5, warmup=2):
     out = {}
     out["projection_step_pacc_chkdt_ms"] = med(lambda: plan.projection_step(u, v, ww, p, w.dt, p_acc=pacc, dti=dti), restore)
     out["projection_step_pacc_ms"] = med(lambda: plan.projection_step(u, v, ww, p, w.dt, p_acc=pacc), restore)
+    out["projection_step_eq3e_ms"] = med(lambda: plan.projection_step(u, v, ww, p, w.dt, p_acc=pacc, nu_dt_half=4.4e-8), restore)
     out["chkdt_ms"] = med(lambda: plan.chkdt(u, v, ww, dti), lambda: None)
     out["chkdt_gbs"] = 24.0 * w.cells / (out["chkdt_ms"] * 1e-3) / 1e9
     alpha = -2.0 / (0.5 * 1.77e-4 * 1e-3)          # -2/(gamma nu dt): gamma ~ 1/2, nu = 1/5640, dt = 1e-3

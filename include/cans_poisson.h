@@ -140,6 +140,17 @@ int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* 
                          double dt, double* dti, void* stream);
 
 /*
+ * cans_projection_step_implicit -- cans_projection_step with the pressure update of the implicit-diffusion scheme, eq. 3e
+ * (SURVEY 8f row f4):
+ *     p_acc += Phi - nu_dt_half * L Phi,      nu_dt_half = gamma_k nu dt / 2  (>= 0; 0 is eq. 2d and needs no p_acc),
+ * L the 7-point Laplacian of eq. 5 with the ghost rule of Phi on every side.  The correction kernel forms L Phi from the Phi
+ * values it already holds for the gradient plus its lower neighbours (its own carry in z, cache hits in x and y): the pass
+ * still moves 72 B/cell.  p_acc is required when nu_dt_half > 0.  Everything else as cans_projection_step.
+ */
+int cans_projection_step_implicit(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double* p_acc,
+                                  double dt, double nu_dt_half, double* dti, void* stream);
+
+/*
  * cans_chkdt -- the max-reduction of Listing 1:
  *     dti = max over cells of max(dtix, dtiy, dtiz),
  *     dtix = |u|/dx + |v(i,j)+v(i,j-1)+v(i+1,j)+v(i+1,j-1)|/(4 dy) + |w(i,j,k)+w(i,j,k-1)+w(i+1,j,k)+w(i+1,j,k-1)|/(4 dzf[k])

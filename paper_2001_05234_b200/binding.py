@@ -25,7 +25,7 @@ MAX_KERNEL_RECORDS = 16      # CANS_MAX_KERNEL_RECORDS of the header
 
 EXPORTED_SYMBOLS = (
     "cans_poisson_plan_create", "cans_poisson_plan_destroy", "cans_poisson_solve", "cans_projection",
-    "cans_projection_step", "cans_chkdt", "cans_chkdt_static", "cans_helmholtz_plan_create", "cans_helmholtz_solve",
+    "cans_projection_step", "cans_projection_step_implicit", "cans_chkdt", "cans_chkdt_static", "cans_helmholtz_plan_create", "cans_helmholtz_solve",
     "cans_probe_fp64_fma", "cans_probe_tile_copy",
     "cans_projection_set_lower_face", "cans_poisson_solve_host", "cans_projection_host",
     "cans_last_error", "cans_last_status", "cans_plan_launches_per_solve",
@@ -79,6 +79,8 @@ def _load() -> ctypes.CDLL:
     lib.cans_probe_tile_copy.argtypes = [vp, vp, i32, ctypes.POINTER(ctypes.c_float), vp]
     lib.cans_projection_step.restype = i32
     lib.cans_projection_step.argtypes = [vp, vp, vp, vp, vp, vp, ctypes.c_double, vp, vp]
+    lib.cans_projection_step_implicit.restype = i32
+    lib.cans_projection_step_implicit.argtypes = [vp, vp, vp, vp, vp, vp, dbl, dbl, vp, vp]
     lib.cans_chkdt.restype = i32
     lib.cans_chkdt.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.cans_chkdt_static.restype = i32
@@ -217,13 +219,17 @@ class PoissonPlan:
                                     _dev_ptr(w, self.shape), _dev_ptr(p, self.shape), float(dt),
                                     _stream_ptr(stream)))
 
-    def projection_step(self, u, v, w, p, dt: float, p_acc=None, dti=None, stream=None):
+    def projection_step(self, u, v, w, p, dt: float, p_acc=None, dti=None, stream=None, nu_dt_half: float = 0.0):
         """cans_projection_step: the projection, plus p_acc += Phi (eq. 2d) in the correction kernel when p_acc is
-        given, plus the chkdt reduction of the corrected velocities into the one-element CUDA tensor dti when given."""
-        _check(_lib.cans_projection_step(self._h, _dev_ptr(u, self.shape), _dev_ptr(v, self.shape),
-                                         _dev_ptr(w, self.shape), _dev_ptr(p, self.shape),
-                                         None if p_acc is None else _dev_ptr(p_acc, self.shape), float(dt),
-                                         None if dti is None else _dev_ptr(dti, (1,)), _stream_ptr(stream)))
+        given, plus the chkdt reduction of the corrected velocities into the one-element CUDA tensor dti when given.
+        nu_dt_half > 0: cans_projection_step_implicit, p_acc += Phi - nu_dt_half * L Phi (eq. 3e)."""
+        pa = None if p_acc is None else _dev_ptr(p_acc, self.shape)
+        dp = None if dti is None else _dev_ptr(dti, (1,))
+        fields = (_dev_ptr(u, self.shape), _dev_ptr(v, self.shape), _dev_ptr(w, self.shape), _dev_ptr(p, self.shape))
+        if nu_dt_half == 0.0:
+            _check(_lib.cans_projection_step(self._h, *fields, pa, float(dt), dp, _stream_ptr(stream)))
+        else:
+            _check(_lib.cans_projection_step_implicit(self._h, *fields, pa, float(dt), float(nu_dt_half), dp, _stream_ptr(stream)))
 
     def chkdt(self, u, v, w, dti, stream=None):
         """cans_chkdt: dti[0] = max over cells of the per-face sums of Listing 1 (one-element CUDA float64 tensor)."""

@@ -61,6 +61,7 @@ int report_cuda_failure(cudaError_t e, const char* where) { return fail_cuda(e, 
 // ------------------------------------------------------------------------------------------------
 constexpr int GRAD_KC = 32;
 
+template <bool LAP>
 __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
     const int hx = a.nx / 2;
     const size_t cols = (size_t)hx * a.ny;
@@ -74,11 +75,29 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
     const size_t rowo = (size_t)j * a.nx + i;
     size_t o = (size_t)k0 * plane + rowo;
     double2 ph = *reinterpret_cast<const double2*>(a.phi + o);
+    double2 phm = ph;                              // LAP: the plane below, carried like the centre value
+    if (LAP) {
+        if (k0 > 0) phm = *reinterpret_cast<const double2*>(a.phi + o - plane);
+        else {
+            phm = *reinterpret_cast<const double2*>(a.phi + (size_t)a.lz_idx * plane + rowo);
+            phm.x *= a.lz_sgn; phm.y *= a.lz_sgn;
+        }
+    }
     for (int k = k0; k < k1; ++k, o += plane) {
         GradIn in;
         in.o = o;
         in.k = k;
         in.ph = ph;
+        if (LAP) {
+            in.phzm = phm;
+            phm = ph;
+            in.phxm = (i > 0) ? a.phi[o - 1] : a.lx_sgn * a.phi[o + a.lx_idx];
+            if (j > 0) in.phym = *reinterpret_cast<const double2*>(a.phi + o - a.nx);
+            else {
+                in.phym = *reinterpret_cast<const double2*>(a.phi + (size_t)k * plane + (size_t)a.ly_idx * a.nx + i);
+                in.phym.x *= a.ly_sgn; in.phym.y *= a.ly_sgn;
+            }
+        }
         in.phx = (i + 2 < a.nx) ? a.phi[o + 2] : a.gx_sgn * a.phi[o - i + a.gx_idx];
         if (j + 1 < a.ny) in.phy = *reinterpret_cast<const double2*>(a.phi + o + a.nx);
         else {
@@ -95,8 +114,8 @@ __global__ void __launch_bounds__(256) grad_correct_kernel(const GradArgs a) {
         in.uu = *reinterpret_cast<const double2*>(a.u + o);
         in.vv = *reinterpret_cast<const double2*>(a.v + o);
         in.ww = *reinterpret_cast<const double2*>(a.w + o);
-        if (a.pacc) in.pa = *reinterpret_cast<const double2*>(a.pacc + o);
-        grad_apply(a, in);
+        if (LAP || a.pacc) in.pa = *reinterpret_cast<const double2*>(a.pacc + o);
+        grad_apply<LAP>(a, in);
     }
 }
 
@@ -656,7 +675,8 @@ static int launch_grad(cans_poisson_plan* pl, const GradArgs& g, cudaStream_t st
     const size_t cols = (size_t)pl->nx / 2 * pl->ny;
     dim3 grid((unsigned)((cols + 255) / 256), (unsigned)((g.k1 - g.k0 + GRAD_KC - 1) / GRAD_KC));
     LaunchScope scope(pl, st, "grad_correct");
-    grad_correct_kernel<<<grid, 256, 0, st>>>(g);
+    if (g.pacc && g.lap_coef != 0.0) grad_correct_kernel<true><<<grid, 256, 0, st>>>(g);     // eq. 3e
+    else grad_correct_kernel<false><<<grid, 256, 0, st>>>(g);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail_cuda(e, "gradient correction launch");
     return CANS_OK;
@@ -765,7 +785,14 @@ int cans_projection(cans_poisson_plan* plan, double* u, double* v, double* w, do
 
 int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double* p_acc, double dt,
                          double* dti, void* stream) {
+    return cans_projection_step_implicit(plan, u, v, w, p, p_acc, dt, 0.0, dti, stream);
+}
+
+int cans_projection_step_implicit(cans_poisson_plan* plan, double* u, double* v, double* w, double* p, double* p_acc, double dt,
+                                  double nu_dt_half, double* dti, void* stream) {
     g_status = CANS_OK;
+    if (!(nu_dt_half >= 0.0)) return fail(CANS_ERR_INVALID_ARG, "nu_dt_half (gamma nu dt / 2 of eq. 3e) must be >= 0");
+    if (nu_dt_half > 0.0 && !p_acc) return fail(CANS_ERR_INVALID_ARG, "eq. 3e updates p_acc: it must be non-NULL when nu_dt_half > 0");
     if (!plan || !u || !v || !w || !p) return fail(CANS_ERR_INVALID_ARG, "plan, u, v, w, p must be non-NULL");
     if (plan->stagger == 2) return fail(CANS_ERR_INVALID_ARG, "a plan for an unknown on the z faces solves cans_helmholtz_solve only");
     if (p_acc && ((reinterpret_cast<size_t>(p_acc) & 15) != 0 || p_acc == p || p_acc == u || p_acc == v || p_acc == w))
@@ -807,6 +834,18 @@ int cans_projection_step(cans_poisson_plan* plan, double* u, double* v, double* 
     ghost(plan->bc[0][1], plan->nx, &g.gx_idx, &g.gx_sgn);
     ghost(plan->bc[1][1], plan->ny, &g.gy_idx, &g.gy_sgn);
     ghost(plan->bc[2][1], plan->nz, &g.gz_idx, &g.gz_sgn);
+    auto ghost_below = [](char lo, int n, int* idx, double* sgn) {
+        if (lo == 'P') { *idx = n - 1; *sgn = 1.0; }
+        else if (lo == 'N') { *idx = 0; *sgn = 1.0; }
+        else { *idx = 0; *sgn = -1.0; }
+    };
+    ghost_below(plan->bc[0][0], plan->nx, &g.lx_idx, &g.lx_sgn);
+    ghost_below(plan->bc[1][0], plan->ny, &g.ly_idx, &g.ly_sgn);
+    ghost_below(plan->bc[2][0], plan->nz, &g.lz_idx, &g.lz_sgn);
+    g.lap_coef = nu_dt_half;
+    g.rdx2 = a.rdx * a.rdx; g.rdy2 = a.rdy * a.rdy;
+    g.rdzc0 = 1.0 / plan->dzc0;
+    g.rdzf = plan->rdzf;
     int rc = run_core(plan, p, &a, &g, st);
     if (rc) return rc;
     // a7 on the registered lower faces of pressure-Dirichlet sides (planes on 'N' sides are prescribed inflow)

@@ -241,3 +241,64 @@ def test_projection_step_fuses_eq_2d_and_returns_chkdt(B, nx, ny, nz, bcs):
         plan.projection_step(us, vs, ws, ps, dt, p_acc=ps)
     assert ei.value.status == B.CANS_ERR_INVALID_ARG
     plan.close()
+
+
+def _implicit_case(B, nx, ny, nz, bc, coef, seed, stretch=1.6):
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    if bc[2][0] == "P":
+        dzc = dzf = None                                  # periodic z: uniform (single-valued wrap spacing)
+    else:
+        dzc_t, dzf_t, _ = wl.tanh_grid(nz, lz, stretch)
+        dzc, dzf = dzc_t.numpy(), dzf_t.numpy()
+    rng = np.random.default_rng(seed)
+    u, v, w, pacc = (rng.standard_normal((nz, ny, nx)) for _ in range(4))
+    pacc *= 100.0
+    faces = _faces(rng, bc, (nz, ny, nx))
+    dt = 1e-3
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc, dzc, dzf)
+    ud, vd, wd, pa = (torch.from_numpy(a).cuda() for a in (u, v, w, pacc))
+    fd = {d: torch.from_numpy(f).cuda() for d, f in faces.items()}
+    for d, t in fd.items():
+        plan.set_lower_face(d, t)
+    pd = torch.empty_like(ud)
+    plan.projection_step(ud, vd, wd, pd, dt, p_acc=pa, nu_dt_half=coef)
+    torch.cuda.synchronize()
+    plan.close()
+    un, vn, wn, phi, _ = orc.projection(u, v, w, dt, lx, ly, lz, bc, dzc, dzf, faces)
+    want = orc.pressure_update_implicit(pacc, phi, coef, lx, ly, lz, bc, dzc, dzf)
+    got = pa.cpu().numpy()
+    # the Laplacian term must matter in this test, or a wrong stencil would pass unnoticed
+    plain = orc.pressure_update(pacc, phi)
+    assert np.linalg.norm(want - plain) >= 0.05 * np.linalg.norm(phi), "test too weak: coef * L Phi is negligible"
+    assert np.linalg.norm(got - want) <= 1e-11 * np.linalg.norm(want), bc
+    assert np.max(np.abs(got - want)) * dt <= 1e-10, bc
+    for g, r in ((ud, un), (vd, vn), (wd, wn)):            # the velocities are those of the plain step
+        assert np.linalg.norm(g.cpu().numpy() - r) <= 1e-11 * np.linalg.norm(r)
+
+
+def test_eq_3e_every_boundary_combination(B):
+    """cans_projection_step_implicit: p_acc += Phi - (gamma nu dt / 2) L Phi (eq. 3e) for all 125 combinations of
+    boundary pairs, against the oracle's apply_laplacian of the oracle's Phi.  The grid is two chunks of planes tall
+    (GRAD_KC = 32), so the carried plane below is exercised across a chunk boundary."""
+    n = 0
+    for px, py, pz in itertools.product(ALL_PAIRS, ALL_PAIRS, ALL_PAIRS):
+        bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
+        _implicit_case(B, 32, 16, 36, bc, 4e-3, seed=n)
+        n += 1
+
+
+@pytest.mark.parametrize("nx,ny,nz,bcs,coef", [(512, 64, 40, ("PP", "PP", "NN"), 2e-5), (96, 768, 9, ("ND", "DD", "DN"), 2e-5),
+                                               (1024, 32, 70, ("NN", "PP", "PP"), 4e-6)])
+def test_eq_3e_on_the_fast_kernel_sizes(B, nx, ny, nz, bcs, coef):
+    _implicit_case(B, nx, ny, nz, tuple((p[0], p[1]) for p in bcs), coef, seed=nx + nz)
+
+
+def test_eq_3e_argument_checks(B):
+    nx, ny, nz = 32, 16, 8
+    plan = B.PoissonPlan(nx, ny, nz, 1.0, 1.0, 1.0, (("P", "P"), ("P", "P"), ("N", "N")))
+    u, v, w, p, pa = (torch.zeros((nz, ny, nx), dtype=torch.float64, device="cuda") for _ in range(5))
+    for kw in ({"nu_dt_half": -1.0, "p_acc": pa}, {"nu_dt_half": 1e-3}):        # negative coefficient; eq. 3e without p_acc
+        with pytest.raises(B.CansError) as ei:
+            plan.projection_step(u, v, w, p, 1e-3, **kw)
+        assert ei.value.status == B.CANS_ERR_INVALID_ARG
+    plan.close()
