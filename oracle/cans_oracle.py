@@ -493,8 +493,10 @@ def helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc=None, dzf=None, stagger=None):
     faces (u: 0, v: 1, w: 2 -- "face-located unknowns in the wall-normal direction").  Along a periodic direction the
     operator is the same as for centres (x, y uniform).  Along z: rows of ``z_face_coefficients``; 'PP' cyclic, 'DD' = walls
     at the lower boundary and at face nz-1 (homogeneous: the wall values do not enter the right-hand side), slot nz-1 is
-    returned as it came.  Other staggered cases (face-located along a non-periodic x or y, or z pairs with 'N') are not
-    implemented (they need the node-based DST-I / DCT-I family): NotImplementedError."""
+    returned as it came; 'DN' = wall below, zero normal derivative at the upper boundary face nz-1 (an outflow / free-slip
+    top: that face is an unknown, mirrored neighbour above).  Other staggered cases are not implemented: face-located along
+    a non-periodic x or y (the node-based DST-I / DCT-I family), and z pairs with a lower 'N' (the lower boundary face
+    would be an unknown, and the compact layout has no slot for it): NotImplementedError."""
     f = np.asarray(f, dtype=np.float64)
     nz, ny, nx = f.shape
     if dzc is None or dzf is None:
@@ -505,8 +507,8 @@ def helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc=None, dzf=None, stagger=None):
     px, py, pz = pair_of(bc[0]), pair_of(bc[1]), pair_of(bc[2])
     if stagger in (0, 1) and (px, py)[stagger] != "PP":
         raise NotImplementedError("face-located unknowns along a non-periodic x or y")
-    if stagger == 2 and pz not in ("PP", "DD"):
-        raise NotImplementedError("face-located unknowns along z need PP or DD")
+    if stagger == 2 and pz not in ("PP", "DD", "DN"):
+        raise NotImplementedError("face-located unknowns along z need PP, DD or DN")
     Bx, lamx, wx = basis(px, nx)
     By, lamy, wy = basis(py, ny)
     fh = np.matmul(By, np.matmul(f, Bx.T))
@@ -518,6 +520,14 @@ def helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc=None, dzf=None, stagger=None):
         if pz == "DD":
             n_solve = nz - 1                   # wall nodes below face 0 and at face nz-1: their couplings drop out
             a, b, c = a[:n_solve], b[:n_solve], c[:n_solve]
+        elif pz == "DN":
+            # zero normal derivative AT the upper boundary face: face nz-1 is an unknown, the face above it is the mirror
+            # image of face nz-2 (ghost cell of width dzf_{nz-1}), so its coupling 1/(dzc_nz dzf_{nz-1}) adds to a_{nz-1}
+            a, c = a.copy(), c.copy()
+            ghost = 1.0 / (dzc[nz] * dzf[nz - 1])
+            b[nz - 1] = -(a[nz - 1] + ghost)
+            a[nz - 1] += ghost
+            c[nz - 1] = 0.0
         solver = _cyclic_thomas if pz == "PP" else thomas
     elif pz == "PP":
         a, c = z_coefficients(dzc, dzf)

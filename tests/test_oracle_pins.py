@@ -662,12 +662,19 @@ def test_chkdt_is_invariant_under_shifts_along_periodic_directions():
 # ----------------------------------------------------------------------------------------------
 # NEXT row f4: the Helmholtz solve of eq. 3b, cell-centred and with the unknown on the z faces
 # ----------------------------------------------------------------------------------------------
-def face_second_difference_1d(nz, dzc, dzf, periodic):
+def face_second_difference_1d(nz, dzc, dzf, periodic, upper_neumann=False):
     """nz x nz matrix of the second difference of a FACE-located quantity, written from the geometry alone: face k at
     height zf_{k+1}, neighbours dzf_k below and dzf_{k+1} above, control volume dzc_{k+1}.  Non-periodic: wall nodes below
-    face 0 and at face nz-1 (value 0), so row nz-1 is left empty."""
+    face 0 and at face nz-1 (value 0), so row nz-1 is left empty -- unless upper_neumann: then face nz-1 (the upper
+    boundary) is an unknown whose upper neighbour is the mirror image of face nz-2, a ghost cell of width dzf_{nz-1} away."""
     M = np.zeros((nz, nz))
     rows = nz if periodic else nz - 1
+    if upper_neumann:
+        k = nz - 1
+        lo = 1.0 / (dzc[k + 1] * dzf[k])
+        up = 1.0 / (dzc[k + 1] * dzf[k])          # mirrored cell
+        M[k, k] = -(lo + up)
+        M[k, k - 1] = lo + up                     # w_{k+1} := w_{k-1}
     for k in range(rows):
         lo = 1.0 / (dzc[k + 1] * dzf[k])
         up = 1.0 / (dzc[k + 1] * dzf[(k + 1) % nz])
@@ -678,7 +685,7 @@ def face_second_difference_1d(nz, dzc, dzf, periodic):
         else:
             if k - 1 >= 0:
                 M[k, k - 1] += lo
-            if k + 1 <= nz - 2:
+            if k + 1 <= nz - 2 or (upper_neumann and k + 1 <= nz - 1):
                 M[k, k + 1] += up
     return M
 
@@ -704,17 +711,17 @@ def test_helmholtz_vs_dense_lu(grid):
             got = orc.helmholtz_solve(f, alpha, lx, ly, lz, bc, dzc_u, dzf)
             assert np.max(np.abs(got - ref)) < 2e-12 * np.max(np.abs(ref)), (px, py, pz, alpha)
     # unknown on the z faces (w): walls (DD) and periodic, x / y any pair
-    for px, py, pz in itertools.product(["PP", "DD", "ND"], ["PP", "NN"], ["DD", "PP"]):
+    for px, py, pz in itertools.product(["PP", "DD", "ND"], ["PP", "NN"], ["DD", "PP", "DN"]):
         bc = bc_of(px, py, pz)
         dzc_u = dzc.copy()
         if pz == "PP":
             dzc_u[0] = dzc_u[-1] = 0.5 * (dzf[0] + dzf[-1])
         Lx = second_difference_1d(nx, px) / (lx / nx) ** 2
         Ly = second_difference_1d(ny, py) / (ly / ny) ** 2
-        Lz = face_second_difference_1d(nz, dzc_u, dzf, pz == "PP")
+        Lz = face_second_difference_1d(nz, dzc_u, dzf, pz == "PP", upper_neumann=(pz == "DN"))
         f = rng.uniform(-1, 1, (nz, ny, nx))
         alpha = -3.5
-        rows = np.ones(nz) if pz == "PP" else np.concatenate([np.ones(nz - 1), [0.0]])     # row nz-1 of DD: identity
+        rows = np.ones(nz) if pz in ("PP", "DN") else np.concatenate([np.ones(nz - 1), [0.0]])     # row nz-1 of DD: identity
         R = np.diag(rows)
         M = (np.kron(R, np.kron(Iy, Lx)) + np.kron(R, np.kron(Ly, Ix)) + np.kron(Lz, np.kron(Iy, Ix))
              + np.kron(alpha * R + (Iz - R), np.kron(Iy, Ix)))
@@ -732,6 +739,24 @@ def test_helmholtz_vs_dense_lu(grid):
         orc.helmholtz_solve(f, -1.0, lx, ly, lz, bc_of("NN", "PP", "DD"), dzc, dzf, stagger=0)
     with pytest.raises(NotImplementedError):
         orc.helmholtz_solve(f, -1.0, lx, ly, lz, bc_of("PP", "PP", "NN"), dzc, dzf, stagger=2)
+
+
+def test_helmholtz_face_unknown_with_outflow_top_eigenmodes():
+    """Textbook pin of the 'DN' face-located case on a uniform grid: nodes k = 0..n-1 at heights (k+1) dz, zero value at
+    height 0, zero slope at the last node.  The eigenvectors of that second difference are sin((q + 1/2) pi (k+1) / n) with
+    eigenvalues -(4/dz^2) sin^2((q + 1/2) pi / (2n)) (the DST-III family), so for a right-hand side that is one of them,
+    constant in x and y, Phi = f / (lambda + alpha)."""
+    nx, ny, nz = 4, 4, 9
+    lx, ly, lz = 1.0, 1.0, 1.8
+    dz = lz / nz
+    k = np.arange(nz)
+    for q in (0, 3, nz - 1):
+        vec = np.sin((q + 0.5) * np.pi * (k + 1) / nz)
+        lam = -4.0 / dz**2 * np.sin((q + 0.5) * np.pi / (2 * nz)) ** 2
+        f = np.broadcast_to(vec[:, None, None], (nz, ny, nx)).copy()
+        alpha = -2.5
+        got = orc.helmholtz_solve(f, alpha, lx, ly, lz, bc_of("PP", "PP", "DN"), stagger=2)
+        assert np.max(np.abs(got - f / (lam + alpha))) < 1e-12 * np.max(np.abs(f / (lam + alpha))), q
 
 
 def test_helmholtz_closed_forms():
