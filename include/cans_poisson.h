@@ -85,9 +85,11 @@ cans_poisson_plan* cans_poisson_plan_create(int nx, int ny, int nz,
  *            0, 1, 2: it lives on the +x / +y / +z faces (u, v, w of the staggered arrangement).  Along a periodic
  *            direction the operator is the one for centres.  stagger = 2 with z walls ('D','D'): faces 0..nz-2 are the
  *            unknowns, the wall nodes below face 0 and at face nz-1 are homogeneous (a moving wall is folded into f by the
- *            caller) and slot nz-1 of q is returned as it came; stagger = 2 with periodic z: cyclic systems.  Every other
- *            face-located case (non-periodic x or y: node-based DST-I / DCT-I; z pairs containing 'N') returns NULL with
- *            CANS_ERR_UNSUPPORTED_BC.
+ *            caller) and slot nz-1 of q is returned as it came; stagger = 2 with ('D','N'): wall below, zero normal
+ *            derivative AT the upper boundary face (outflow / free-slip top), face nz-1 is an unknown with a mirrored upper
+ *            neighbour; stagger = 2 with periodic z: cyclic systems.  Every other face-located case (non-periodic x or y:
+ *            node-based DST-I / DCT-I; a lower 'N' in z: the lower boundary face has no slot in this layout) returns NULL
+ *            with CANS_ERR_UNSUPPORTED_BC.
  *   q        DEVICE, nx*ny*nz doubles: f on entry, Phi on exit.     alpha < 0.
  * The pivots entering each z segment depend on alpha: the plan keeps up to CANS_MAX_PIVOT_TABLES tables (N/16 doubles each;
  * the first, for alpha = 0, from plan creation) and builds one -- one device allocation and one extra kernel on the caller's

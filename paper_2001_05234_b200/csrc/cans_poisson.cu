@@ -524,8 +524,9 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
         fail(CANS_ERR_UNSUPPORTED_BC, "an unknown on the faces of a non-periodic x or y direction needs the node-based DST-I / DCT-I transforms (not implemented)");
         return nullptr;
     }
-    if (stagger == 2 && !((bc[2][0] == 'P') || (bc[2][0] == 'D' && bc[2][1] == 'D'))) {
-        fail(CANS_ERR_UNSUPPORTED_BC, "an unknown on the z faces is implemented between walls ('D','D') and for periodic z");
+    if (stagger == 2 && bc[2][0] == 'N') {
+        fail(CANS_ERR_UNSUPPORTED_BC, "an unknown on the z faces with a lower 'N' side is not implemented (the lower boundary "
+                                      "face would be an unknown and the compact layout has no slot for it): use 'P', ('D','D') or ('D','N')");
         return nullptr;
     }
     FftRadices fx, fy;
@@ -565,7 +566,7 @@ cans_poisson_plan* cans_helmholtz_plan_create(int nx, int ny, int nz, double lx,
     pl->singular = (kx == KIND_PP || kx == KIND_NN) && (ky == KIND_PP || ky == KIND_NN) && bc[2][0] != 'D' && bc[2][1] != 'D';
     pl->cyclic = bc[2][0] == 'P';
     pl->stagger = stagger;
-    pl->nz_solve = (stagger == 2 && bc[2][0] == 'D') ? nz - 1 : nz;
+    pl->nz_solve = (stagger == 2 && bc[2][0] == 'D' && bc[2][1] == 'D') ? nz - 1 : nz;
     pl->npivots = 0;
     pl->pivot_clock = 0;
     pl->device = 0;

@@ -162,26 +162,35 @@ struct ZRows {
 // lo / up: 'N' or 'D', or both 'P' (cyclic system: no boundary folding, the wrap couplings a_0 and c_{nz-1} are returned
 // separately and zeroed in the rows).  nzp >= nz: rows beyond nz are decoupled identity-like rows (a = c = g = 0, b = -1).
 // face != 0: the unknown lives on the +z faces (wall-normal velocity of eq. 3b): a_k = 1/(dzc_{k+1} dzf_k),
-// c_k = 1/(dzc_{k+1} dzf_{k+1}); walls ('D','D'): rows 0..nz-2, wall nodes carry no coupling; periodic: wrapped.
+// c_k = 1/(dzc_{k+1} dzf_{k+1}); walls ('D','D'): rows 0..nz-2, wall nodes carry no coupling; periodic: wrapped;
+// wall below and zero slope at the top ('D','N'): rows 0..nz-1, the last with a mirrored upper neighbour.
 inline ZRows make_z_rows(int nz, int nzp, const double* dzc, const double* dzf, char lo, char up, int face = 0) {
     ZRows z;
     if (face) {
         z.a.assign(nzp, 0.0); z.b.assign(nzp, -1.0); z.c.assign(nzp, 0.0); z.g.assign(nzp, 0.0);
         z.rdzf.resize(nz); z.dzf.resize(nz);
         z.lz_sum = 0.0;
-        const int rows = (lo == 'P') ? nz : nz - 1;
+        const bool open_top = (lo == 'D' && up == 'N');      // zero slope AT the upper boundary face: face nz-1 is an unknown
+        const int rows = (lo == 'P' || open_top) ? nz : nz - 1;
         for (int k = 0; k < nz; ++k) { z.rdzf[k] = 1.0 / dzf[k]; z.dzf[k] = dzf[k]; z.lz_sum += dzf[k]; }
         for (int k = 0; k < rows; ++k) {
             z.a[k] = 1.0 / (dzc[k + 1] * dzf[k]);
             z.c[k] = 1.0 / (dzc[k + 1] * dzf[(k + 1) % nz]);
             z.b[k] = -(z.a[k] + z.c[k]);
         }
+        if (open_top) {
+            // the face above face nz-1 is the mirror image of face nz-2 (ghost cell of width dzf_{nz-1}): its coupling
+            // folds into a_{nz-1}
+            const double ghost = 1.0 / (dzc[nz] * dzf[nz - 1]);
+            z.b[nz - 1] = -(z.a[nz - 1] + ghost);
+            z.a[nz - 1] += ghost;
+            z.c[nz - 1] = 0.0;
+        }
         z.a0w = z.a[0];
         z.cw = z.c[rows - 1];
         z.a[0] = 0.0;
         z.c[rows - 1] = 0.0;
         for (int k = 1; k < rows; ++k) z.g[k] = z.a[k] * z.c[k - 1];
-        (void)up;
         return z;
     }
     z.a.assign(nzp, 0.0); z.b.assign(nzp, -1.0); z.c.assign(nzp, 0.0); z.g.assign(nzp, 0.0);

@@ -74,7 +74,8 @@ def test_plan_create_rejects_bad_arguments_without_a_gpu(binding, kwargs, status
 @pytest.mark.parametrize("bc,stagger,status", [
     ((("N", "N"), ("P", "P"), ("D", "D")), 0, 2),      # faces along a non-periodic x: DST-I / DCT-I family, not implemented
     ((("P", "P"), ("D", "N"), ("D", "D")), 1, 2),
-    ((("P", "P"), ("P", "P"), ("N", "N")), 2, 2),      # faces along z: walls or periodic only
+    ((("P", "P"), ("P", "P"), ("N", "N")), 2, 2),      # faces along z: no lower 'N' (the lower boundary face has no slot)
+    ((("P", "P"), ("P", "P"), ("N", "D")), 2, 2),
     ((("P", "P"), ("P", "P"), ("D", "D")), 3, 1),
 ])
 def test_helmholtz_plan_rejects_unsupported_staggering_without_a_gpu(binding, bc, stagger, status):

@@ -63,12 +63,14 @@ def test_cell_centred_helmholtz_every_boundary_combination(B, nx, ny, nz, stretc
 @pytest.mark.parametrize("nx,ny,nz,stretch", [(48, 32, 33, 1.6), (1024, 64, 9, None), (32, 48, 512, 1.6), (32, 16, 257, 2.0), (32, 32, 600, 1.6)])
 def test_face_located_unknowns(B, nx, ny, nz, stretch):
     """The three velocity components of the channel configuration: u (faces in x), v (faces in y) with no-slip walls in z
-    ('D','D', cell-centred in z), w on the z faces between the walls; and w in a triperiodic box."""
+    ('D','D', cell-centred in z), w on the z faces between the walls; w in a triperiodic box; w with a wall below and zero
+    normal derivative at the upper boundary face ('D','N')."""
     lx, ly, lz = 2 * np.pi, np.pi, 2.0
     rng = np.random.default_rng(5 * nx + nz)
     alpha = -1.7e5
     cases = [(0, ("PP", "PP", "DD")), (1, ("PP", "PP", "DD")), (2, ("PP", "PP", "DD")), (2, ("NN", "DN", "DD")),
-             (2, ("PP", "PP", "PP")), (2, ("DD", "PP", "PP")), (-1, ("PP", "PP", "DD"))]
+             (2, ("PP", "PP", "PP")), (2, ("DD", "PP", "PP")), (-1, ("PP", "PP", "DD")),
+             (2, ("PP", "PP", "DN")), (2, ("ND", "NN", "DN"))]        # wall below, outflow / free-slip top: face nz-1 is an unknown
     for stagger, (px, py, pz) in cases:
         bc = ((px[0], px[1]), (py[0], py[1]), (pz[0], pz[1]))
         dzc, dzf = grid(nz, lz, stretch, pz == "PP")
