@@ -105,3 +105,33 @@ def test_the_same_call_twice_gives_the_same_bits(B):
     a = _case(B, 3, 256, 64, 70, bc, 1.0, 0.0)
     b = _case(B, 3, 256, 64, 70, bc, 1.0, 0.0)
     assert a[0] == a[1] == b[0] == b[1]
+
+
+@pytest.mark.gpu
+def test_largest_grid_the_fixed_array_admits(B):
+    """1024 x 1024 x 1024: nz at CANS_STATIC_MAX_NZ and exactly CANS_STATIC_MAX_CTAS CTAs, so every slot of the fixed array is
+    in use (26 GB of fields; generated on the device).  The maximum is planted once in the first CTA's cells and once in the
+    last one's: the plan-free call must find it, and agree with the planned call to the bit."""
+    nx = ny = nz = 1024
+    assert ((nx // 2) * ny // 256) * ((nz + 31) // 32) == B.STATIC_MAX_CTAS and nz == B.STATIC_MAX_NZ
+    lx, ly, lz = 2 * np.pi, np.pi, 2.0
+    bc = (("P", "P"), ("N", "N"), ("N", "N"))
+    gen = torch.Generator(device="cuda").manual_seed(11)
+    u, v, w = (1e-3 * torch.rand((nz, ny, nx), dtype=torch.float64, device="cuda", generator=gen) for _ in range(3))
+    plan = B.PoissonPlan(nx, ny, nz, lx, ly, lz, bc)
+    planned = torch.zeros((1,), dtype=torch.float64, device="cuda")
+    static = torch.zeros((1,), dtype=torch.float64, device="cuda")
+    for (k, j, i) in ((0, 0, 1), (nz - 1, ny - 1, nx - 2)):
+        old = float(u[k, j, i])
+        u[k, j, i] = 5.0
+        plan.chkdt(u, v, w, planned)
+        B.chkdt_static(u, v, w, static, lx, ly, lz, bc)
+        torch.cuda.synchronize()
+        assert float(static[0]) == float(planned[0])
+        assert float(static[0]) >= 5.0 * nx / lx                  # |u| / dx of the planted face alone
+        u[k, j, i] = old
+    plan.chkdt(u, v, w, planned)
+    B.chkdt_static(u, v, w, static, lx, ly, lz, bc)
+    torch.cuda.synchronize()
+    assert float(static[0]) == float(planned[0]) < 1.0            # and nothing of the planted runs is left behind
+    plan.close()
